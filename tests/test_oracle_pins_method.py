@@ -1,0 +1,414 @@
+"""Pins for the oracle's grid operators and for the whole method.
+
+Invariants the paper states, library routines on special cases
+(numpy/scipy convolutions), brute force on tiny inputs, the O(N^2) direct Coulomb sum and the
+rock-salt Madelung constant.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import Oracle
+from paper_2510_05961_b200.workloads import make_workload, rock_salt, open_random
+
+
+def small_system(periodic, n=60, seed=7, box=(12.0, 11.0, 10.0)):
+    rng = np.random.default_rng(seed)
+    pos = rng.random((n, 3)) * np.array(box)
+    q = rng.uniform(-1, 1, n)
+    q -= q.mean()
+    return pos, q, box
+
+
+# ---------------------------------------------------------------- geometry
+
+def test_grid_extents_periodic_and_open():
+    o = Oracle((45.12,) * 3, (1, 1, 1), 1.41, 8.0, 4, 1)
+    assert o.L == 6                                                   # 32 -> 1
+    assert [o.level_info(l)["M"][0] for l in range(1, 7)] == [32, 16, 8, 4, 2, 1]
+    assert o.level_info(1)["h"][0] == pytest.approx(45.12 / 32)
+    o = Oracle((20.0,) * 3, (0, 0, 0), 2.0, 6.0, 4, 3)
+    assert [o.level_info(l)["M"] for l in (1, 2, 3)] == [(14,) * 3, (9,) * 3, (6,) * 3]
+    o = Oracle((100.0, 100.0, 40.0), (1, 1, 0), 1.5, 10.0, 6, 4)
+    assert o.L == 7
+    assert [o.level_info(l)["M"] for l in range(1, 8)] == [
+        (64, 64, 32), (32, 32, 19), (16, 16, 12), (8, 8, 9), (4, 4, 7), (2, 2, 6), (1, 1, 6)]
+    with pytest.raises(ValueError):
+        Oracle((10.0, 10.0, 10.0), (1, 0, 0), 1.0, 3.0, 4, 2)          # one periodic axis: T4
+    with pytest.raises(ValueError):
+        Oracle((10.0, 10.0, 10.0), (1, 1, 1), 1.0, 5.1, 4, 2)          # a > L/2
+
+
+# ---------------------------------------------------------------- anterpolation / restriction
+
+@pytest.mark.parametrize("periodic,p", [((1, 1, 1), 4), ((0, 0, 0), 4), ((1, 1, 0), 6), ((1, 1, 1), 6)])
+def test_grid_charge_conserved_on_every_level(periodic, p):
+    pos, q, box = small_system(periodic)
+    q = q + 0.37                                              # non-neutral on purpose
+    o = Oracle((16.0, 16.0, 16.0), periodic, 1.0, 3.0, p, 3)
+    o.anterpolate(pos, q)
+    for l in range(1, o.L):
+        o.restrict(l)
+    for l in range(1, o.L + 1):
+        assert o.grid(l, "Q").sum() == pytest.approx(q.sum(), rel=1e-12)
+
+
+def test_anterpolation_first_moment():
+    # B-splines reproduce linear functions: sum_m x_m Q_m = sum_i q_i x_i (open box, Eq. 9)
+    pos, q, box = small_system((0, 0, 0))
+    o = Oracle(box, (0, 0, 0), 1.0, 3.0, 4, 2)
+    Q = o.anterpolate(pos, q)
+    info = o.level_info(1)
+    for ax in range(3):
+        coords = (np.arange(info["M"][ax]) + info["lo"][ax]) * info["h"][ax]
+        shape = [1, 1, 1]; shape[2 - ax] = -1
+        assert (Q * coords.reshape(shape)).sum() == pytest.approx((q * pos[:, ax]).sum(), abs=1e-11)
+
+
+@pytest.mark.parametrize("periodic,p,box", [((1, 1, 1), 4, (16.0,) * 3), ((1, 1, 1), 6, (16.0,) * 3),
+                                            ((0, 0, 0), 4, (20.0,) * 3)])
+def test_restricted_charge_equals_coarse_anterpolation(periodic, p, box):
+    # q~^l = I q~^(l-1) holds exactly for nested B-splines
+    rng = np.random.default_rng(3)
+    pos = rng.random((50, 3)) * np.array(box)
+    q = rng.uniform(-1, 1, 50)
+    fine = Oracle(box, periodic, 1.0, 3.0, p, 2)
+    coarse = Oracle(box, periodic, 2.0, 3.0, p, 1)
+    fine.anterpolate(pos, q)
+    Q2 = fine.restrict(1)
+    Qc = coarse.anterpolate(pos, q)
+    assert fine.level_info(2)["M"] == coarse.level_info(1)["M"]
+    assert fine.level_info(2)["lo"] == coarse.level_info(1)["lo"]
+    assert Q2 == pytest.approx(Qc, abs=1e-13)
+
+
+@pytest.mark.parametrize("periodic,p", [((1, 1, 1), 4), ((0, 0, 0), 6), ((1, 1, 0), 4)])
+def test_prolongation_is_transpose_of_restriction(periodic, p):
+    # I_l^(l-1) = (I_(l-1)^l)^T  <=>  <I q, e> = <q, I^T e>
+    o = Oracle((16.0, 16.0, 12.0), periodic, 1.0, 3.0, p, 3)
+    rng = np.random.default_rng(5)
+    for l in (1, 2):
+        qf = rng.standard_normal(o.grid(l, "Q").shape)
+        ec = rng.standard_normal(o.grid(l + 1, "E").shape)
+        o.set_grid(l, "Q", qf)
+        Iq = o.restrict(l)
+        o.set_grid(l, "E", np.zeros_like(qf)); o.set_grid(l + 1, "E", ec)
+        ITe = o.prolong_add(l)
+        assert (Iq * ec).sum() == pytest.approx((qf * ITe).sum(), rel=1e-12)
+
+
+def test_restriction_matches_numpy_convolution_1d():
+    # a grid varying along x only, periodic: (I q)_m = sum_n J_(n-2m) q_n  via numpy on a tiled copy
+    o = Oracle((16.0,) * 3, (1, 1, 1), 1.0, 3.0, 4, 2)
+    rng = np.random.default_rng(11)
+    line = rng.standard_normal(16)
+    o.set_grid(1, "Q", np.broadcast_to(line, (16, 16, 16)).copy())
+    Q2 = o.restrict(1)
+    J = oracle.two_scale(4)
+    full = np.convolve(np.tile(line, 3), J[::-1], mode="same")[16:32]   # correlation with J
+    ref = full[0::2] * J.sum()**2                                      # y and z passes see constants: factor (sum J)
+    assert Q2[0, 0, :] == pytest.approx(ref, rel=1e-12)
+
+
+# ---------------------------------------------------------------- stencils and convolution
+
+def test_stencil_assembly_matches_numpy_separable_convolution():
+    # Eq. 20: K = w' (x) w' (x) w' * k_l(h o n), here re-assembled with numpy.convolve
+    o = Oracle((20.0, 20.0, 20.0), (1, 1, 1), 2.5, 5.0, 4, 1, mu=2)       # M=8, L=4
+    w = oracle.omega(4, 2); hw = len(w) // 2
+    for l in (1, 2):
+        info = o.level_info(l)
+        Kr = info["Kr"]; h = info["h"]
+        K = o.stencil(l)
+        R = [k - hw for k in Kr]
+        n = [np.arange(-r, r + 1) for r in R]
+        zz, yy, xx = np.meshgrid(n[2] * h[2], n[1] * h[1], n[0] * h[0], indexing="ij")
+        rr = np.sqrt(xx**2 + yy**2 + zz**2)
+        s = np.vectorize(lambda r: oracle.kernel(4, 5.0, o.L, l, r))(rr)
+        ref = s
+        for ax in range(3):
+            ref = np.apply_along_axis(lambda v: np.convolve(v, w), ax, ref)
+        assert K.shape == ref.shape
+        assert K == pytest.approx(ref, abs=1e-15)
+    # intermediate stencils are K^1 divided by two, repeatedly
+    assert o.stencil(2) == pytest.approx(o.stencil(1) / 2, abs=1e-16)
+    assert o.stencil(3) == pytest.approx(o.stencil(1) / 4, abs=1e-16)
+
+
+def test_stencil_symmetric():
+    o = Oracle((20.0, 20.0, 10.0), (1, 1, 0), 1.3, 4.0, 4, 3)
+    for l in (1, 2):
+        K = o.stencil(l)
+        assert K == pytest.approx(K[::-1, ::-1, ::-1], abs=1e-14)
+        assert K == pytest.approx(np.swapaxes(K, 1, 2), abs=1e-14)      # h_x == h_y
+
+
+@pytest.mark.parametrize("periodic", [(1, 1, 1), (0, 0, 0), (1, 1, 0)])
+def test_convolution_matches_library(periodic):
+    # Eq. 11 against scipy.signal / FFT circular convolution on a padded / tiled array
+    from scipy.signal import fftconvolve
+    o = Oracle((8.0, 8.0, 8.0), periodic, 1.0, 2.0, 4, 2, mu=1)
+    l = 1
+    info = o.level_info(l)
+    M = info["M"]
+    K = o.stencil(l)
+    rng = np.random.default_rng(9)
+    q = rng.standard_normal((M[2], M[1], M[0]))
+    got = o.apply_stencil(l, q)
+    # embed q in the middle of a 3x3x3 tiling (periodic axes) or zero padding (open axes)
+    reps = q
+    for ax_np, per in zip((0, 1, 2), periodic[::-1]):
+        pad = reps.shape[ax_np]
+        if per:
+            reps = np.concatenate([reps] * 5, axis=ax_np)
+        else:
+            z = np.zeros_like(reps)
+            reps = np.concatenate([z, z, reps, z, z], axis=ax_np)
+    full = fftconvolve(reps, K, mode="same")
+    sl = tuple(slice(2 * n, 3 * n) for n in q.shape)
+    assert got == pytest.approx(full[sl], abs=1e-11)
+
+
+# ---------------------------------------------------------------- short range
+
+@pytest.mark.parametrize("periodic,box", [((1, 1, 1), (12.0, 11.0, 10.0)), ((0, 0, 0), (12.0, 11.0, 10.0)),
+                                          ((1, 1, 0), (8.0, 7.0, 13.0))])
+def test_short_range_cells_equal_brute_force(periodic, box):
+    pos, q, box = small_system(periodic, n=300, box=box)
+    o = Oracle(box, periodic, 1.0, 3.4, 4, 2)
+    Fb, Vb, Wb = o.short_range(pos, q, method="brute")
+    Fc, Vc, Wc = o.short_range(pos, q, method="cells")
+    assert Fc == pytest.approx(Fb, abs=1e-12)
+    assert Vc == pytest.approx(Vb, abs=1e-12)
+    assert Wc == pytest.approx(Wb, abs=1e-11)
+    sel = np.array([0, 17, 299], dtype=np.int32)
+    Fs, Vs, _ = o.short_range(pos, q, sel=sel)
+    assert Fs == pytest.approx(Fb[sel], abs=1e-14) and Vs == pytest.approx(Vb[sel], abs=1e-14)
+
+
+def test_short_range_against_numpy_minimum_image():
+    pos, q, box = small_system((1, 1, 0), n=80, box=(8.0, 7.0, 13.0))
+    a = 3.4
+    o = Oracle(box, (1, 1, 0), 1.0, a, 4, 2)
+    F, V, W = o.short_range(pos, q)
+    d = pos[:, None, :] - pos[None, :, :]
+    for ax in (0, 1):
+        d[..., ax] -= box[ax] * np.round(d[..., ax] / box[ax])
+    r = np.sqrt((d**2).sum(-1)); np.fill_diagonal(r, np.inf)
+    k0 = np.vectorize(lambda x: oracle.kernel(4, a, 3, 0, x) if x < a else 0.0)(r)
+    assert V == pytest.approx((k0 * q[None, :]).sum(1), abs=1e-13)
+    # the short-range energy must equal the direct Coulomb energy minus the smooth part
+    U0 = 0.5 * (q * V).sum()
+    smooth = np.vectorize(lambda x: oracle.gamma(4, x / a) / a if x < a else 1 / x)(r)
+    coul = np.where(np.isfinite(r), 1 / r, 0.0)
+    assert U0 == pytest.approx(0.5 * (q[:, None] * q[None, :] * (coul - np.where(np.isfinite(r), smooth, 0))).sum(), rel=1e-12)
+
+
+# ---------------------------------------------------------------- whole method: exact references
+
+def test_config1_against_direct_sum():
+    # BASELINE.json configs[0]: checked against the O(N^2) direct Coulomb sum
+    w = make_workload("cfg1_open512")
+    U, F, V = oracle.direct_sum(w.positions, w.charges)
+    errs = {}
+    for mu in (0, 4):
+        r = Oracle(w.box, w.periodic, w.h, w.a, w.p, w.levels, mu=mu).evaluate(w.positions, w.charges)
+        errs[mu] = (abs(r["energy"] - U) / abs(U),
+                    np.sqrt(((r["forces"] - F)**2).mean() / (F**2).mean()),
+                    np.sqrt(((r["potentials"] - V)**2).mean()) / V.std())
+    assert errs[4][0] < 2e-3 and errs[4][1] < 4e-3 and errs[4][2] < 5e-3
+    assert errs[0][0] < 0.15 and errs[0][1] < 2e-2
+    assert errs[4][0] < errs[0][0] and errs[4][1] < errs[0][1]
+
+
+def test_open_system_converges_to_direct_sum():
+    # error falls as h shrinks and a grows; p = 6 beats p = 4 at the same cost parameters
+    pos, q = open_random(200, 12.0, 99)
+    U, F, V = oracle.direct_sum(pos, q)
+
+    def ferr(h, a, p, levels):
+        r = Oracle((12.0,) * 3, (0, 0, 0), h, a, p, levels).evaluate(pos, q, want_virial=False)
+        return np.sqrt(((r["forces"] - F)**2).mean() / (F**2).mean()), abs(r["energy"] - U) / abs(U)
+    e1 = ferr(2.0, 4.0, 4, 2)
+    e2 = ferr(1.0, 4.0, 4, 2)
+    e3 = ferr(1.0, 6.0, 4, 2)
+    e4 = ferr(1.0, 6.0, 6, 2)
+    assert e1[0] > e2[0] > e3[0] > e4[0]
+    assert e4[0] < 2e-4 and e4[1] < 1e-4
+    # one level or three: the same Coulomb sum within MSM error
+    e5 = ferr(1.0, 6.0, 6, 1)
+    e6 = ferr(1.0, 3.0, 6, 3)
+    assert e5[0] < 5e-4 and e6[0] < 5e-3
+
+
+def test_madelung_constant_rock_salt(golden):
+    # P:306-318; BASELINE.json configs[1] shape (smaller supercell: the result per ion is the same)
+    Mref = golden["madelung_nacl"]["more_digits"]
+    assert abs(Mref - golden["madelung_nacl"]["value"]) < 5e-7
+    pos, q = rock_salt(4, 5.64)
+    L = 4 * 5.64
+
+    def madelung(h, a, p, mu):
+        r = Oracle((L,) * 3, (1, 1, 1), h, a, p, 1, mu=mu).evaluate(pos, q, want_virial=False)
+        assert np.abs(r["forces"]).max() < 1e-12            # forces vanish by symmetry
+        return -r["energy"] * 2.82 / (len(q) / 2)
+    m0 = madelung(1.41, 8.0, 4, 0)
+    m4 = madelung(1.41, 8.0, 4, 4)
+    assert abs(m4 - Mref) < 2e-4                            # "within MSM error"
+    assert abs(m0 - Mref) < 6e-3
+    assert abs(m4 - Mref) < abs(m0 - Mref)
+    # tighter parameters: p = 6, larger cutoff, finer grid -> many decimals
+    m6 = madelung(0.705, 11.0, 6, 4)
+    assert abs(m6 - Mref) < 5e-6
+
+
+def test_madelung_same_for_supercells():
+    def madelung(nc):
+        pos, q = rock_salt(nc, 5.64)
+        L = nc * 5.64
+        r = Oracle((L,) * 3, (1, 1, 1), 1.41, 5.0, 4, 1).evaluate(pos, q, want_virial=False)
+        return -r["energy"] * 2.82 / (len(q) / 2)
+    assert madelung(2) == pytest.approx(madelung(4), rel=1e-11)
+
+
+def test_slab_against_brute_force_image_sum():
+    # reading T3, pinned by brute force: images |n_x|,|n_y| <= n, extrapolated in 1/n
+    rng = np.random.default_rng(7)
+    box = (10.0, 10.0, 4.0)
+    pos = rng.random((40, 3)) * np.array(box)
+    q = rng.uniform(-1, 1, 40); q -= q.mean()
+    us = {}
+    for n in (40, 80, 160):
+        us[n] = oracle.direct_sum(pos, q, box, (1, 1, 0), nimg=n, want_fv=False)[0]
+    # error ~ c/n + d/n^2: two Richardson steps
+    r1 = 2 * us[80] - us[40]; r2 = 2 * us[160] - us[80]
+    uref = (4 * r2 - r1) / 3
+    assert abs(r2 - r1) < 1e-4
+    errs = []
+    for m1 in (8, 16, 32):
+        r = Oracle(box, (1, 1, 0), 10.0 / m1, 5.0, 6, 1).evaluate(pos, q, want_virial=False)
+        errs.append(abs(r["energy"] - uref))
+    assert errs[0] < 5e-3 and errs[1] < 1e-4 and errs[2] < 2e-5
+    assert errs[0] > errs[1] > errs[2]
+
+
+# ---------------------------------------------------------------- derivatives (Eq. 17-18, reading V)
+
+@pytest.mark.parametrize("periodic,p,box", [((1, 1, 1), 4, (12.0,) * 3), ((0, 0, 0), 4, (12.0,) * 3),
+                                            ((1, 1, 0), 6, (12.0, 12.0, 8.0))])
+def test_forces_and_potentials_are_energy_derivatives(periodic, p, box):
+    pos, q, _ = small_system(periodic, n=40, box=box)
+    pos = 0.5 + pos * (np.array(box) - 1.0) / np.array(box)     # keep clear of the open faces
+    o = Oracle(box, periodic, 1.5, 4.0, p, 2)
+    r = o.evaluate(pos, q)
+    assert r["energy"] == pytest.approx(0.5 * (q * r["potentials"]).sum(), rel=1e-13)
+    d = 1e-5
+    for i in (0, 13, 39):
+        for ax in range(3):
+            pp = pos.copy(); pm = pos.copy()
+            pp[i, ax] += d; pm[i, ax] -= d
+            fd = -(o.evaluate(pp, q, False)["energy"] - o.evaluate(pm, q, False)["energy"]) / (2 * d)
+            assert r["forces"][i, ax] == pytest.approx(fd, rel=2e-6, abs=1e-8)
+        qp = q.copy(); qm = q.copy()
+        qp[i] += d; qm[i] -= d
+        fd = (o.evaluate(pos, qp, False)["energy"] - o.evaluate(pos, qm, False)["energy"]) / (2 * d)
+        assert r["potentials"][i] == pytest.approx(fd, rel=1e-8, abs=1e-9)
+
+
+@pytest.mark.parametrize("periodic,box", [((1, 1, 1), (12.0, 13.0, 14.0)), ((1, 1, 0), (12.0, 13.0, 8.0))])
+def test_virial_is_strain_derivative_per_axis(periodic, box):
+    # W_aa = -dU/d eps_aa with the number of grid points fixed and a fixed (reading V)
+    pos, q, _ = small_system(periodic, n=40, box=box)
+    h, a, p = 1.5, 4.0, 4
+    r = Oracle(box, periodic, h, a, p, 2).evaluate(pos, q)
+    e = 1e-5
+    for ax in range(3):
+        if not periodic[ax]:
+            continue                        # an open axis has no own spacing parameter; see isotropic test
+        us = []
+        for s in (+e, -e):
+            b = list(box); b[ax] *= (1 + s)
+            pp = pos.copy(); pp[:, ax] *= (1 + s)
+            us.append(Oracle(b, periodic, h, a, p, 2).evaluate(pp, q, False)["energy"])
+        fd = -(us[0] - us[1]) / (2 * e)
+        assert r["virial"][ax] == pytest.approx(fd, rel=1e-6, abs=1e-8)
+
+
+@pytest.mark.parametrize("periodic,box", [((0, 0, 0), (12.0, 12.0, 12.0)), ((1, 1, 0), (12.0, 12.0, 6.0)),
+                                          ((1, 1, 1), (12.0, 12.0, 12.0))])
+def test_virial_trace_is_isotropic_strain_derivative(periodic, box):
+    pos, q, _ = small_system(periodic, n=40, box=box)
+    h, a, p = 1.5, 4.0, 4
+    r = Oracle(box, periodic, h, a, p, 2).evaluate(pos, q)
+    e = 1e-5
+    us = []
+    for s in (+e, -e):
+        b = [x * (1 + s) for x in box]
+        us.append(Oracle(b, periodic, h * (1 + s), a, p, 2).evaluate(pos * (1 + s), q, False)["energy"])
+    fd = -(us[0] - us[1]) / (2 * e)
+    assert r["virial"][:3].sum() == pytest.approx(fd, rel=1e-6)
+    # exact Coulomb is homogeneous of degree -1: tr W = U; MSM agrees within its error
+    # (coarse parameters here: h = 1.5, a = 4)
+    assert r["virial"][:3].sum() == pytest.approx(r["energy"], rel=0.25)
+
+
+def test_virial_open_system_matches_sum_r_f():
+    # open system: W_ab ~ sum_i r_ia F_ib (exact for exact Coulomb): fixes sign and index order of
+    # the off-diagonal components within MSM error
+    pos, q = open_random(150, 10.0, 5)
+    o = Oracle((10.0,) * 3, (0, 0, 0), 1.0, 5.0, 6, 2)
+    r = o.evaluate(pos, q)
+    U, F, V = oracle.direct_sum(pos, q)
+    ref = pos.T @ F
+    W = r["virial"]
+    full = np.array([[W[0], W[3], W[4]], [W[3], W[1], W[5]], [W[4], W[5], W[2]]])
+    assert full == pytest.approx(ref, abs=5e-3 * np.abs(ref).max())
+    # swapping the x and y coordinates of every particle swaps the components accordingly
+    r2 = o.evaluate(pos[:, [1, 0, 2]], q)["virial"]
+    assert r2[[1, 0, 2, 3, 5, 4]] == pytest.approx(W, rel=1e-10, abs=1e-10)
+
+
+# ---------------------------------------------------------------- invariances
+
+def test_zero_charge_padding_changes_nothing():
+    # P:326
+    pos, q, box = small_system((1, 1, 1), n=50, box=(12.0,) * 3)
+    o = Oracle(box, (1, 1, 1), 1.5, 4.0, 4, 1)
+    r = o.evaluate(pos, q)
+    rng = np.random.default_rng(2)
+    pos2 = np.concatenate([pos, rng.random((17, 3)) * 12.0]); q2 = np.concatenate([q, np.zeros(17)])
+    r2 = o.evaluate(pos2, q2)
+    assert r2["energy"] == pytest.approx(r["energy"], rel=1e-13)
+    assert r2["forces"][:50] == pytest.approx(r["forces"], abs=1e-13)
+    assert r2["forces"][50:] == pytest.approx(np.zeros((17, 3)), abs=0)
+    assert r2["virial"] == pytest.approx(r["virial"], rel=1e-12)
+
+
+def test_periodic_translation_by_box_vector_and_wrapping():
+    pos, q, box = small_system((1, 1, 0), n=50, box=(12.0, 12.0, 8.0))
+    o = Oracle(box, (1, 1, 0), 1.5, 4.0, 4, 1)
+    r = o.evaluate(pos, q)
+    shifted = pos + np.array([12.0, -24.0, 0.0])
+    r2 = o.evaluate(shifted, q)
+    assert r2["energy"] == pytest.approx(r["energy"], rel=1e-12)
+    assert r2["forces"] == pytest.approx(r["forces"], abs=1e-11)
+    with pytest.raises(ValueError):
+        o.evaluate(pos + np.array([0, 0, 8.1]), q)          # open coordinate outside the box
+
+
+def test_rigid_shift_changes_result_only_within_msm_error():
+    pos, q = rock_salt(4, 5.64)
+    L = 4 * 5.64
+    o = Oracle((L,) * 3, (1, 1, 1), 1.41, 8.0, 4, 1)
+    u0 = o.evaluate(pos, q, False)["energy"]
+    sh = pos + np.array([0.37, 0.11, 0.93])
+    u1 = o.evaluate(sh - L * np.floor(sh / L), q, False)["energy"]
+    assert u1 == pytest.approx(u0, rel=1e-3)
+    assert u1 != u0
+
+
+def test_open_levels_change_only_msm_error_and_periodic_ignores_levels():
+    pos, q, box = small_system((1, 1, 1), n=50, box=(12.0,) * 3)
+    e1 = Oracle(box, (1, 1, 1), 1.5, 4.0, 4, 1).evaluate(pos, q, False)["energy"]
+    e3 = Oracle(box, (1, 1, 1), 1.5, 4.0, 4, 3).evaluate(pos, q, False)["energy"]
+    assert e1 == e3                                           # reading G4
