@@ -1,0 +1,143 @@
+/* include/msm.h -- C ABI of libmsm_b200: the multilevel summation method (MSM) with B-spline
+ * interpolation for point charges (arxiv 2510.05961, "msmJAX"; PAPER.md cited as P:<line>) as
+ * hand-written CUDA for sm_100a.
+ *
+ * One evaluation computes, for N point charges in an orthorhombic box with full, mixed (two
+ * periodic axes) or no periodicity, the MSM approximation of
+ *     U = 1/2 sum_i sum_{j != i} q_i q_j / r_ij                               (Eq. 1, k(r) = 1/r)
+ * together with forces -grad_i U, potentials dU/dq_i (the "charge gradient", Eq. 18) and the
+ * virial -dU/d eps (the stress of P:31 times the volume, sign flipped).  Coulomb constant 1
+ * (P:300).  The stages behind msm_evaluate are the paper's: short-range pair sum of k_0 with the
+ * self term (Eq. 5), anterpolation (Eq. 9, Alg. 1), restriction / prolongation
+ * (Eq. 19), per-level stencil convolution (Eq. 11; stencils P:268 Eq. 20 from the
+ * splitting P:276 Eq. 21), the top level, and interpolation with its derivatives (P:220-230
+ * Eq. 16-18).  Where PAPER.md is silent the readings of DESIGN.md apply (K1, K2, G1-G4, J1, Q,
+ * T1-T4, V).
+ *
+ * No torch types cross this boundary: plain pointers (host or device, as stated) and sizes.
+ * Nothing here throws or aborts; every call returns msm_status_t.  There is no CPU fallback: a
+ * call fails with MSM_ERR_CUDA if no CUDA device is usable.
+ */
+#ifndef MSM_B200_H
+#define MSM_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct msm_plan msm_plan_t; /* opaque; owns all device and host scratch buffers */
+
+typedef enum {
+  MSM_OK = 0,
+  MSM_ERR_INVALID_ARG = 1,        /* non-positive box/h/a, odd or unsupported p, levels < 1, NULL */
+  MSM_ERR_UNSUPPORTED = 2,        /* exactly one periodic axis (reading T4); unequal periodic grid
+                                     counts (reading B3); top grid larger than MSM_MAX_TOP_POINTS */
+  MSM_ERR_CUTOFF_TOO_LARGE = 3,   /* periodic axis with a > box/2: minimum image invalid */
+  MSM_ERR_TOO_MANY_PARTICLES = 4, /* n > max_particles */
+  MSM_ERR_OUT_OF_BOX = 5,         /* open-axis coordinate outside [0, box], or non-finite input */
+  MSM_ERR_NOMEM = 6,
+  MSM_ERR_CUDA = 7
+} msm_status_t;
+
+typedef enum { MSM_FP64 = 0, MSM_FP32 = 1 } msm_precision_t;
+
+#define MSM_MAX_LEVELS 32
+#define MSM_MAX_TOP_POINTS 4096
+
+/* The paper's statement of the problem (cutoff, spacing, order; cell; periodicity). */
+typedef struct {
+  double box[3];     /* orthorhombic edge lengths; the box is [0,box_x) x [0,box_y) x [0,box_z)   */
+  int periodic[3];   /* per axis: 1 periodic, 0 open                                             */
+  double h;          /* target finest grid spacing h_1.  Periodic axes use M_1 = 2^round(log2(box/h))
+                        points (reading G1); open axes use h exactly              */
+  double a;          /* level-zero cutoff r_cut^(0) (Eq. 3)                                 */
+  int p;             /* B-spline order (support in grid cells; degree p-1): 4, 6 or 8      */
+  int levels;        /* open box: number of grid levels L (the last is summed densely, untruncated
+                        k_L).  Periodic / mixed: number of grids run as tiled stages; the rest of
+                        the hierarchy, down to one point per periodic axis, is folded into
+                        one dense operator at plan time; the result does not depend on it (G4)   */
+  int precision;     /* msm_precision_t: element type of ALL particle and grid arrays            */
+  int mu;            /* extra quasi-interpolation terms in omega' (reading Q); < 0: default 4     */
+  int max_particles; /* capacity; msm_evaluate with n above it fails                             */
+  int device;        /* CUDA device ordinal                                                      */
+} msm_params_t;
+
+typedef struct {
+  int L_full;                        /* number of grid levels of the method              */
+  int n_tiled;                       /* levels run as tiled stages; level n_tiled is the top grid */
+  int mu;                            /* omega' setting in use                                    */
+  int omega_halfwidth;               /* p/2 - 1 + mu                                             */
+  int grid_dims[MSM_MAX_LEVELS][3];  /* points per axis, levels 1..L_full at index l-1            */
+  int grid_lo[MSM_MAX_LEVELS][3];    /* node index of the first point (0 on periodic axes)       */
+  double grid_h[MSM_MAX_LEVELS][3];  /* spacing per axis                                         */
+  int stencil_taps[MSM_MAX_LEVELS];  /* taps of the sampled stencil inside the cutoff ellipsoid  */
+  int pair_cells[3];                 /* short-range cell grid                                    */
+  int top_points;                    /* points of the top grid (size of the dense operator)      */
+  size_t device_bytes;               /* device memory owned by the plan                          */
+} msm_plan_info_t;
+
+/* Build a plan: all host-side mathematics in fp64 (grid hierarchy, two-scale mask J, quasi-
+ * interpolation sequence omega', sampled stencils of every k_l and of their strain derivatives,
+ * the dense top-level operator, cell-list geometry) and every device buffer for up to
+ * max_particles.  On failure *plan_out is NULL. */
+msm_status_t msm_plan_create(const msm_params_t *params, msm_plan_t **plan_out);
+
+msm_status_t msm_plan_info(const msm_plan_t *plan, msm_plan_info_t *info_out);
+
+/* One evaluation, enqueued on cuda_stream (a cudaStream_t; NULL = the default stream).
+ *   d_positions  device, n x 3 row-major (x,y,z per particle), plan precision; not modified.
+ *                Periodic coordinates are wrapped into the box; open coordinates must lie in
+ *                [0, box] (else MSM_ERR_OUT_OF_BOX, reported after the call completes).
+ *   d_charges    device, n, plan precision; not modified.
+ *   d_forces     device, n x 3, plan precision, caller order; may be NULL.
+ *   d_potentials device, n, dU/dq_i, so that U = 1/2 sum q_i potentials_i; may be NULL.
+ *   h_energy     host, 1 double; may be NULL.
+ *   h_virial     host, 6 doubles xx yy zz xy xz yz of -dU/d eps_ab (number of grid points and a
+ *                fixed, reading V); may be NULL (the strain-derivative work is then skipped).
+ * The caller owns all six buffers; the plan owns every scratch buffer and msm_evaluate allocates
+ * nothing.  Device outputs are stream-ordered; the call synchronises the stream before returning
+ * (it always reads back the status flag, the energy and the virial in one small copy).
+ * Neutrality is assumed on periodic axes: the single-point top level contributes zero (reading
+ * T2), which for a non-neutral input is the neutralising-background convention. */
+msm_status_t msm_evaluate(msm_plan_t *plan, int n, const void *d_positions, const void *d_charges,
+                          void *d_forces, void *d_potentials, double *h_energy, double *h_virial,
+                          void *cuda_stream);
+
+/* The same call with HOST buffers (the end-to-end path): copies positions and charges to plan-
+ * owned device staging, evaluates, copies forces and potentials back. Pointers are host memory
+ * (pinned memory makes the copies asynchronous). */
+msm_status_t msm_evaluate_host(msm_plan_t *plan, int n, const void *h_positions,
+                               const void *h_charges, void *h_forces, void *h_potentials,
+                               double *h_energy, double *h_virial, void *cuda_stream);
+
+/* Per-stage CUDA-event timing of the following msm_evaluate calls (off by default; when on, the
+ * stages run back to back on one stream with an event between them). */
+msm_status_t msm_set_profiling(msm_plan_t *plan, int enabled);
+
+/* Stage names and milliseconds of the last profiled evaluate. The arrays belong to the plan. */
+msm_status_t msm_get_stage_times(const msm_plan_t *plan, int *n_stages, const char *const **names,
+                                 const float **milliseconds);
+
+/* Number of kernels the last msm_evaluate launched (counted at the launch sites). */
+msm_status_t msm_get_launch_count(const msm_plan_t *plan, int *count);
+
+/* Parity taps: copy a grid of the last evaluate to the host as doubles, indexed [z][y][x].
+ * kind 0: grid charge Q^l, 1: potential E^l (after prolongation), for 1 <= level <= n_tiled. */
+msm_status_t msm_debug_copy_grid(const msm_plan_t *plan, int level, int kind, double *h_out,
+                                 size_t capacity);
+
+void msm_plan_destroy(msm_plan_t *plan);
+
+const char *msm_status_string(msm_status_t s);
+
+/* Microbenchmarks used for the roofline denominators the driver does not provide (FP32 / FP64
+ * FMA peak of the CUDA cores).  kind 0: FFMA, 1: DFMA.  Returns TFLOP/s (2 flops per FMA) through
+ * *tflops, timed with CUDA events on the given device. */
+msm_status_t msm_measure_fma_peak(int device, int kind, double *tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MSM_B200_H */

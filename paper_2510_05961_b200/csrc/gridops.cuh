@@ -1,0 +1,138 @@
+// gridops.cuh -- S4 restriction and S7 prolongation (Eq. 19, separable, one axis at a
+// time), and the omega' pre-filter that writes the haloed (padded) copy of a level's grid
+// charge which the stencil convolution reads (Eq. 20's omega' factors moved from the stencil to the
+// grid charge: K * q = s * (omega' (x) omega' (x) omega' * q)).
+//
+// One thread per output element; x is the fastest index in every array, so each warp reads and
+// writes contiguous runs (the grids at config sizes are L2-resident).
+#pragma once
+#include "device_common.cuh"
+
+namespace msm {
+
+constexpr int kMaxAxisTaps = 2 * 32 + 1;
+
+template <typename T> struct AxisTaps {
+  int n;                  // number of taps, offsets -(n/2) .. n/2
+  T c[kMaxAxisTaps];
+};
+
+struct AxisDims {
+  int in[3], out[3];      // array dims (x, y, z)
+  int axis;
+  int periodic;
+};
+
+__device__ __forceinline__ size_t lin(const int d[3], int x, int y, int z) {
+  return ((size_t)z * d[1] + y) * d[0] + x;
+}
+
+// out[o] = sum_k w[k] in_logical[o - H - k]: omega' filter that also lays down the halo.
+// Logical input index i: periodic -> in[i mod M]; open -> in[i] inside [0, M), else 0.
+template <typename T>
+__global__ void k_pad_filter(AxisDims d, int H, AxisTaps<T> w, const T* __restrict__ in, T* __restrict__ out) {
+  const size_t total = (size_t)d.out[0] * d.out[1] * d.out[2];
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= total) return;
+  int c[3] = {(int)(t % d.out[0]), (int)((t / d.out[0]) % d.out[1]), (int)(t / ((size_t)d.out[0] * d.out[1]))};
+  const int g = c[d.axis] - H, M = d.in[d.axis], hw = w.n / 2;
+  T acc = 0;
+  for (int k = -hw; k <= hw; ++k) {
+    int i = g - k;
+    if (d.periodic) i = imod(i, M);
+    else if (i < 0 || i >= M) continue;
+    c[d.axis] = i;
+    acc = fma(w.c[k + hw], in[lin(d.in, c[0], c[1], c[2])], acc);
+  }
+  out[t] = acc;
+}
+
+// out[m] = sum_n J_n in[2(m + lo_out) + n - lo_in]   (restriction along one axis)
+template <typename T>
+__global__ void k_restrict_axis(AxisDims d, int lo_in, int lo_out, AxisTaps<T> J, const T* __restrict__ in,
+                                T* __restrict__ out) {
+  const size_t total = (size_t)d.out[0] * d.out[1] * d.out[2];
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= total) return;
+  int c[3] = {(int)(t % d.out[0]), (int)((t / d.out[0]) % d.out[1]), (int)(t / ((size_t)d.out[0] * d.out[1]))};
+  const int m = c[d.axis], M = d.in[d.axis], hw = J.n / 2;
+  if (d.periodic && M == 1) { out[t] = in[lin(d.in, c[0], c[1], c[2])]; return; }
+  T acc = 0;
+  for (int n = -hw; n <= hw; ++n) {
+    int i = 2 * (m + lo_out) + n - lo_in;
+    if (d.periodic) i = imod(i, M);
+    else if (i < 0 || i >= M) continue;
+    c[d.axis] = i;
+    acc = fma(J.c[n + hw], in[lin(d.in, c[0], c[1], c[2])], acc);
+  }
+  out[t] = acc;
+}
+
+// out[i] (+)= sum_n J_n in[m], 2(m + lo_in) + n = i + lo_out   (prolongation = exact transpose)
+template <typename T, bool ADD>
+__global__ void k_prolong_axis(AxisDims d, int lo_in, int lo_out, AxisTaps<T> J, const T* __restrict__ in,
+                               T* __restrict__ out) {
+  const size_t total = (size_t)d.out[0] * d.out[1] * d.out[2];
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= total) return;
+  int c[3] = {(int)(t % d.out[0]), (int)((t / d.out[0]) % d.out[1]), (int)(t / ((size_t)d.out[0] * d.out[1]))};
+  const int i = c[d.axis], Mi = d.in[d.axis], Mo = d.out[d.axis], hw = J.n / 2;
+  T acc = 0;
+  if (d.periodic && Mo == 1) {
+    acc = in[lin(d.in, c[0], c[1], c[2])];
+  } else {
+    for (int n = -hw; n <= hw; ++n) {
+      int m;
+      if (d.periodic) {
+        const int v = imod(i - n, Mo);
+        if (v & 1) continue;
+        m = v >> 1;
+      } else {
+        const int v = i + lo_out - n;
+        if (v & 1) continue;
+        m = v / 2 - lo_in;            // v even (possibly negative): exact
+        if (m < 0 || m >= Mi) continue;
+      }
+      c[d.axis] = m;
+      acc = fma(J.c[n + hw], in[lin(d.in, c[0], c[1], c[2])], acc);
+    }
+  }
+  if (ADD) out[t] += acc; else out[t] = acc;
+}
+
+// S6: dense top-level operator e = T q, one warp per row; with VIRIAL also the six quadratic forms
+// q_r (TD_k q)_r per row (summed later in fixed order).
+template <typename T, bool VIRIAL>
+__global__ void __launch_bounds__(128)
+k_top_dense(int G, const T* __restrict__ Tm, const T* __restrict__ TD, const T* __restrict__ q,
+            T* __restrict__ e, double* __restrict__ wrow) {
+  const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  if (row >= G) return;
+  constexpr int NK = VIRIAL ? 7 : 1;
+  double acc[NK];
+#pragma unroll
+  for (int k = 0; k < NK; ++k) acc[k] = 0.0;
+  for (int col = lane; col < G; col += 32) {
+    const double qc = (double)q[col];
+    acc[0] += (double)Tm[(size_t)row * G + col] * qc;
+    if (VIRIAL) {
+#pragma unroll
+      for (int k = 0; k < 6; ++k) acc[k + 1] += (double)TD[((size_t)k * G + row) * G + col] * qc;
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < NK; ++k)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc[k] += __shfl_down_sync(0xffffffffu, acc[k], o);
+  if (lane == 0) {
+    e[row] = (T)acc[0];
+    if (VIRIAL) {
+      const double qr = (double)q[row];
+#pragma unroll
+      for (int k = 0; k < 6; ++k) wrow[(size_t)row * 6 + k] = -0.5 * qr * acc[k + 1];
+    }
+  }
+}
+
+}  // namespace msm

@@ -1,0 +1,282 @@
+// msm_create.cu -- msm_plan_create / msm_plan_destroy / msm_plan_info: host mathematics (fp64)
+// and every device buffer of a plan. See include/msm.h.
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "plan.hpp"
+
+namespace msm {
+const char* const kStageNames[kNumStages] = {"sort", "pair", "anterpolate", "restrict", "convolve",
+                                             "top", "prolongate", "interpolate", "reduce"};
+}
+
+using namespace msm;
+
+namespace {
+
+struct CudaFail {};
+
+void* dev_alloc(msm_plan* p, size_t bytes) {
+  void* d = nullptr;
+  if (bytes == 0) bytes = 16;
+  if (cudaMalloc(&d, bytes) != cudaSuccess) throw std::bad_alloc();
+  if (cudaMemset(d, 0, bytes) != cudaSuccess) throw CudaFail();
+  p->allocs.push_back(d);
+  p->bytes += bytes;
+  return d;
+}
+
+template <typename T> void* upload_as(msm_plan* p, const std::vector<double>& v) {
+  std::vector<T> t(v.size());
+  for (size_t i = 0; i < v.size(); ++i) t[i] = (T)v[i];
+  void* d = dev_alloc(p, std::max<size_t>(t.size(), 4) * sizeof(T));
+  if (!t.empty() && cudaMemcpy(d, t.data(), t.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess)
+    throw CudaFail();
+  return d;
+}
+
+void* upload(msm_plan* p, const std::vector<double>& v) {
+  return p->fp32 ? upload_as<float>(p, v) : upload_as<double>(p, v);
+}
+
+int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+// stencil row table + chunked taps of one tiled level (see conv.cuh)
+void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
+  const Level& lv = p->H->lev[l];
+  LevelDev& d = p->lev[l];
+  const SampledStencil st = sample_level_stencil(*p->H, *p->S, l);
+  d.taps = st.taps;
+  ConvGeom& g = d.cg;
+  for (int ax = 0; ax < 3; ++ax) { g.M[ax] = lv.M[ax]; g.R[ax] = st.R[ax]; }
+  g.X0 = round_up(st.R[0], 4);
+  g.tiles[0] = (lv.M[0] + XT - 1) / XT;
+  g.tiles[1] = (lv.M[1] + 31) / 32;
+  g.tiles[2] = (lv.M[2] + ZT - 1) / ZT;
+  g.P[0] = g.tiles[0] * XT + 2 * g.X0 + 4;
+  g.P[1] = g.tiles[1] * 32 + 2 * st.R[1];
+  g.P[2] = g.tiles[2] * ZT + 2 * st.R[2];
+  const int WX = XT + 2 * g.X0 + 4;
+  int pitch = WX;
+  if (p->fp32) { pitch = round_up(pitch, 4); if (((pitch / 4) & 1) == 0) pitch += 4; }
+  else { pitch = round_up(pitch, 2); if (((pitch / 2) & 1) == 0) pitch += 2; }
+  g.pitch = pitch;
+  d.smem = (size_t)(32 + 2 * st.R[1]) * pitch * p->esz;
+  d.units = g.tiles[0] * g.tiles[1] * g.tiles[2];
+
+  const double A = std::ldexp(p->mp.a, l);
+  const int ny = 2 * st.R[1] + 1, nz = 2 * st.R[2] + 1;
+  std::vector<int4> rows((size_t)ny * nz);
+  std::vector<double> ts, tg;
+  for (int dz = -st.R[2]; dz <= st.R[2]; ++dz)
+    for (int dy = -st.R[1]; dy <= st.R[1]; ++dy) {
+      int4& r = rows[(size_t)(dz + st.R[2]) * ny + (dy + st.R[1])];
+      const double y = dy * lv.h[1], z = dz * lv.h[2];
+      const double rem = A * A - y * y - z * z;
+      int Rx = -1;
+      if (rem > 0) {
+        Rx = std::min(st.R[0], (int)std::floor(std::sqrt(rem) / lv.h[0]));
+        while (Rx >= 0 && (Rx * lv.h[0]) * (Rx * lv.h[0]) >= rem) --Rx;
+      }
+      if (Rx < 0) { r = make_int4(0, 1, 0, 0); continue; }
+      const int clo = (-Rx + g.X0) / 4, chi = (Rx + g.X0) / 4;
+      r = make_int4((int)(ts.size() / 4), clo, chi, 0);
+      for (int c = clo; c <= chi; ++c)
+        for (int t = 0; t < 4; ++t) {
+          const int dx = 4 * c - g.X0 + t;
+          const bool in = dx >= -Rx && dx <= Rx;
+          ts.push_back(in ? st.at(st.s, dx, dy, dz) : 0.0);
+          tg.push_back(in ? st.at(st.g, dx, dy, dz) : 0.0);
+        }
+    }
+  d.rows = (int4*)dev_alloc(p, rows.size() * sizeof(int4));
+  if (cudaMemcpy(d.rows, rows.data(), rows.size() * sizeof(int4), cudaMemcpyHostToDevice) != cudaSuccess)
+    throw CudaFail();
+  d.staps = upload(p, ts);
+  d.gtaps = upload(p, tg);
+  d.pad = dev_alloc(p, (size_t)g.P[0] * g.P[1] * g.P[2] * p->esz);
+  d.wpart = (double*)dev_alloc(p, (size_t)d.units * 6 * sizeof(double));
+}
+
+msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
+  p->prm = *prm;
+  p->fp32 = prm->precision == MSM_FP32;
+  p->esz = p->fp32 ? 4 : 8;
+  p->mu = prm->mu < 0 ? 4 : prm->mu;
+  Params& mp = p->mp;
+  for (int ax = 0; ax < 3; ++ax) { mp.box[ax] = prm->box[ax]; mp.periodic[ax] = prm->periodic[ax] ? 1 : 0; }
+  mp.h = prm->h; mp.a = prm->a; mp.p = prm->p; mp.levels = prm->levels; mp.mu = p->mu;
+  if (prm->max_particles < 1 || (prm->precision != MSM_FP32 && prm->precision != MSM_FP64) || p->mu > 28)
+    return MSM_ERR_INVALID_ARG;
+  if (prm->p != 4 && prm->p != 6 && prm->p != 8) return prm->p > 0 && (prm->p & 1) == 0 && prm->p <= 8
+                                                             ? MSM_ERR_UNSUPPORTED : MSM_ERR_INVALID_ARG;
+  p->H = new Hierarchy(mp);
+  if (p->H->status == 2) return MSM_ERR_UNSUPPORTED;
+  if (p->H->status == 3) return MSM_ERR_INVALID_ARG;
+  if (p->H->status == 4) return MSM_ERR_CUTOFF_TOO_LARGE;
+  const Hierarchy& H = *p->H;
+  p->P = prm->p;
+  p->w = H.w;
+  p->n_t = std::min(prm->levels, H.L);
+  if (H.lev[p->n_t].points() > MSM_MAX_TOP_POINTS) return MSM_ERR_UNSUPPORTED;
+  p->S = new Splitting(prm->p, prm->a, H.L);
+  p->J = two_scale_mask(prm->p);
+  p->omega = quasi_interp_sequence(prm->p, p->mu);
+  p->pieces = new SplinePieces(prm->p);
+
+  if (cudaSetDevice(prm->device) != cudaSuccess) return MSM_ERR_CUDA;
+
+  // ---- grids
+  size_t tmp_elems = 16;
+  const int XT = p->fp32 ? 16 : 8, ZT = 4;
+  for (int l = 1; l <= p->n_t; ++l) {
+    const size_t pts = H.lev[l].points();
+    p->lev[l].Q = dev_alloc(p, pts * p->esz);
+    p->lev[l].E = dev_alloc(p, pts * p->esz);
+    tmp_elems = std::max(tmp_elems, pts);
+    if (l < p->n_t) {
+      build_conv_tables(p, l, XT, ZT);
+      const ConvGeom& g = p->lev[l].cg;
+      tmp_elems = std::max(tmp_elems, (size_t)g.P[0] * g.P[1] * g.P[2]);
+      if (p->lev[l].smem > 227 * 1024) return MSM_ERR_UNSUPPORTED;
+    }
+  }
+  p->tmpA = dev_alloc(p, tmp_elems * p->esz);
+  p->tmpB = dev_alloc(p, tmp_elems * p->esz);
+
+  // ---- top operator (always built with its strain derivatives: plan-time cost only)
+  {
+    const TopOperator top = build_top_operator(H, *p->S, p->omega, p->J, p->n_t, true);
+    p->G = top.G;
+    p->topT = upload(p, top.T);
+    std::vector<double> td;
+    td.reserve((size_t)6 * top.G * top.G);
+    for (int k = 0; k < 6; ++k) td.insert(td.end(), top.TD[k].begin(), top.TD[k].end());
+    p->topTD = upload(p, td);
+    p->top_wrow = (double*)dev_alloc(p, (size_t)top.G * 6 * sizeof(double));
+  }
+
+  // ---- particle side
+  BinGeom& bg = p->bg;
+  for (int ax = 0; ax < 3; ++ax) {
+    bg.box[ax] = prm->box[ax];
+    bg.periodic[ax] = mp.periodic[ax];
+    bg.nc[ax] = std::max(1, (int)std::floor(prm->box[ax] / (0.5 * prm->a)));
+    bg.cell_edge[ax] = prm->box[ax] / bg.nc[ax];
+    bg.h1[ax] = H.lev[1].h[ax];
+    bg.ng[ax] = mp.periodic[ax] ? H.lev[1].M[ax] : (int)std::floor(prm->box[ax] / prm->h) + 1;
+  }
+  const long long npc = (long long)bg.nc[0] * bg.nc[1] * bg.nc[2];
+  const long long ngc = (long long)bg.ng[0] * bg.ng[1] * bg.ng[2];
+  if (npc > (1ll << 28) || ngc > (1ll << 28)) return MSM_ERR_UNSUPPORTED;
+  p->n_pcells = (int)npc; p->n_gcells = (int)ngc;
+  p->pair_rows = bg.nc[1] * bg.nc[2];
+  p->cap = prm->max_particles;
+  const size_t cap = (size_t)p->cap;
+  p->ibuf_count = (size_t)2 * p->n_pcells + 2 * p->n_gcells + 8;
+  p->ibuf = (int*)dev_alloc(p, p->ibuf_count * sizeof(int));
+  p->phist = p->ibuf;
+  p->ghist = p->phist + p->n_pcells;
+  p->pfill = p->ghist + p->n_gcells;
+  p->gfill = p->pfill + p->n_pcells;
+  p->flag = p->gfill + p->n_gcells;
+  p->pstart = (int*)dev_alloc(p, ((size_t)p->n_pcells + 1) * sizeof(int));
+  p->gstart = (int*)dev_alloc(p, ((size_t)p->n_gcells + 1) * sizeof(int));
+  p->ptotals = (int*)dev_alloc(p, ((size_t)p->n_pcells / 4096 + 2) * sizeof(int));
+  p->gtotals = (int*)dev_alloc(p, ((size_t)p->n_gcells / 4096 + 2) * sizeof(int));
+  p->pcell = (int*)dev_alloc(p, cap * sizeof(int));
+  p->gcell = (int*)dev_alloc(p, cap * sizeof(int));
+  p->porder = (int*)dev_alloc(p, cap * sizeof(int));
+  p->gorder = (int*)dev_alloc(p, cap * sizeof(int));
+  p->pcellx = (int*)dev_alloc(p, cap * sizeof(int));
+  p->gcell_sorted = (int*)dev_alloc(p, cap * sizeof(int));
+  p->prec = dev_alloc(p, cap * 4 * p->esz);
+  p->grec = dev_alloc(p, cap * 4 * p->esz);
+  p->Fsr = dev_alloc(p, cap * 3 * p->esz);
+  p->Vsr = dev_alloc(p, cap * p->esz);
+  p->pair_wpart = (double*)dev_alloc(p, (size_t)p->pair_rows * 6 * sizeof(double));
+  p->n_eblocks = (int)((cap + 127) / 128);
+  p->epart = (double*)dev_alloc(p, (size_t)p->n_eblocks * sizeof(double));
+  p->results = (double*)dev_alloc(p, 8 * sizeof(double));
+  p->in_pos = dev_alloc(p, cap * 3 * p->esz);
+  p->in_q = dev_alloc(p, cap * p->esz);
+  p->out_F = dev_alloc(p, cap * 3 * p->esz);
+  p->out_V = dev_alloc(p, cap * p->esz);
+  if (cudaMallocHost((void**)&p->h_results, 8 * sizeof(double)) != cudaSuccess) return MSM_ERR_NOMEM;
+  for (int i = 0; i <= kNumStages; ++i)
+    if (cudaEventCreate(&p->ev[i]) != cudaSuccess) return MSM_ERR_CUDA;
+  return MSM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+void msm_plan_destroy(msm_plan_t* p) {
+  if (!p) return;
+  for (void* d : p->allocs) cudaFree(d);
+  if (p->h_results) cudaFreeHost(p->h_results);
+  for (int i = 0; i <= kNumStages; ++i)
+    if (p->ev[i]) cudaEventDestroy(p->ev[i]);
+  delete p->H; delete p->S; delete p->pieces;
+  delete p;
+}
+
+msm_status_t msm_plan_create(const msm_params_t* params, msm_plan_t** plan_out) {
+  if (!plan_out) return MSM_ERR_INVALID_ARG;
+  *plan_out = nullptr;
+  if (!params) return MSM_ERR_INVALID_ARG;
+  msm_plan* p = new (std::nothrow) msm_plan();
+  if (!p) return MSM_ERR_NOMEM;
+  msm_status_t st;
+  try {
+    st = create_impl(params, p);
+  } catch (const std::bad_alloc&) {
+    st = MSM_ERR_NOMEM;
+  } catch (const CudaFail&) {
+    st = MSM_ERR_CUDA;
+  } catch (...) {
+    st = MSM_ERR_CUDA;
+  }
+  if (st != MSM_OK) { cudaGetLastError(); msm_plan_destroy(p); return st; }
+  *plan_out = p;
+  return MSM_OK;
+}
+
+msm_status_t msm_plan_info(const msm_plan_t* p, msm_plan_info_t* info) {
+  if (!p || !info) return MSM_ERR_INVALID_ARG;
+  std::memset(info, 0, sizeof(*info));
+  info->L_full = p->H->L;
+  info->n_tiled = p->n_t;
+  info->mu = p->mu;
+  info->omega_halfwidth = p->w;
+  for (int l = 1; l <= p->H->L && l <= MSM_MAX_LEVELS; ++l)
+    for (int ax = 0; ax < 3; ++ax) {
+      info->grid_dims[l - 1][ax] = p->H->lev[l].M[ax];
+      info->grid_lo[l - 1][ax] = p->H->lev[l].lo[ax];
+      info->grid_h[l - 1][ax] = p->H->lev[l].h[ax];
+    }
+  for (int l = 1; l < p->n_t; ++l) info->stencil_taps[l - 1] = p->lev[l].taps;
+  for (int ax = 0; ax < 3; ++ax) info->pair_cells[ax] = p->bg.nc[ax];
+  info->top_points = p->G;
+  info->device_bytes = p->bytes;
+  return MSM_OK;
+}
+
+const char* msm_status_string(msm_status_t s) {
+  switch (s) {
+    case MSM_OK: return "ok";
+    case MSM_ERR_INVALID_ARG: return "invalid argument";
+    case MSM_ERR_UNSUPPORTED: return "unsupported configuration";
+    case MSM_ERR_CUTOFF_TOO_LARGE: return "cutoff larger than half a periodic box edge";
+    case MSM_ERR_TOO_MANY_PARTICLES: return "more particles than the plan's capacity";
+    case MSM_ERR_OUT_OF_BOX: return "coordinate outside an open box axis, or non-finite input";
+    case MSM_ERR_NOMEM: return "out of memory";
+    case MSM_ERR_CUDA: return "CUDA error";
+  }
+  return "unknown status";
+}
+
+}  // extern "C"

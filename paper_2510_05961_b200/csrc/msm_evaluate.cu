@@ -1,0 +1,363 @@
+// msm_evaluate.cu -- msm_evaluate: enqueues the whole hot path (S1..S9 of DESIGN.md) on one stream.
+#include <algorithm>
+#include <cstring>
+
+#include "gridops.cuh"
+#include "pair.cuh"
+#include "particle_grid.cuh"
+#include "plan.hpp"
+#include "sort.cuh"
+
+using namespace msm;
+
+namespace {
+
+struct Seg {
+  const double* ptr;
+  int count;      // rows of 6 (or of 1 for the energy)
+  double scale[6];
+};
+constexpr int kMaxSegs = MSM_MAX_LEVELS + 4;
+struct FinalizeArgs {
+  int nseg;
+  Seg seg[kMaxSegs];
+  const double* epart;
+  int ne;
+};
+
+// S9: U = sum of the block partials; W = sum over segments of scale_k * partial_k. One block,
+// fixed order -> deterministic.
+__global__ void __launch_bounds__(256) k_finalize(FinalizeArgs a, const int* __restrict__ flag,
+                                                  double* __restrict__ results) {
+  __shared__ double red[8];
+  double e = 0.0;
+  for (int i = threadIdx.x; i < a.ne; i += 256) e += a.epart[i];
+  e = block_reduce_sum<256>(e, red);
+  if (threadIdx.x == 0) results[0] = e;
+  for (int k = 0; k < 6; ++k) {
+    double w = 0.0;
+    for (int s = 0; s < a.nseg; ++s) {
+      double t = 0.0;
+      for (int i = threadIdx.x; i < a.seg[s].count; i += 256) t += a.seg[s].ptr[(size_t)i * 6 + k];
+      w += a.seg[s].scale[k] * t;
+    }
+    w = block_reduce_sum<256>(w, red);
+    if (threadIdx.x == 0) results[1 + k] = w;
+  }
+  if (threadIdx.x == 0) results[7] = (double)(*flag);
+}
+
+inline unsigned blocks_for(size_t n, int bs) { return (unsigned)std::max<size_t>(1, (n + bs - 1) / bs); }
+
+template <typename T> AxisTaps<T> make_taps(const std::vector<double>& v) {
+  AxisTaps<T> t;
+  t.n = (int)v.size();
+  for (int i = 0; i < t.n; ++i) t.c[i] = (T)v[i];
+  return t;
+}
+
+template <typename T, int P> SplineTab<T, P> make_tab(const SplinePieces& sp) {
+  SplineTab<T, P> t;
+  for (int j = 0; j < P; ++j)
+    for (int k = 0; k < P; ++k) { t.c[j][k] = (T)sp.coef[j][k]; t.d[j][k] = (T)sp.dcoef[j][k]; }
+  return t;
+}
+
+#define MSM_LAUNCH(plan, ...) do { __VA_ARGS__; ++(plan)->launches; } while (0)
+
+template <typename T, int P>
+msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, void* d_F, void* d_V,
+                        bool want_virial, cudaStream_t st) {
+  using V4 = typename Vec4<T>::type;
+  const Hierarchy& H = *p->H;
+  const T* pos = (const T*)d_pos;
+  const T* q = (const T*)d_q;
+  int evi = 0;
+  auto mark = [&]() { if (p->profiling) cudaEventRecord(p->ev[evi], st); ++evi; };
+  p->launches = 0;
+  mark();
+
+  // ---------------- S1 sort
+  cudaMemsetAsync(p->ibuf, 0, p->ibuf_count * sizeof(int), st);
+  MSM_LAUNCH(p, (k_bin<T><<<blocks_for(n, 256), 256, 0, st>>>(n, pos, p->bg, p->pcell, p->gcell, p->phist,
+                                                               p->ghist, p->flag)));
+  {
+    const int tp = (p->n_pcells + kScanTile - 1) / kScanTile, tg = (p->n_gcells + kScanTile - 1) / kScanTile;
+    MSM_LAUNCH(p, (k_scan_tiles<<<tp, kScanThreads, 0, st>>>(p->n_pcells, p->phist, p->pstart, p->ptotals)));
+    MSM_LAUNCH(p, (k_scan_tiles<<<tg, kScanThreads, 0, st>>>(p->n_gcells, p->ghist, p->gstart, p->gtotals)));
+    MSM_LAUNCH(p, (k_scan_totals<<<1, kScanThreads, 0, st>>>(tp, p->ptotals)));
+    MSM_LAUNCH(p, (k_scan_totals<<<1, kScanThreads, 0, st>>>(tg, p->gtotals)));
+    MSM_LAUNCH(p, (k_scan_add<<<blocks_for(p->n_pcells, 256), 256, 0, st>>>(p->n_pcells, p->pstart, p->ptotals, n)));
+    MSM_LAUNCH(p, (k_scan_add<<<blocks_for(p->n_gcells, 256), 256, 0, st>>>(p->n_gcells, p->gstart, p->gtotals, n)));
+  }
+  MSM_LAUNCH(p, (k_scatter<<<blocks_for(n, 256), 256, 0, st>>>(n, p->pcell, p->gcell, p->pstart, p->gstart,
+                                                                 p->pfill, p->gfill, p->porder, p->gorder)));
+  MSM_LAUNCH(p, (k_sort_cells<<<blocks_for(p->n_pcells, 128), 128, 0, st>>>(p->n_pcells, p->pstart, p->porder)));
+  MSM_LAUNCH(p, (k_sort_cells<<<blocks_for(p->n_gcells, 128), 128, 0, st>>>(p->n_gcells, p->gstart, p->gorder)));
+  MSM_LAUNCH(p, (k_build_records<T><<<blocks_for(n, 256), 256, 0, st>>>(
+                    n, pos, q, p->bg, p->porder, p->pcell, p->gorder, p->gcell, (V4*)p->prec, (V4*)p->grec,
+                    p->gcell_sorted, p->pcellx)));
+  mark();
+
+  // ---------------- S2 pair
+  {
+    PairParams<T> pp;
+    bool any_minimg = false;
+    for (int ax = 0; ax < 3; ++ax) {
+      pp.nc[ax] = p->bg.nc[ax];
+      pp.periodic[ax] = p->bg.periodic[ax];
+      pp.minimg[ax] = (p->bg.periodic[ax] && p->bg.nc[ax] < 5) ? 1 : 0;
+      pp.omin[ax] = -2;
+      pp.omax[ax] = pp.minimg[ax] ? std::min(2, p->bg.nc[ax] - 3) : 2;   // nc distinct cells
+      if (pp.minimg[ax]) { pp.omin[ax] = -std::min(2, p->bg.nc[ax] - 1 - pp.omax[ax]); }
+      any_minimg |= pp.minimg[ax] != 0;
+      pp.edge[ax] = (T)p->bg.cell_edge[ax];
+      pp.box[ax] = (T)p->bg.box[ax];
+      pp.inv_box[ax] = (T)(1.0 / p->bg.box[ax]);
+    }
+    (void)any_minimg;
+    const double a = p->mp.a;
+    pp.a2 = (T)(a * a); pp.inv_a = (T)(1.0 / a); pp.inv_a2 = (T)(1.0 / (a * a)); pp.two_inv_a3 = (T)(2.0 / (a * a * a));
+    for (int k = 0; k < 8; ++k) pp.c[k] = (T)p->S->c[k];
+    pp.p = P;
+    if (want_virial)
+      MSM_LAUNCH(p, (k_pair<T, P, true><<<p->pair_rows, kPairWarps * 32, 0, st>>>(
+                        pp, p->pstart, (const V4*)p->prec, p->pcellx, p->porder, (T*)p->Fsr, (T*)p->Vsr, p->pair_wpart)));
+    else
+      MSM_LAUNCH(p, (k_pair<T, P, false><<<p->pair_rows, kPairWarps * 32, 0, st>>>(
+                        pp, p->pstart, (const V4*)p->prec, p->pcellx, p->porder, (T*)p->Fsr, (T*)p->Vsr, p->pair_wpart)));
+  }
+  mark();
+
+  // ---------------- S3 anterpolation
+  GridGeom gg;
+  for (int ax = 0; ax < 3; ++ax) {
+    gg.M[ax] = H.lev[1].M[ax]; gg.lo[ax] = H.lev[1].lo[ax]; gg.ng[ax] = p->bg.ng[ax];
+    gg.periodic[ax] = p->bg.periodic[ax];
+  }
+  const SplineTab<T, P> tab = make_tab<T, P>(*p->pieces);
+  MSM_LAUNCH(p, (k_anterpolate<T, P><<<blocks_for(H.lev[1].points(), 128), 128, 0, st>>>(
+                    gg, tab, p->gstart, (const V4*)p->grec, (T*)p->lev[1].Q)));
+  mark();
+
+  // ---------------- S4 restriction
+  const AxisTaps<T> Jt = make_taps<T>(p->J), Wt = make_taps<T>(p->omega);
+  for (int l = 1; l < p->n_t; ++l) {
+    const Level &f = H.lev[l], &c = H.lev[l + 1];
+    const T* src = (const T*)p->lev[l].Q;
+    int din[3] = {f.M[0], f.M[1], f.M[2]};
+    for (int ax = 0; ax < 3; ++ax) {
+      AxisDims d;
+      for (int k = 0; k < 3; ++k) { d.in[k] = din[k]; d.out[k] = din[k]; }
+      d.out[ax] = c.M[ax];
+      d.axis = ax; d.periodic = p->bg.periodic[ax];
+      T* dst = ax == 2 ? (T*)p->lev[l + 1].Q : (T*)(ax == 0 ? p->tmpA : p->tmpB);
+      const size_t tot = (size_t)d.out[0] * d.out[1] * d.out[2];
+      MSM_LAUNCH(p, (k_restrict_axis<T><<<blocks_for(tot, 256), 256, 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
+      src = dst;
+      din[ax] = c.M[ax];
+    }
+  }
+  mark();
+
+  // ---------------- S5 convolution on the tiled levels
+  int nseg = 0;
+  FinalizeArgs fa;
+  for (int l = 1; l < p->n_t; ++l) {
+    LevelDev& d = p->lev[l];
+    const ConvGeom& g = d.cg;
+    const Level& lv = H.lev[l];
+    // omega' filter + halo, x then y then z
+    const T* src = (const T*)d.Q;
+    int din[3] = {lv.M[0], lv.M[1], lv.M[2]};
+    const int halo[3] = {g.X0, g.R[1], g.R[2]};
+    for (int ax = 0; ax < 3; ++ax) {
+      AxisDims ad;
+      for (int k = 0; k < 3; ++k) { ad.in[k] = din[k]; ad.out[k] = din[k]; }
+      ad.out[ax] = g.P[ax];
+      ad.axis = ax; ad.periodic = p->bg.periodic[ax];
+      T* dst = ax == 2 ? (T*)d.pad : (T*)(ax == 0 ? p->tmpA : p->tmpB);
+      const size_t tot = (size_t)ad.out[0] * ad.out[1] * ad.out[2];
+      // along the filtered axis the logical size is the grid's, not the (already padded) array's
+      ad.in[ax] = lv.M[ax];
+      MSM_LAUNCH(p, (k_pad_filter<T><<<blocks_for(tot, 256), 256, 0, st>>>(ad, halo[ax], Wt, src, dst)));
+      src = dst;
+      din[ax] = g.P[ax];
+    }
+    constexpr int XT = sizeof(T) == 4 ? 16 : 8, ZT = 4;
+    if (want_virial) {
+      auto kern = k_conv<T, XT, ZT, true>;
+      if (d.smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d.smem);
+      MSM_LAUNCH(p, (kern<<<d.units, 32, d.smem, st>>>(g, d.rows, (const T*)d.staps, (const T*)d.gtaps,
+                                                      (const T*)d.pad, (const T*)d.Q, (T*)d.E, d.wpart)));
+      Seg& s = fa.seg[nseg++];
+      s.ptr = d.wpart; s.count = d.units;
+      const double hx = lv.h[0], hy = lv.h[1], hz = lv.h[2];
+      const double sc[6] = {hx * hx, hy * hy, hz * hz, hx * hy, hx * hz, hy * hz};
+      for (int k = 0; k < 6; ++k) s.scale[k] = -0.5 * sc[k];
+    } else {
+      auto kern = k_conv<T, XT, ZT, false>;
+      if (d.smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d.smem);
+      MSM_LAUNCH(p, (kern<<<d.units, 32, d.smem, st>>>(g, d.rows, (const T*)d.staps, (const T*)d.gtaps,
+                                                      (const T*)d.pad, (const T*)d.Q, (T*)d.E, d.wpart)));
+    }
+  }
+  mark();
+
+  // ---------------- S6 top level
+  {
+    LevelDev& d = p->lev[p->n_t];
+    const unsigned nb = blocks_for((size_t)p->G * 32, 128);
+    if (want_virial) {
+      MSM_LAUNCH(p, (k_top_dense<T, true><<<nb, 128, 0, st>>>(p->G, (const T*)p->topT, (const T*)p->topTD,
+                                                             (const T*)d.Q, (T*)d.E, p->top_wrow)));
+      Seg& s = fa.seg[nseg++];
+      s.ptr = p->top_wrow; s.count = p->G;
+      for (int k = 0; k < 6; ++k) s.scale[k] = 1.0;
+    } else {
+      MSM_LAUNCH(p, (k_top_dense<T, false><<<nb, 128, 0, st>>>(p->G, (const T*)p->topT, (const T*)p->topTD,
+                                                              (const T*)d.Q, (T*)d.E, p->top_wrow)));
+    }
+  }
+  mark();
+
+  // ---------------- S7 prolongation + accumulate, z then y then x
+  for (int l = p->n_t - 1; l >= 1; --l) {
+    const Level &f = H.lev[l], &c = H.lev[l + 1];
+    const T* src = (const T*)p->lev[l + 1].E;
+    int din[3] = {c.M[0], c.M[1], c.M[2]};
+    const int order[3] = {2, 1, 0};
+    for (int s3 = 0; s3 < 3; ++s3) {
+      const int ax = order[s3];
+      AxisDims d;
+      for (int k = 0; k < 3; ++k) { d.in[k] = din[k]; d.out[k] = din[k]; }
+      d.out[ax] = f.M[ax];
+      d.axis = ax; d.periodic = p->bg.periodic[ax];
+      const size_t tot = (size_t)d.out[0] * d.out[1] * d.out[2];
+      if (s3 < 2) {
+        T* dst = (T*)(s3 == 0 ? p->tmpA : p->tmpB);
+        MSM_LAUNCH(p, (k_prolong_axis<T, false><<<blocks_for(tot, 256), 256, 0, st>>>(d, c.lo[ax], f.lo[ax], Jt, src, dst)));
+        src = dst;
+      } else {
+        MSM_LAUNCH(p, (k_prolong_axis<T, true><<<blocks_for(tot, 256), 256, 0, st>>>(d, c.lo[ax], f.lo[ax], Jt, src,
+                                                                                    (T*)p->lev[l].E)));
+      }
+      din[ax] = f.M[ax];
+    }
+  }
+  mark();
+
+  // ---------------- S8 interpolation + outputs
+  const int neb = (int)blocks_for(n, 128);
+  MSM_LAUNCH(p, (k_interpolate<T, P><<<neb, 128, 0, st>>>(
+                    n, gg, tab, (T)(1.0 / H.lev[1].h[0]), (T)(1.0 / H.lev[1].h[1]), (T)(1.0 / H.lev[1].h[2]),
+                    (T)(p->S->gamma0() / p->mp.a), (const V4*)p->grec, p->gcell_sorted, p->gorder,
+                    (const T*)p->lev[1].E, (const T*)p->Fsr, (const T*)p->Vsr, (T*)d_F, (T*)d_V, p->epart)));
+  mark();
+
+  // ---------------- S9 reductions
+  if (want_virial) {
+    Seg& s = fa.seg[nseg++];
+    s.ptr = p->pair_wpart; s.count = p->pair_rows;
+    for (int k = 0; k < 6; ++k) s.scale[k] = 1.0;
+  }
+  fa.nseg = nseg;
+  fa.epart = p->epart; fa.ne = neb;
+  MSM_LAUNCH(p, (k_finalize<<<1, 256, 0, st>>>(fa, p->flag, p->results)));
+  mark();
+  cudaMemcpyAsync(p->h_results, p->results, 8 * sizeof(double), cudaMemcpyDeviceToHost, st);
+  if (cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }
+  if (cudaGetLastError() != cudaSuccess) return MSM_ERR_CUDA;
+  if (p->profiling)
+    for (int i = 0; i < kNumStages; ++i) cudaEventElapsedTime(&p->stage_ms[i], p->ev[i], p->ev[i + 1]);
+  return MSM_OK;
+}
+
+template <typename T>
+msm_status_t evaluate_p(msm_plan* p, int n, const void* pos, const void* q, void* F, void* V, bool wv, cudaStream_t st) {
+  switch (p->P) {
+    case 4: return evaluate_t<T, 4>(p, n, pos, q, F, V, wv, st);
+    case 6: return evaluate_t<T, 6>(p, n, pos, q, F, V, wv, st);
+    case 8: return evaluate_t<T, 8>(p, n, pos, q, F, V, wv, st);
+  }
+  return MSM_ERR_UNSUPPORTED;
+}
+
+}  // namespace
+
+extern "C" {
+
+msm_status_t msm_evaluate(msm_plan_t* p, int n, const void* d_positions, const void* d_charges, void* d_forces,
+                          void* d_potentials, double* h_energy, double* h_virial, void* cuda_stream) {
+  if (!p || n < 0 || (n > 0 && (!d_positions || !d_charges))) return MSM_ERR_INVALID_ARG;
+  if (n > p->cap) return MSM_ERR_TOO_MANY_PARTICLES;
+  if (cudaSetDevice(p->prm.device) != cudaSuccess) return MSM_ERR_CUDA;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const bool wv = h_virial != nullptr;
+  const msm_status_t s = p->fp32 ? evaluate_p<float>(p, n, d_positions, d_charges, d_forces, d_potentials, wv, st)
+                                 : evaluate_p<double>(p, n, d_positions, d_charges, d_forces, d_potentials, wv, st);
+  if (s != MSM_OK) return s;
+  if (h_energy) *h_energy = p->h_results[0];
+  if (h_virial) std::memcpy(h_virial, p->h_results + 1, 6 * sizeof(double));
+  if (p->h_results[7] != 0.0) return MSM_ERR_OUT_OF_BOX;
+  return MSM_OK;
+}
+
+msm_status_t msm_evaluate_host(msm_plan_t* p, int n, const void* h_positions, const void* h_charges, void* h_forces,
+                               void* h_potentials, double* h_energy, double* h_virial, void* cuda_stream) {
+  if (!p || n < 0 || (n > 0 && (!h_positions || !h_charges))) return MSM_ERR_INVALID_ARG;
+  if (n > p->cap) return MSM_ERR_TOO_MANY_PARTICLES;
+  if (cudaSetDevice(p->prm.device) != cudaSuccess) return MSM_ERR_CUDA;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t e = p->esz;
+  if (cudaMemcpyAsync(p->in_pos, h_positions, (size_t)n * 3 * e, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+      cudaMemcpyAsync(p->in_q, h_charges, (size_t)n * e, cudaMemcpyHostToDevice, st) != cudaSuccess) {
+    cudaGetLastError();
+    return MSM_ERR_CUDA;
+  }
+  const msm_status_t s = msm_evaluate(p, n, p->in_pos, p->in_q, h_forces ? p->out_F : nullptr,
+                                      h_potentials ? p->out_V : nullptr, h_energy, h_virial, cuda_stream);
+  if (s != MSM_OK && s != MSM_ERR_OUT_OF_BOX) return s;
+  if (h_forces) cudaMemcpyAsync(h_forces, p->out_F, (size_t)n * 3 * e, cudaMemcpyDeviceToHost, st);
+  if (h_potentials) cudaMemcpyAsync(h_potentials, p->out_V, (size_t)n * e, cudaMemcpyDeviceToHost, st);
+  if (cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }
+  return s;
+}
+
+msm_status_t msm_set_profiling(msm_plan_t* p, int enabled) {
+  if (!p) return MSM_ERR_INVALID_ARG;
+  p->profiling = enabled != 0;
+  return MSM_OK;
+}
+
+msm_status_t msm_get_stage_times(const msm_plan_t* p, int* n_stages, const char* const** names,
+                                 const float** milliseconds) {
+  if (!p || !n_stages || !names || !milliseconds) return MSM_ERR_INVALID_ARG;
+  *n_stages = kNumStages;
+  *names = kStageNames;
+  *milliseconds = p->stage_ms;
+  return MSM_OK;
+}
+
+msm_status_t msm_get_launch_count(const msm_plan_t* p, int* count) {
+  if (!p || !count) return MSM_ERR_INVALID_ARG;
+  *count = p->launches;
+  return MSM_OK;
+}
+
+msm_status_t msm_debug_copy_grid(const msm_plan_t* p, int level, int kind, double* h_out, size_t capacity) {
+  if (!p || !h_out || level < 1 || level > p->n_t || (kind != 0 && kind != 1)) return MSM_ERR_INVALID_ARG;
+  const size_t pts = p->H->lev[level].points();
+  if (capacity < pts) return MSM_ERR_INVALID_ARG;
+  const void* src = kind == 0 ? p->lev[level].Q : p->lev[level].E;
+  if (p->fp32) {
+    std::vector<float> tmp(pts);
+    if (cudaMemcpy(tmp.data(), src, pts * 4, cudaMemcpyDeviceToHost) != cudaSuccess) return MSM_ERR_CUDA;
+    for (size_t i = 0; i < pts; ++i) h_out[i] = tmp[i];
+  } else if (cudaMemcpy(h_out, src, pts * 8, cudaMemcpyDeviceToHost) != cudaSuccess) {
+    return MSM_ERR_CUDA;
+  }
+  return MSM_OK;
+}
+
+}  // extern "C"

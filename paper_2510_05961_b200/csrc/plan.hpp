@@ -1,0 +1,74 @@
+// plan.hpp -- the opaque msm_plan: host mathematics + every device buffer of one MSM setup.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/msm.h"
+#include "conv.cuh"
+#include "plan_math.hpp"
+
+namespace msm {
+
+constexpr int kNumStages = 9;
+extern const char* const kStageNames[kNumStages];
+
+struct LevelDev {
+  void *Q = nullptr, *E = nullptr, *pad = nullptr;   // grid charge, potential, haloed filtered charge
+  ConvGeom cg{};
+  int4* rows = nullptr;
+  void *staps = nullptr, *gtaps = nullptr;
+  int units = 0;
+  double* wpart = nullptr;                           // units x 6
+  int taps = 0;
+  size_t smem = 0;
+};
+
+}  // namespace msm
+
+struct msm_plan {
+  msm_params_t prm{};
+  msm::Params mp{};
+  msm::Hierarchy* H = nullptr;
+  msm::Splitting* S = nullptr;
+  int P = 4, n_t = 1, mu = 4, w = 0;
+  bool fp32 = false;
+  size_t esz = 8;
+  std::vector<double> J, omega;
+  msm::SplinePieces* pieces = nullptr;
+
+  std::vector<void*> allocs;
+  size_t bytes = 0;
+
+  msm::LevelDev lev[MSM_MAX_LEVELS + 1];
+  void *tmpA = nullptr, *tmpB = nullptr;
+
+  // top operator
+  int G = 0;
+  void *topT = nullptr, *topTD = nullptr;
+  double* top_wrow = nullptr;
+
+  // particles
+  int cap = 0;
+  msm::BinGeom bg{};
+  int n_pcells = 0, n_gcells = 0, pair_rows = 0;
+  int* ibuf = nullptr;          // [phist(n_pcells+1) | ghist(n_gcells+1) | pfill | gfill | flag]
+  size_t ibuf_count = 0;
+  int *phist = nullptr, *ghist = nullptr, *pfill = nullptr, *gfill = nullptr, *flag = nullptr;
+  int *pstart = nullptr, *gstart = nullptr, *ptotals = nullptr, *gtotals = nullptr;
+  int *pcell = nullptr, *gcell = nullptr, *porder = nullptr, *gorder = nullptr, *pcellx = nullptr,
+      *gcell_sorted = nullptr;
+  void *prec = nullptr, *grec = nullptr, *Fsr = nullptr, *Vsr = nullptr;
+  double *pair_wpart = nullptr, *epart = nullptr, *results = nullptr;
+  int n_eblocks = 0;
+  double* h_results = nullptr;  // pinned: U, W[6], flag
+  // staging for msm_evaluate_host
+  void *in_pos = nullptr, *in_q = nullptr, *out_F = nullptr, *out_V = nullptr;
+
+  // profiling
+  bool profiling = false;
+  cudaEvent_t ev[msm::kNumStages + 1]{};
+  float stage_ms[msm::kNumStages]{};
+  int launches = 0;
+};

@@ -1,0 +1,209 @@
+// sort.cuh -- S1: binning and counting sort of the particles, once by short-range cell and once
+// by level-1 grid cell (replaces the paper's neighbour list; its construction is inside our
+// timing). Within a cell particles are ordered by original index, so every later per-cell sum has
+// a fixed order (run-to-run deterministic results).
+#pragma once
+#include "device_common.cuh"
+
+namespace msm {
+
+// wrapped / clamped coordinate and its integer cell, in fp64 on both precisions
+__device__ __forceinline__ double wrap_coord(double x, double L, int periodic) {
+  if (periodic) {
+    x -= L * floor(x / L);
+    if (x >= L) x = 0.0;
+  }
+  return x;
+}
+
+// pass 1: cell ids + histograms (+ input validation)
+template <typename T>
+__global__ void k_bin(int n, const T* __restrict__ pos, BinGeom g, int* __restrict__ pcell,
+                      int* __restrict__ gcell, int* __restrict__ phist, int* __restrict__ ghist,
+                      int* __restrict__ flag) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int pc[3], gc[3];
+  bool bad = false;
+#pragma unroll
+  for (int ax = 0; ax < 3; ++ax) {
+    double x = (double)pos[3 * (size_t)i + ax];
+    if (!isfinite(x)) { bad = true; x = 0.0; }
+    if (!g.periodic[ax] && (x < 0.0 || x > g.box[ax])) { bad = true; x = fmin(fmax(x, 0.0), g.box[ax]); }
+    x = wrap_coord(x, g.box[ax], g.periodic[ax]);
+    int c = (int)floor(x / g.cell_edge[ax]);
+    pc[ax] = min(max(c, 0), g.nc[ax] - 1);
+    int k = (int)floor(x / g.h1[ax]);
+    gc[ax] = min(max(k, 0), g.ng[ax] - 1);
+  }
+  if (bad) atomicOr(flag, 1);
+  const int pci = (pc[2] * g.nc[1] + pc[1]) * g.nc[0] + pc[0];
+  const int gci = (gc[2] * g.ng[1] + gc[1]) * g.ng[0] + gc[0];
+  pcell[i] = pci;
+  gcell[i] = gci;
+  atomicAdd(&phist[pci], 1);
+  atomicAdd(&ghist[gci], 1);
+}
+
+// exclusive scan, three kernels: per-block scan of 4096-element tiles, scan of the tile totals,
+// add-back. data[m] must be writable (the total is written there).
+constexpr int kScanThreads = 1024;
+constexpr int kScanPerThread = 4;
+constexpr int kScanTile = kScanThreads * kScanPerThread;
+
+__global__ void k_scan_tiles(int m, const int* __restrict__ in, int* __restrict__ out,
+                             int* __restrict__ totals) {
+  __shared__ int wsum[32];
+  const int base = blockIdx.x * kScanTile + threadIdx.x * kScanPerThread;
+  int v[kScanPerThread], s = 0;
+#pragma unroll
+  for (int k = 0; k < kScanPerThread; ++k) {
+    v[k] = (base + k < m) ? in[base + k] : 0;
+    s += v[k];
+  }
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  int inc = s;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += t;
+  }
+  if (lane == 31) wsum[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    int t = wsum[lane];
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int u = __shfl_up_sync(0xffffffffu, t, o);
+      if (lane >= o) t += u;
+    }
+    wsum[lane] = t;
+  }
+  __syncthreads();
+  int excl = inc - s + (wid > 0 ? wsum[wid - 1] : 0);
+#pragma unroll
+  for (int k = 0; k < kScanPerThread; ++k) {
+    if (base + k < m) out[base + k] = excl;
+    excl += v[k];
+  }
+  if (threadIdx.x == kScanThreads - 1) totals[blockIdx.x] = excl;
+}
+
+__global__ void k_scan_totals(int nt, int* __restrict__ totals) {  // one block, nt <= 1024*? loop
+  __shared__ int carry_s;
+  __shared__ int wsum[32];
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  for (int base = 0; base < nt; base += kScanThreads) {
+    const int i = base + threadIdx.x;
+    const int v = i < nt ? totals[i] : 0;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += t;
+    }
+    if (lane == 31) wsum[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+      int t = wsum[lane];
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int u = __shfl_up_sync(0xffffffffu, t, o);
+        if (lane >= o) t += u;
+      }
+      wsum[lane] = t;
+    }
+    __syncthreads();
+    const int carry = carry_s;
+    const int excl = carry + inc - v + (wid > 0 ? wsum[wid - 1] : 0);
+    if (i < nt) totals[i] = excl;
+    __syncthreads();
+    if (threadIdx.x == kScanThreads - 1) carry_s = excl + v;
+    __syncthreads();
+  }
+}
+
+__global__ void k_scan_add(int m, int* __restrict__ out, const int* __restrict__ totals, int n_total) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < m) out[i] += totals[i / kScanTile];
+  if (i == 0) out[m] = n_total;
+}
+
+// pass 2: scatter original indices into their cell's segment (slot order arbitrary here)
+__global__ void k_scatter(int n, const int* __restrict__ pcell, const int* __restrict__ gcell,
+                          const int* __restrict__ pstart, const int* __restrict__ gstart,
+                          int* __restrict__ pfill, int* __restrict__ gfill, int* __restrict__ porder,
+                          int* __restrict__ gorder) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int pc = pcell[i], gc = gcell[i];
+  porder[pstart[pc] + atomicAdd(&pfill[pc], 1)] = i;
+  gorder[gstart[gc] + atomicAdd(&gfill[gc], 1)] = i;
+}
+
+// pass 3: canonical order inside each cell (ascending original index): insertion sort per cell
+__global__ void k_sort_cells(int ncell, const int* __restrict__ start, int* __restrict__ order) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncell) return;
+  const int s = start[c], e = start[c + 1];
+  for (int i = s + 1; i < e; ++i) {
+    const int v = order[i];
+    int j = i - 1;
+    while (j >= s && order[j] > v) { order[j + 1] = order[j]; --j; }
+    order[j + 1] = v;
+  }
+}
+
+// pass 4: sorted records. Pair order: cell-relative coordinates + charge (fp32-safe: magnitudes
+// stay below one cell edge). Grid order: fractions t in [0,1] of the particle's grid cell + charge.
+template <typename T>
+__global__ void k_build_records(int n, const T* __restrict__ pos, const T* __restrict__ q, BinGeom g,
+                                const int* __restrict__ porder, const int* __restrict__ pcell,
+                                const int* __restrict__ gorder, const int* __restrict__ gcell,
+                                typename Vec4<T>::type* __restrict__ prec,
+                                typename Vec4<T>::type* __restrict__ grec, int* __restrict__ gcell_sorted,
+                                int* __restrict__ pcellx) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  {
+    const int i = porder[k];
+    int c = pcell[i];
+    const int cx = c % g.nc[0]; c /= g.nc[0];
+    const int cy = c % g.nc[1], cz = c / g.nc[1];
+    const int cc[3] = {cx, cy, cz};
+    T r[3];
+#pragma unroll
+    for (int ax = 0; ax < 3; ++ax) {
+      double x = (double)pos[3 * (size_t)i + ax];
+      if (!isfinite(x)) x = 0.0;
+      if (!g.periodic[ax]) x = fmin(fmax(x, 0.0), g.box[ax]);
+      x = wrap_coord(x, g.box[ax], g.periodic[ax]);
+      r[ax] = (T)(x - cc[ax] * g.cell_edge[ax]);
+    }
+    prec[k] = make_vec4<T>(r[0], r[1], r[2], q[i]);
+    pcellx[k] = cx;
+  }
+  {
+    const int i = gorder[k];
+    const int cid = gcell[i];
+    int c = cid;
+    const int cx = c % g.ng[0]; c /= g.ng[0];
+    const int cy = c % g.ng[1], cz = c / g.ng[1];
+    const int cc[3] = {cx, cy, cz};
+    T t[3];
+#pragma unroll
+    for (int ax = 0; ax < 3; ++ax) {
+      double x = (double)pos[3 * (size_t)i + ax];
+      if (!isfinite(x)) x = 0.0;
+      if (!g.periodic[ax]) x = fmin(fmax(x, 0.0), g.box[ax]);
+      x = wrap_coord(x, g.box[ax], g.periodic[ax]);
+      t[ax] = (T)(x / g.h1[ax] - (double)cc[ax]);
+    }
+    grec[k] = make_vec4<T>(t[0], t[1], t[2], q[i]);
+    gcell_sorted[k] = cid;
+  }
+}
+
+}  // namespace msm
