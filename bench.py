@@ -1,0 +1,339 @@
+#!/usr/bin/env python
+"""bench.py -- MSM energy+forces+potentials+virial particles/s on B200 (BASELINE.json metric).
+
+A "step" is one msm_evaluate over one batch of synthetic input: the whole hot path (sort, pair,
+anterpolation, restriction, per-level convolution, top level, prolongation, interpolation,
+reductions), all outputs requested. Default workload: BASELINE config 4 at N = 999 999 (fp32), the
+largest single-GPU configuration; `--workload` selects another (see workloads.WORKLOAD_NAMES).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl reference]
+
+N > 1 (under torchrun): the path does not shard (replicas only), so every
+rank evaluates its own replica of the workload; value = N * particles / max-over-ranks time.
+`--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "msm_energy_forces_particles_per_s"
+UNIT = "particles/s"
+FLOP_PER_PAIR = 30.0          # r^2, rsqrt, Horner g and g', 4 accumulations
+SM_COUNT, FP32_LANES, SM_MAX_GHZ = 148, 128, 1.965
+
+
+def derived_alu_peak_tflops(dtype: str) -> float:
+    """FP32: 148 SMs x 128 FMA lanes x 2 flop x 1.965 GHz (guide's unit counts and max clock);
+    FP64: half the lanes (64 per SM on B200; the DFMA microbenchmark measures ~0.47 of FFMA)."""
+    lanes = FP32_LANES if dtype == "f32" else FP32_LANES // 2
+    return SM_COUNT * lanes * 2 * SM_MAX_GHZ * 1e-3
+
+
+def load_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (the recipe's clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def count_pairs(w) -> float:
+    """Directed in-cutoff pairs of the workload (the pair kernel's algorithmic unit)."""
+    import numpy as np
+    try:
+        from scipy.spatial import cKDTree
+        bs = [b if p else 0.0 for b, p in zip(w.box, w.periodic)]
+        pos = np.array(w.positions, copy=True)
+        for ax in range(3):
+            if w.periodic[ax]:
+                pos[:, ax] -= w.box[ax] * np.floor(pos[:, ax] / w.box[ax])
+                pos[pos[:, ax] >= w.box[ax], ax] = 0.0
+        tree = cKDTree(pos, boxsize=bs if any(w.periodic) else None)
+        return float(tree.count_neighbors(tree, w.a) - w.n)
+    except Exception:
+        vol = w.box[0] * w.box[1] * w.box[2]
+        return w.n * (w.n - 1) / vol * 4.0 / 3.0 * math.pi * w.a ** 3
+
+
+def stage_work(stage: str, w, plan, esz: int, pairs: float):
+    """Algorithmic work of one stage per evaluation -> (kind, amount): kind 'flop' (ALU-bound
+    stages) or 'byte' (HBM-bound stages). Per-unit figures: DESIGN.md "Algorithmic work"."""
+    info = plan.info
+    n = w.n
+
+    def G(l):
+        d = info.grid_dims[l - 1]
+        return d[0] * d[1] * d[2]
+    nt = info.n_tiled
+    if stage == "pair":
+        return "flop", FLOP_PER_PAIR * pairs
+    if stage.startswith("conv_l"):
+        l = int(stage[6:])
+        return "flop", 2.0 * info.stencil_taps[l - 1] * G(l)
+    if stage.startswith("filter_l"):
+        l = int(stage[8:])
+        return "byte", 2.0 * esz * G(l)                      # read Q^l, write the filtered copy
+    if stage == "sort":
+        return "byte", n * (4 * esz) * 2 + n * 4 * 2         # read pos,q; write sorted records; perm
+    if stage == "anterpolate":
+        return "flop", n * (3 * w.p * 2 * w.p + 2.0 * w.p ** 3)
+    if stage == "interpolate":
+        return "flop", n * (6 * w.p * 2 * w.p + 8.0 * w.p ** 3)
+    if stage == "restrict":
+        return "byte", sum(esz * (G(l) + G(l + 1)) for l in range(1, nt))
+    if stage == "prolongate":
+        return "byte", sum(esz * (G(l + 1) + 2 * G(l)) for l in range(1, nt))
+    if stage == "top":
+        return "flop", 2.0 * info.top_points ** 2
+    return "byte", n * esz * 2.0                              # reduce
+
+
+def run_ours(args, rank: int, world: int):
+    import numpy as np
+    import torch
+    from paper_2510_05961_b200 import msm
+    from paper_2510_05961_b200.workloads import make_workload
+
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    w = make_workload(args.workload)
+    prec = w.precision
+    esz = 4 if prec == "fp32" else 8
+    plan = msm.Plan.for_workload(w, prec, device=local)
+    dt = plan.torch_dtype
+    npdt = np.float32 if prec == "fp32" else np.float64
+    pos = torch.tensor(w.positions, dtype=dt, device=dev).contiguous()
+    q = torch.tensor(w.charges, dtype=dt, device=dev).contiguous()
+    F = torch.zeros((w.n, 3), dtype=dt, device=dev)
+    V = torch.zeros(w.n, dtype=dt, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident arm (value)
+    plan.set_profiling(True)          # one cudaEventRecord between stages: per-stage times, live
+    for _ in range(args.warmup):
+        plan.evaluate(pos, q, F, V)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    stage_sum, launches, energy = {}, 0, 0.0
+    barrier()
+    for s in range(args.steps):
+        flush.fill_(s & 0xFF)                               # L2 flush, outside the event pair
+        ev[s][0].record()
+        energy, _ = plan.evaluate(pos, q, F, V)             # energy + forces + potentials + virial
+        ev[s][1].record()
+        torch.cuda.synchronize()
+        for k, v in plan.stage_times().items():
+            stage_sum[k] = stage_sum.get(k, 0.0) + v
+        launches += plan.launch_count()
+    barrier()
+    ms_total = sum(a.elapsed_time(b) for a, b in ev)
+    clocks = sampler.stop() if rank == 0 else None
+
+    # ---- end-to-end arm: host buffers through msm_evaluate_host, copies inside the timed region
+    hpos = torch.tensor(w.positions, dtype=dt).pin_memory()
+    hq = torch.tensor(w.charges, dtype=dt).pin_memory()
+    hF = torch.zeros((w.n, 3), dtype=dt).pin_memory()
+    hV = torch.zeros(w.n, dtype=dt).pin_memory()
+    for _ in range(max(1, args.warmup)):
+        plan.evaluate_host(hpos, hq, hF, hV)
+    ev2 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    for s in range(args.steps):
+        flush.fill_(s & 0xFF)
+        ev2[s][0].record()
+        plan.evaluate_host(hpos, hq, hF, hV)
+        ev2[s][1].record()
+        torch.cuda.synchronize()
+    barrier()
+    ms_e2e = sum(a.elapsed_time(b) for a, b in ev2)
+
+    t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device=dev)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total, ms_e2e = float(t[0]), float(t[1])
+    if rank != 0:
+        return None
+
+    peaks, peak_src = load_peaks()
+    dtype = "f32" if prec == "fp32" else "f64"
+    alu_peak = derived_alu_peak_tflops(dtype)
+    fma_meas = msm.measure_fma_peak(prec, local)
+    pairs = count_pairs(w)
+    stages = {}
+    for k, v in stage_sum.items():
+        ms = v / args.steps
+        kind, amount = stage_work(k, w, plan, esz, pairs)
+        if kind == "flop":
+            ach = amount / (ms * 1e-3) * 1e-12 if ms > 0 else 0.0
+            stages[k] = {"ms": round(ms, 5), "bound": "alu", "achieved": round(ach, 4), "unit": "TFLOP/s",
+                         "frac": round(ach / alu_peak, 5)}
+        else:
+            ach = amount / (ms * 1e-3) * 1e-9 if ms > 0 else 0.0
+            stages[k] = {"ms": round(ms, 5), "bound": "hbm", "achieved": round(ach, 2), "unit": "GB/s",
+                         "frac": round(ach / peaks["hbm_gbs"], 5)}
+    dom = max(stages, key=lambda k: stages[k]["ms"])
+    d = stages[dom]
+    roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"],
+                "peak": round(alu_peak, 2) if d["bound"] == "alu" else peaks["hbm_gbs"], "unit": d["unit"],
+                "frac": d["frac"], "traffic": None,
+                "peak_source": ("derived: 148 SM x %d lanes x 2 x 1.965 GHz" % (128 if dtype == "f32" else 64))
+                if d["bound"] == "alu" else f"{peak_src} MEASURED_PEAKS.json hbm_gbs",
+                "measured_fma_tflops": round(fma_meas, 2), "share_of_step": round(d["ms"] / (ms_total / args.steps), 4)}
+    out = {
+        "metric": METRIC, "value": world * w.n * args.steps / (ms_total * 1e-3), "unit": UNIT,
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
+        "config": {"workload": args.workload, "particles": w.n, "box": list(w.box), "periodic": list(w.periodic),
+                   "p": w.p, "h_target": w.h, "a": w.a, "levels": w.levels, "mu": int(plan.info.mu),
+                   "grids": [list(plan.info.grid_dims[i]) for i in range(plan.info.n_tiled)],
+                   "outputs": "energy+forces+potentials+virial", "parallelism": "replicas" if world > 1 else "1gpu",
+                   "l2": "256 MiB fill between steps (outside the per-step event pairs)"},
+        "e2e": {"value": world * w.n * args.steps / (ms_e2e * 1e-3), "unit": UNIT,
+                "h2d_bytes_per_step": w.n * 4 * esz, "d2h_bytes_per_step": w.n * 4 * esz + 64,
+                "ms_per_step": ms_e2e / args.steps},
+        "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "stages": stages,
+        "energy": energy,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(args.workload, 1, 0)[0]
+    return out
+
+
+# The oracle's bounded sample of each workload: same recipe, density and plan parameters, fewer
+# particles where the full case would take minutes on the host (about 10-30 s of CPU work).
+CPU_SAMPLE = {"cfg4_water1m": "cfg4_water300k"}
+
+
+def cpu_baseline(workload: str, steps: int, warmup: int):
+    """Time the oracle as it stands (gcc -O2 -fopenmp, fp64) on the host cores."""
+    import oracle
+    from paper_2510_05961_b200.workloads import make_workload
+    sample = CPU_SAMPLE.get(workload, workload)
+    w = make_workload(sample)
+    orc = oracle.Oracle(w.box, w.periodic, w.h, w.a, w.p, w.levels, mu=4)
+    for _ in range(warmup):
+        orc.evaluate(w.positions, w.charges, want_virial=True)
+    times = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        orc.evaluate(w.positions, w.charges, want_virial=True)
+        times.append(time.perf_counter() - t0)
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    total = sum(times)
+    note = "whole workload" if sample == workload else \
+        f"{sample}: {w.n} particles of the same recipe, density and plan parameters"
+    return {"value": w.n * steps / total, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{note}; one full oracle evaluation (fp64, all outputs) per step",
+            "seconds_per_step": total / steps}, w
+
+
+def run_reference(args, rank: int):
+    if rank != 0:
+        return None
+    cb, w = cpu_baseline(args.workload, args.steps, min(args.warmup, 1))
+    return {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": cb["seconds_per_step"] * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "sample": cb["sample"]},
+            "cpu_baseline": cb,
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4_water1m")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        args.steps = args.steps if args.steps is not None else 2
+        args.warmup = args.warmup if args.warmup is not None else 1
+        out = run_reference(args, rank)
+    else:
+        args.steps = args.steps if args.steps is not None else 20
+        args.warmup = max(3, args.warmup if args.warmup is not None else 5)
+        out = run_ours(args, rank, world)
+    if out is not None:
+        print(json.dumps(out), flush=True)
+    if world > 1 and args.impl == "ours":
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -7,11 +7,6 @@
 
 #include "plan.hpp"
 
-namespace msm {
-const char* const kStageNames[kNumStages] = {"sort", "pair", "anterpolate", "restrict", "convolve",
-                                             "top", "prolongate", "interpolate", "reduce"};
-}
-
 using namespace msm;
 
 namespace {
@@ -205,8 +200,17 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   p->out_F = dev_alloc(p, cap * 3 * p->esz);
   p->out_V = dev_alloc(p, cap * p->esz);
   if (cudaMallocHost((void**)&p->h_results, 8 * sizeof(double)) != cudaSuccess) return MSM_ERR_NOMEM;
-  for (int i = 0; i <= kNumStages; ++i)
+  for (int i = 0; i <= kMaxStages; ++i)
     if (cudaEventCreate(&p->ev[i]) != cudaSuccess) return MSM_ERR_CUDA;
+  // stage list of msm_evaluate, in launch order
+  for (const char* s : {"sort", "pair", "anterpolate", "restrict"}) p->stage_name_store.push_back(s);
+  for (int l = 1; l < p->n_t; ++l) {
+    p->stage_name_store.push_back("filter_l" + std::to_string(l));
+    p->stage_name_store.push_back("conv_l" + std::to_string(l));
+  }
+  for (const char* s : {"top", "prolongate", "interpolate", "reduce"}) p->stage_name_store.push_back(s);
+  for (const std::string& s : p->stage_name_store) p->stage_names.push_back(s.c_str());
+  p->n_stages = (int)p->stage_names.size();
   return MSM_OK;
 }
 
@@ -218,7 +222,7 @@ void msm_plan_destroy(msm_plan_t* p) {
   if (!p) return;
   for (void* d : p->allocs) cudaFree(d);
   if (p->h_results) cudaFreeHost(p->h_results);
-  for (int i = 0; i <= kNumStages; ++i)
+  for (int i = 0; i <= kMaxStages; ++i)
     if (p->ev[i]) cudaEventDestroy(p->ev[i]);
   delete p->H; delete p->S; delete p->pieces;
   delete p;

@@ -184,6 +184,7 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
       src = dst;
       din[ax] = g.P[ax];
     }
+    mark();
     constexpr int XT = sizeof(T) == 4 ? 16 : 8, ZT = 4;
     if (want_virial) {
       auto kern = k_conv<T, XT, ZT, true>;
@@ -201,8 +202,8 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
       MSM_LAUNCH(p, (kern<<<d.units, 32, d.smem, st>>>(g, d.rows, (const T*)d.staps, (const T*)d.gtaps,
                                                       (const T*)d.pad, (const T*)d.Q, (T*)d.E, d.wpart)));
     }
+    mark();
   }
-  mark();
 
   // ---------------- S6 top level
   {
@@ -269,7 +270,7 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
   if (cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }
   if (cudaGetLastError() != cudaSuccess) return MSM_ERR_CUDA;
   if (p->profiling)
-    for (int i = 0; i < kNumStages; ++i) cudaEventElapsedTime(&p->stage_ms[i], p->ev[i], p->ev[i + 1]);
+    for (int i = 0; i < p->n_stages; ++i) cudaEventElapsedTime(&p->stage_ms[i], p->ev[i], p->ev[i + 1]);
   return MSM_OK;
 }
 
@@ -333,8 +334,8 @@ msm_status_t msm_set_profiling(msm_plan_t* p, int enabled) {
 msm_status_t msm_get_stage_times(const msm_plan_t* p, int* n_stages, const char* const** names,
                                  const float** milliseconds) {
   if (!p || !n_stages || !names || !milliseconds) return MSM_ERR_INVALID_ARG;
-  *n_stages = kNumStages;
-  *names = kStageNames;
+  *n_stages = p->n_stages;
+  *names = p->stage_names.data();
   *milliseconds = p->stage_ms;
   return MSM_OK;
 }

@@ -11,8 +11,7 @@
 
 namespace msm {
 
-constexpr int kNumStages = 9;
-extern const char* const kStageNames[kNumStages];
+constexpr int kMaxStages = 2 * MSM_MAX_LEVELS + 16;   // sort pair anterpolate restrict {filter,conv}_l* top ...
 
 struct LevelDev {
   void *Q = nullptr, *E = nullptr, *pad = nullptr;   // grid charge, potential, haloed filtered charge
@@ -68,7 +67,10 @@ struct msm_plan {
 
   // profiling
   bool profiling = false;
-  cudaEvent_t ev[msm::kNumStages + 1]{};
-  float stage_ms[msm::kNumStages]{};
+  cudaEvent_t ev[msm::kMaxStages + 1]{};
+  float stage_ms[msm::kMaxStages]{};
+  int n_stages = 0;                               // stages of the last evaluate
+  std::vector<std::string> stage_name_store;      // fixed at plan creation (same order every call)
+  std::vector<const char*> stage_names;
   int launches = 0;
 };

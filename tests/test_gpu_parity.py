@@ -1,0 +1,243 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded inputs. Every test here needs a B200 and is marked gpu.
+
+Small cases span several tiles of every kernel and leave ragged tails; the config-sized cases are
+BASELINE.json's configs 1, 2, 3 (fp64 + fp32) and 5 in the launch configuration bench.py times.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from parity_util import compare, run_gpu, run_oracle, small_workload
+
+pytestmark = pytest.mark.gpu
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _log(name, errs):
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    with open(os.path.join(ROOT, "gpurun_out", "parity.jsonl"), "a") as f:
+        f.write(json.dumps({"case": name, **{k: float(v) for k, v in errs.items()}}) + "\n")
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_cuda():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2510_05961_b200 import msm
+    msm.lib()   # fails loudly if the extension is missing
+
+
+@pytest.mark.parametrize("kind,n,p", [("open", 700, 4), ("periodic", 1531, 4), ("slab", 1203, 4),
+                                      ("open", 333, 6), ("periodic", 900, 6), ("slab", 777, 6),
+                                      ("periodic", 500, 8)])
+def test_small_cases_fp64(kind, n, p):
+    w = small_workload(kind, n, seed=100 + n, p=p)
+    ref = run_oracle(w)
+    gpu = run_gpu(w)
+    _log(w.name + f"_p{p}", compare(w, gpu, ref, "fp64"))
+
+
+@pytest.mark.parametrize("kind,n,p", [("open", 700, 4), ("periodic", 1531, 4), ("slab", 1203, 6)])
+def test_small_cases_fp32(kind, n, p):
+    w = small_workload(kind, n, seed=100 + n, p=p, precision="fp32")
+    ref = run_oracle(w)
+    gpu = run_gpu(w, precision="fp32")
+    _log(w.name + f"_p{p}_fp32", compare(w, gpu, ref, "fp32"))
+
+
+@pytest.mark.parametrize("mu", [0, 2])
+def test_other_mu(mu):
+    w = small_workload("periodic", 640, seed=9, p=4)
+    ref = run_oracle(w, mu=mu)
+    gpu = run_gpu(w, mu=mu)
+    _log(w.name + f"_mu{mu}", compare(w, gpu, ref, "fp64"))
+
+
+def test_without_virial_same_results():
+    w = small_workload("periodic", 640, seed=9, p=4)
+    a = run_gpu(w, want_virial=True)
+    b = run_gpu(w, want_virial=False)
+    assert a["energy"] == b["energy"]
+    assert np.array_equal(a["forces"], b["forces"]) and np.array_equal(a["potentials"], b["potentials"])
+
+
+@pytest.mark.parametrize("name", ["cfg1_open512", "cfg2_nacl4096", "cfg2_nacl4096_shifted"])
+def test_configs_small_fp64(name):
+    from paper_2510_05961_b200.workloads import make_workload
+    w = make_workload(name)
+    ref = run_oracle(w)
+    gpu = run_gpu(w)
+    _log(name, compare(w, gpu, ref, "fp64"))
+
+
+def test_config1_close_to_direct_sum():
+    """Config 1's own check: MSM (GPU) against the O(N^2) direct Coulomb sum, within MSM error."""
+    from oracle import direct_sum
+    from paper_2510_05961_b200.workloads import make_workload
+    w = make_workload("cfg1_open512")
+    gpu = run_gpu(w)
+    U, F, V = direct_sum(w.positions, w.charges)
+    assert abs(gpu["energy"] - U) / abs(U) < 5e-3
+    assert np.sqrt(np.mean((gpu["forces"] - F) ** 2)) / np.sqrt(np.mean(F ** 2)) < 1e-2
+
+
+def test_config2_madelung_constant():
+    """Config 2's own check: the GPU energy reproduces the rock-salt Madelung constant 1.747565
+    (Eq. 22) within MSM error; forces vanish by symmetry."""
+    from paper_2510_05961_b200.workloads import make_workload
+    w = make_workload("cfg2_nacl4096")
+    gpu = run_gpu(w)
+    M = -gpu["energy"] * 2.82 / 2048
+    assert abs(M - 1.747565) < 5e-4, M
+    assert np.abs(gpu["forces"]).max() < 1e-9
+
+
+@pytest.mark.parametrize("name", ["cfg3_water30k_fp64", "cfg3_water30k_fp32"])
+def test_config3_water(name):
+    from paper_2510_05961_b200.workloads import make_workload
+    w = make_workload(name)
+    ref = run_oracle(w)
+    gpu = run_gpu(w)
+    _log(name, compare(w, gpu, ref, w.precision))
+
+
+def test_config5_slab():
+    from paper_2510_05961_b200.workloads import make_workload
+    w = make_workload("cfg5_slab100k")
+    ref = run_oracle(w)
+    gpu = run_gpu(w)
+    _log(w.name, compare(w, gpu, ref, "fp64"))
+
+
+def test_config4_one_million_sampled():
+    """BASELINE config 4 at N = 999 999, fp32, in bench.py's launch configuration: the oracle
+    cannot run the whole case in seconds, so check (a) sampled particles' short-range potential
+    and force against the oracle's brute-force pair sum over ALL particles, (b) the level-1 grid
+    charge against the oracle's anterpolation (full grid), (c) properties that hold at any size:
+    U = 1/2 sum q_i V_i, total grid charge = total charge, net force ~ 0."""
+    import torch
+    from oracle import Oracle
+    from paper_2510_05961_b200 import msm
+    from paper_2510_05961_b200.workloads import make_workload
+    w = make_workload("cfg4_water1m")
+    plan = msm.Plan.for_workload(w, "fp32")
+    dev = torch.device("cuda", 0)
+    pos = torch.tensor(w.positions, dtype=torch.float32, device=dev)
+    q = torch.tensor(w.charges, dtype=torch.float32, device=dev)
+    F = torch.zeros((w.n, 3), dtype=torch.float32, device=dev)
+    V = torch.zeros(w.n, dtype=torch.float32, device=dev)
+    U, W = plan.evaluate(pos, q, F, V)
+    Fh, Vh = F.cpu().numpy().astype(np.float64), V.cpu().numpy().astype(np.float64)
+    # (c) properties
+    assert abs(U - 0.5 * np.dot(w.charges, Vh)) <= 1e-6 * abs(U)
+    Q1 = plan.debug_grid(1, "Q")
+    assert abs(Q1.sum() - w.charges.sum()) < 1e-2
+    assert np.abs(Fh.sum(axis=0)).max() < 1e-3 * np.abs(Fh).sum(axis=0).max()
+    # (b) anterpolation, whole grid
+    orc = Oracle(w.box, w.periodic, w.h, w.a, w.p, w.levels)
+    Qr = orc.anterpolate(w.positions, w.charges)
+    assert np.abs(Q1 - Qr).max() <= 2e-5 * np.abs(Qr).max()
+    # (a) sampled short-range part + interpolation of the GPU's own E1 by the oracle
+    sel = np.random.default_rng(0).choice(w.n, 64, replace=False).astype(np.int32)
+    Fs, Vs, _ = orc.short_range(w.positions, w.charges, sel=sel, want_virial=False)
+    orc.set_grid(1, "E", plan.debug_grid(1, "E"))
+    Fl, Vl = orc.interpolate(w.positions[sel], w.charges[sel])
+    from oracle import gamma
+    Vref = Vs + Vl - w.charges[sel] * gamma(w.p, 0.0) / w.a
+    Fref = Fs + Fl
+    assert np.abs(Vh[sel] - Vref).max() <= 2e-5 * np.abs(Vref).max()
+    assert np.sqrt(np.mean((Fh[sel] - Fref) ** 2)) <= 1e-4 * np.sqrt(np.mean(Fref ** 2))
+
+
+def test_host_entry_point_matches_device_entry_point():
+    w = small_workload("periodic", 1531, seed=1631, p=4)
+    from paper_2510_05961_b200 import msm
+    gpu = run_gpu(w)
+    plan = gpu["plan"]
+    F = np.zeros((w.n, 3)); V = np.zeros(w.n)
+    U, W = plan.evaluate_host(np.ascontiguousarray(w.positions), np.ascontiguousarray(w.charges), F, V)
+    assert U == gpu["energy"] and np.array_equal(F, gpu["forces"]) and np.array_equal(V, gpu["potentials"])
+    assert np.array_equal(W, gpu["virial"])
+
+
+def test_deterministic_and_permutation_invariant():
+    """Fixed summation orders: repeated calls are bit-identical; permuting the input permutes the
+    per-particle outputs (bit-identical short-range + interpolation; the grids see the same
+    canonical order only up to the index order inside a cell, so compare to 1e-13)."""
+    w = small_workload("periodic", 1531, seed=1631, p=4)
+    a = run_gpu(w)
+    b = run_gpu(w)
+    assert a["energy"] == b["energy"] and np.array_equal(a["forces"], b["forces"])
+    perm = np.random.default_rng(3).permutation(w.n)
+    import dataclasses
+    wp = dataclasses.replace(w, positions=w.positions[perm], charges=w.charges[perm])
+    c = run_gpu(wp)
+    assert abs(c["energy"] - a["energy"]) <= 1e-12 * abs(a["energy"])
+    assert np.abs(c["forces"] - a["forces"][perm]).max() <= 1e-12 * np.abs(a["forces"]).max()
+
+
+def test_edge_cases():
+    import torch
+    from paper_2510_05961_b200 import msm
+    dev = torch.device("cuda", 0)
+    plan = msm.Plan((20.0,) * 3, (1, 1, 1), 2.0, 6.0, 4, 2, "fp64", max_particles=16)
+    # empty input
+    z3 = torch.zeros((0, 3), dtype=torch.float64, device=dev)
+    z1 = torch.zeros(0, dtype=torch.float64, device=dev)
+    U, W = plan.evaluate(z3, z1, z3.clone(), z1.clone())
+    assert U == 0.0 and np.all(W == 0.0)
+    # one particle: only the self-interaction through the grid minus the self term (MSM error)
+    pos = torch.tensor([[3.0, 4.0, 5.0]], dtype=torch.float64, device=dev)
+    q = torch.tensor([1.0], dtype=torch.float64, device=dev)
+    F = torch.zeros((1, 3), dtype=torch.float64, device=dev); V = torch.zeros(1, dtype=torch.float64, device=dev)
+    U, W = plan.evaluate(pos, q, F, V)
+    from oracle import Oracle
+    ref = Oracle((20.0,) * 3, (1, 1, 1), 2.0, 6.0, 4, 2).evaluate(pos.cpu().numpy(), q.cpu().numpy())
+    assert abs(U - ref["energy"]) <= 1e-10 * max(abs(ref["energy"]), 1e-3)
+    # capacity
+    big = torch.zeros((17, 3), dtype=torch.float64, device=dev)
+    with pytest.raises(msm.MsmError) as e:
+        plan.evaluate(big, torch.zeros(17, dtype=torch.float64, device=dev))
+    assert e.value.status == 4
+    # periodic coordinates outside the box are wrapped, not rejected
+    pos2 = torch.tensor([[3.0, 4.0, 5.0], [23.5, -16.0, 45.0]], dtype=torch.float64, device=dev)
+    q2 = torch.tensor([1.0, -1.0], dtype=torch.float64, device=dev)
+    U2, _ = plan.evaluate(pos2, q2)
+    pos3 = torch.tensor([[3.0, 4.0, 5.0], [3.5, 4.0, 5.0]], dtype=torch.float64, device=dev)
+    U3, _ = plan.evaluate(pos3, q2)
+    assert abs(U2 - U3) <= 1e-12 * abs(U3)
+    # open axis: out of box and non-finite are reported
+    oplan = msm.Plan((20.0,) * 3, (0, 0, 0), 2.0, 6.0, 4, 2, "fp64", max_particles=16)
+    bad = torch.tensor([[3.0, 4.0, 25.0], [1.0, 1.0, 1.0]], dtype=torch.float64, device=dev)
+    with pytest.raises(msm.MsmError) as e:
+        oplan.evaluate(bad, q2)
+    assert e.value.status == 5
+    nan = torch.tensor([[3.0, float("nan"), 5.0], [1.0, 1.0, 1.0]], dtype=torch.float64, device=dev)
+    with pytest.raises(msm.MsmError) as e:
+        oplan.evaluate(nan, q2)
+    assert e.value.status == 5
+    # particles exactly on the open faces are legal
+    face = torch.tensor([[0.0, 0.0, 0.0], [20.0, 20.0, 20.0]], dtype=torch.float64, device=dev)
+    Uf, _ = oplan.evaluate(face, q2)
+    reff = Oracle((20.0,) * 3, (0, 0, 0), 2.0, 6.0, 4, 2).evaluate(face.cpu().numpy(), q2.cpu().numpy())
+    assert abs(Uf - reff["energy"]) <= 1e-10 * abs(reff["energy"])
+
+
+def test_plan_errors():
+    from paper_2510_05961_b200 import msm
+    with pytest.raises(msm.MsmError) as e:
+        msm.Plan((20.0,) * 3, (1, 1, 1), 2.0, 11.0, 4, 2)          # a > L/2
+    assert e.value.status == 3
+    with pytest.raises(msm.MsmError) as e:
+        msm.Plan((20.0,) * 3, (1, 0, 0), 2.0, 6.0, 4, 2)           # one periodic axis (T4)
+    assert e.value.status == 2
+    with pytest.raises(msm.MsmError) as e:
+        msm.Plan((20.0,) * 3, (1, 1, 1), 2.0, 6.0, 5, 2)           # odd order
+    assert e.value.status == 1
+    with pytest.raises(msm.MsmError) as e:
+        msm.Plan((20.0, -1.0, 20.0), (1, 1, 1), 2.0, 6.0, 4, 2)
+    assert e.value.status == 1
