@@ -123,12 +123,12 @@ def stage_work(stage: str, w, plan, esz: int, pairs: float):
     nt = info.n_tiled
     if stage == "pair":
         return "flop", FLOP_PER_PAIR * pairs
-    if stage.startswith("conv_l"):
-        l = int(stage[6:])
-        return "flop", 2.0 * info.stencil_taps[l - 1] * G(l)
-    if stage.startswith("filter_l"):
-        l = int(stage[8:])
-        return "byte", 2.0 * esz * G(l)                      # read Q^l, write the filtered copy
+    if stage == "conv":                                       # 2 T_s flop per grid point and level
+        return "flop", sum(2.0 * info.stencil_taps[l - 1] * G(l) for l in range(1, nt))
+    if stage == "conv_virial":                                # correlation over the half space of taps
+        return "flop", sum(1.0 * info.stencil_taps[l - 1] * G(l) for l in range(1, nt))
+    if stage == "filter":
+        return "byte", sum(2.0 * esz * G(l) for l in range(1, nt))   # read Q^l, write the filtered copy
     if stage == "sort":
         return "byte", n * (4 * esz) * 2 + n * 4 * 2         # read pos,q; write sorted records; perm
     if stage == "anterpolate":

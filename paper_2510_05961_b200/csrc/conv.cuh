@@ -1,34 +1,63 @@
 // conv.cuh -- S5: per-level grid<->grid convolution with the truncated stencil of k_l
-// (Eq. 11; stencil P:268 Eq. 20), FP-pipe bound.
+// (Eq. 11; stencil P:268 Eq. 20), FP-pipe bound, and the grid part of the virial (reading V).
 //
 // Formulation. K^l = omega'(x)omega'(x)omega' * s_l (Eq. 20) and convolution is associative, so
-// e^l = s_l * qpad with qpad = omega'-filtered, haloed grid charge (k_pad_filter). s_l is non-zero
+// e^l = s_l * qpad with qpad = omega'-filtered, haloed grid charge (gridops.cuh). s_l is non-zero
 // only inside the cutoff ellipsoid (3-5x fewer taps than the folded K^l) and is even in n, so
 // e_m = sum_n s(n) qpad[m + n]. The halo holds periodic images (as many wraps as the stencil
-// needs) or zeros (open axes), so the kernel has no boundary logic.
+// needs) or zeros (open axes), so the kernels have no boundary logic.
 //
-// Work unit = one warp: outputs x in [X, X+XT), y = Y + lane, z in [Z, Z+ZT); each thread keeps
-// XT*ZT accumulators in registers. The warp streams input z-planes through shared memory; one
-// plane feeds all ZT output planes (tap row dz = z_in - z_out), so a 16-byte shared-memory window
-// load is amortised over up to 4*XT*ZT FMAs, and every tap quad (one 16-byte broadcast load from
-// the L1-resident table) feeds 4*XT FMAs. Rows of the stencil are stored as runs of 4-tap chunks
-// covering only the ellipsoid; chunk tests are warp-uniform, so there is no divergence.
+// Work unit = one warp = one block: output tile x in [X, X+XT), y = Y + lane, z in [Z, Z+ZT) and a
+// SLICE of the input z-planes. Each thread keeps XT*ZT accumulators in registers; the warp streams
+// its input planes through shared memory; one plane feeds all ZT output planes (tap row
+// dz = z_in - z_out), so a 16-byte shared-memory window load is amortised over up to 4*XT*ZT FMAs
+// and every tap quad (one 16-byte broadcast load from the L1-resident table) feeds 4*XT FMAs.
+// Stencil rows are stored as runs of 4-tap chunks covering only the ellipsoid; chunk tests are
+// warp-uniform (no divergence). ONE launch covers every tiled level: a block finds its level from
+// the unit ranges in the descriptor table, so the coarse levels (too small to fill 148 SMs on their
+// own) run beside the finest one. Slicing the input planes gives the scheduler units of similar,
+// small size; slice partials go to a scratch array and are summed in slice order by k_sum_slices
+// (deterministic).
 //
-// VIRIAL adds the strain derivative of the level's energy (reading V): with c_t = sum_i q_i
-// qpad[i + n_t] over the thread's outputs, S_ab += g(n_t) n_a n_b c_t, g = k_l'(r)/r; the host
-// scales by -1/2 h_a h_b. Costs one more FMA per tap and output.
+// MODE_VIRIAL computes the strain derivative of the level's energy: with the correlation
+// C(n) = sum_m Q_m qpad[m + n] (even in n), W_ab ~ sum_n g(n) n_a n_b C(n), g = k_l'(r)/r. Only
+// the half space n > 0 (lexicographic in z, y, x) is visited, with weight 2; per tap and output it
+// costs one FMA (c_t = sum_i q_i win[i + t]) plus three per tap for the x-moments.
 #pragma once
 #include "device_common.cuh"
 
 namespace msm {
 
-struct ConvGeom {
+constexpr int kMaxConvLevels = 16;
+constexpr int kMaxConvSlices = 71;
+
+struct ConvLevel {
   int M[3];        // output grid dims
   int P[3];        // padded input dims
   int R[3];        // stencil half-widths (y, z used as halo; x halo is X0)
   int X0;          // x halo, multiple of 4, >= R[0]
-  int tiles[3];    // units per axis
+  int tiles[3];    // output tiles per axis
   int pitch;       // shared-memory row pitch in elements
+  int ny;          // 2 R[1] + 1
+  int nslices;     // potential kernel: slices of the 2 R[2] + ZT input planes
+  int vslices;     // virial kernel: slices of the R[2] + ZT input planes with dz >= 0
+  unsigned char pb[kMaxConvSlices + 1];   // slice s covers input planes [pb[s], pb[s+1]) (balanced by taps)
+  unsigned char vb[kMaxConvSlices + 1];
+  int unit0, vunit0;          // first unit of this level in the potential / virial launch
+  const int4* rows;           // (tap chunk offset, first chunk, last chunk, -) per (dz, dy)
+  const int4* vrows;          // same for the half-space virial taps
+  const void* staps;          // s_l in 4-tap chunks
+  const void* vtaps;          // per chunk: 4 x 2g, 4 x 2g dx, 4 x 2g dx^2
+  const void* pad;            // omega'-filtered haloed grid charge
+  const void* Q;              // grid charge (virial)
+  void* out;                  // E^l if nslices == 1, else scratch [slice][z][y][x]
+  double* wpart;              // virial partials, 6 per unit
+};
+
+struct ConvTable {
+  int nlev;
+  int total_units, total_vunits;
+  ConvLevel lev[kMaxConvLevels];
 };
 
 template <typename T> struct SmemVec;
@@ -55,65 +84,83 @@ template <> struct SmemVec<double> {
   }
 };
 
-template <typename T, int XT, int ZT, bool VIRIAL>
+// stage padded plane pz: rows Y .. Y+nrow-1, x X .. X+WX-1 (padded indices) into shared memory
+template <typename T>
+__device__ __forceinline__ void stage_plane(const ConvLevel& g, const T* __restrict__ qpad, T* plane, int pz,
+                                            int X, int Y, int nrow, int WX, int lane) {
+  const T* src = qpad + ((size_t)pz * g.P[1] + Y) * g.P[0] + X;
+  const int vper = WX / 4, nvec = nrow * vper;
+  __syncwarp();
+  for (int v = lane; v < nvec; v += 32) {
+    const int r = v / vper, cx = (v - r * vper) * 4;
+    T t[4];
+    SmemVec<T>::ldg(src + (size_t)r * g.P[0] + cx, t);
+    T* dst = plane + r * g.pitch + cx;
+    dst[0] = t[0]; dst[1] = t[1]; dst[2] = t[2]; dst[3] = t[3];
+  }
+  __syncwarp();
+}
+
+struct ConvUnit {
+  int lev, X, Y, Z, slice, local;
+};
+
+template <bool VIRIAL, int XT, int ZT>
+__device__ __forceinline__ ConvUnit decode_unit(const ConvTable& tab, int u) {
+  ConvUnit cu;
+  int l = 0;
+#pragma unroll 1
+  for (int k = 1; k < tab.nlev; ++k)
+    if (u >= (VIRIAL ? tab.lev[k].vunit0 : tab.lev[k].unit0)) l = k;
+  const ConvLevel& g = tab.lev[l];
+  int r = u - (VIRIAL ? g.vunit0 : g.unit0);
+  cu.lev = l;
+  cu.local = r;
+  const int ns = VIRIAL ? g.vslices : g.nslices;
+  cu.slice = r % ns; r /= ns;
+  cu.X = (r % g.tiles[0]) * XT; r /= g.tiles[0];
+  cu.Y = (r % g.tiles[1]) * 32;
+  cu.Z = (r / g.tiles[1]) * ZT;
+  return cu;
+}
+
+// ---------------------------------------------------------------------------------- potential
+template <typename T, int XT, int ZT>
 __global__ void __launch_bounds__(32)
-k_conv(ConvGeom g, const int4* __restrict__ rows, const T* __restrict__ staps, const T* __restrict__ gtaps,
-       const T* __restrict__ qpad, const T* __restrict__ Q, T* __restrict__ E, double* __restrict__ wpart) {
+k_conv(const ConvTable* __restrict__ tabp) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* plane = reinterpret_cast<T*>(smem_raw);
+  const ConvTable& tab = *tabp;
   const int lane = threadIdx.x;
-  int u = blockIdx.x;
-  const int tx = u % g.tiles[0]; u /= g.tiles[0];
-  const int ty = u % g.tiles[1], tz = u / g.tiles[1];
-  const int X = tx * XT, Y = ty * 32, Z = tz * ZT;
+  const ConvUnit cu = decode_unit<false, XT, ZT>(tab, blockIdx.x);
+  const ConvLevel& g = tab.lev[cu.lev];
+  const int X = cu.X, Y = cu.Y, Z = cu.Z;
   const int Ry = g.R[1], Rz = g.R[2];
   const int nrow = 32 + 2 * Ry;
   const int WX = XT + 2 * g.X0 + 4;
-  const int ny = 2 * Ry + 1;
+  const int ny = g.ny;
+  const int4* __restrict__ rows = g.rows;
+  const T* __restrict__ staps = reinterpret_cast<const T*>(g.staps);
+  const T* __restrict__ qpad = reinterpret_cast<const T*>(g.pad);
 
   T acc[ZT][XT];
 #pragma unroll
   for (int k = 0; k < ZT; ++k)
 #pragma unroll
     for (int i = 0; i < XT; ++i) acc[k][i] = 0;
-  T qr[VIRIAL ? ZT : 1][VIRIAL ? XT : 1];
-  double S[6] = {0, 0, 0, 0, 0, 0};
-  if (VIRIAL) {
-#pragma unroll
-    for (int k = 0; k < ZT; ++k)
-#pragma unroll
-      for (int i = 0; i < XT; ++i) {
-        const int x = X + i, y = Y + lane, z = Z + k;
-        qr[k][i] = (x < g.M[0] && y < g.M[1] && z < g.M[2]) ? Q[((size_t)z * g.M[1] + y) * g.M[0] + x] : (T)0;
-      }
-  }
 
-  for (int zr = -Rz; zr <= ZT - 1 + Rz; ++zr) {
-    // stage input plane z = Z + zr (padded index + Rz): rows Y .. Y+nrow-1, x X .. X+WX-1 (padded)
-    {
-      const T* src = qpad + ((size_t)(Z + zr + Rz) * g.P[1] + Y) * g.P[0] + X;
-      const int vper = WX / 4, nvec = nrow * vper;
-      __syncwarp();
-      for (int v = lane; v < nvec; v += 32) {
-        const int r = v / vper, cx = (v - r * vper) * 4;
-        T t[4];
-        SmemVec<T>::ldg(src + (size_t)r * g.P[0] + cx, t);
-        T* dst = plane + r * g.pitch + cx;
-        dst[0] = t[0]; dst[1] = t[1]; dst[2] = t[2]; dst[3] = t[3];
-      }
-      __syncwarp();
-    }
+  const int p0 = g.pb[cu.slice], p1 = g.pb[cu.slice + 1];
+  for (int pz = p0; pz < p1; ++pz) {
+    const int zr = pz - Rz;              // input plane z = Z + zr
+    stage_plane<T>(g, qpad, plane, Z + pz, X, Y, nrow, WX, lane);
     for (int dy = -Ry; dy <= Ry; ++dy) {
       int4 re[ZT];
       int cl = 1 << 30, ch = -1;
 #pragma unroll
       for (int k = 0; k < ZT; ++k) {
         const int dz = zr - k;
-        if (dz >= -Rz && dz <= Rz) {
-          re[k] = __ldg(rows + (dz + Rz) * ny + (dy + Ry));
-        } else {
-          re[k] = make_int4(0, 1, 0, 0);   // empty
-        }
+        if (dz >= -Rz && dz <= Rz) re[k] = __ldg(rows + (dz + Rz) * ny + (dy + Ry));
+        else re[k] = make_int4(0, 1, 0, 0);   // empty
         if (re[k].y <= re[k].z) { cl = min(cl, re[k].y); ch = max(ch, re[k].z); }
       }
       const T* srow = plane + (lane + dy + Ry) * g.pitch;
@@ -128,69 +175,145 @@ k_conv(ConvGeom g, const int4* __restrict__ rows, const T* __restrict__ staps, c
 #pragma unroll
         for (int k = 0; k < ZT; ++k) {
           if (c >= re[k].y && c <= re[k].z) {
-            const int toff = (re[k].x + c - re[k].y) * 4;
             T tp[4];
-            SmemVec<T>::ldg(staps + toff, tp);
+            SmemVec<T>::ldg(staps + (re[k].x + c - re[k].y) * 4, tp);
 #pragma unroll
             for (int t = 0; t < 4; ++t)
 #pragma unroll
               for (int i = 0; i < XT; ++i) acc[k][i] = fma(tp[t], win[i + t], acc[k][i]);
-            if (VIRIAL) {
-              T gp[4];
-              SmemVec<T>::ldg(gtaps + toff, gp);
-              const T fdx = (T)(4 * c - g.X0);
-              T e0 = 0, e1 = 0, e2 = 0;
-#pragma unroll
-              for (int t = 0; t < 4; ++t) {
-                T c0 = 0, c1 = 0;
-#pragma unroll
-                for (int i = 0; i < XT; i += 2) {
-                  c0 = fma(qr[k][i], win[i + t], c0);
-                  c1 = fma(qr[k][i + 1], win[i + 1 + t], c1);
-                }
-                const T gc = gp[t] * (c0 + c1), d = fdx + (T)t;
-                e0 += gc;
-                e1 = fma(d, gc, e1);
-                e2 = fma(d * d, gc, e2);
-              }
-              const double fy = (double)dy, fz = (double)(zr - k);
-              const double d0 = (double)e0, d1 = (double)e1;
-              S[0] += (double)e2;
-              S[1] = fma(fy * fy, d0, S[1]);
-              S[2] = fma(fz * fz, d0, S[2]);
-              S[3] = fma(fy, d1, S[3]);
-              S[4] = fma(fz, d1, S[4]);
-              S[5] = fma(fy * fz, d0, S[5]);
-            }
           }
         }
       }
     }
   }
-  // outputs
-  {
-    const int y = Y + lane;
-    if (y < g.M[1]) {
+  // outputs (slice partial or the final value)
+  const int y = Y + lane;
+  if (y < g.M[1]) {
+    T* out = reinterpret_cast<T*>(g.out) + (size_t)cu.slice * g.M[0] * g.M[1] * g.M[2];
 #pragma unroll
-      for (int k = 0; k < ZT; ++k) {
-        const int z = Z + k;
-        if (z < g.M[2]) {
-          T* dst = E + ((size_t)z * g.M[1] + y) * g.M[0] + X;
+    for (int k = 0; k < ZT; ++k) {
+      const int z = Z + k;
+      if (z < g.M[2]) {
+        T* dst = out + ((size_t)z * g.M[1] + y) * g.M[0] + X;
 #pragma unroll
-          for (int i = 0; i < XT; ++i)
-            if (X + i < g.M[0]) dst[i] = acc[k][i];
-        }
+        for (int i = 0; i < XT; ++i)
+          if (X + i < g.M[0]) dst[i] = acc[k][i];
       }
     }
   }
-  if (VIRIAL) {
+}
+
+// E[i] = sum_s part[s][i], s ascending (fixed order)
+template <typename T>
+__global__ void k_sum_slices(size_t n, int nslices, const T* __restrict__ part, T* __restrict__ E) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  T s = part[i];
+  for (int k = 1; k < nslices; ++k) s += part[(size_t)k * n + i];
+  E[i] = s;
+}
+
+// ------------------------------------------------------------------------------------- virial
+template <typename T, int XT, int ZT>
+__global__ void __launch_bounds__(32)
+k_conv_virial(const ConvTable* __restrict__ tabp) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* plane = reinterpret_cast<T*>(smem_raw);
+  const ConvTable& tab = *tabp;
+  const int lane = threadIdx.x;
+  const ConvUnit cu = decode_unit<true, XT, ZT>(tab, blockIdx.x);
+  const ConvLevel& g = tab.lev[cu.lev];
+  const int X = cu.X, Y = cu.Y, Z = cu.Z;
+  const int Ry = g.R[1], Rz = g.R[2];
+  const int nrow = 32 + 2 * Ry;
+  const int WX = XT + 2 * g.X0 + 4;
+  const int ny = g.ny;
+  const int4* __restrict__ rows = g.vrows;
+  const T* __restrict__ vtaps = reinterpret_cast<const T*>(g.vtaps);
+  const T* __restrict__ qpad = reinterpret_cast<const T*>(g.pad);
+  const T* __restrict__ Q = reinterpret_cast<const T*>(g.Q);
+
+  T qr[ZT][XT];
 #pragma unroll
-    for (int k = 0; k < 6; ++k) {
-      double v = S[k];
+  for (int k = 0; k < ZT; ++k)
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-      if (lane == 0) wpart[(size_t)blockIdx.x * 6 + k] = v;
+    for (int i = 0; i < XT; ++i) {
+      const int x = X + i, y = Y + lane, z = Z + k;
+      qr[k][i] = (x < g.M[0] && y < g.M[1] && z < g.M[2]) ? Q[((size_t)z * g.M[1] + y) * g.M[0] + x] : (T)0;
     }
+  double S[6] = {0, 0, 0, 0, 0, 0};
+
+  // only dz = zr - k >= 0: input planes zr in [0, ZT - 1 + Rz], padded index pz = zr + Rz
+  const int p0 = g.vb[cu.slice], p1 = g.vb[cu.slice + 1];
+  for (int pp = p0; pp < p1; ++pp) {
+    const int zr = pp;
+    stage_plane<T>(g, qpad, plane, Z + zr + Rz, X, Y, nrow, WX, lane);
+    for (int dy = -Ry; dy <= Ry; ++dy) {
+      int4 re[ZT];
+      int cl = 1 << 30, ch = -1;
+#pragma unroll
+      for (int k = 0; k < ZT; ++k) {
+        const int dz = zr - k;
+        if (dz >= 0 && dz <= Rz) re[k] = __ldg(rows + dz * ny + (dy + Ry));
+        else re[k] = make_int4(0, 1, 0, 0);
+        if (re[k].y <= re[k].z) { cl = min(cl, re[k].y); ch = max(ch, re[k].z); }
+      }
+      if (ch < cl) continue;
+      T e0[ZT], e1[ZT], e2[ZT];
+#pragma unroll
+      for (int k = 0; k < ZT; ++k) { e0[k] = 0; e1[k] = 0; e2[k] = 0; }
+      const T* srow = plane + (lane + dy + Ry) * g.pitch;
+      for (int c = cl; c <= ch; ++c) {
+        T win[XT + 4];
+#pragma unroll
+        for (int j = 0; j < XT + 4; j += 4) {
+          T t[4];
+          SmemVec<T>::load4(srow + 4 * c + j, t);
+          win[j] = t[0]; win[j + 1] = t[1]; win[j + 2] = t[2]; win[j + 3] = t[3];
+        }
+#pragma unroll
+        for (int k = 0; k < ZT; ++k) {
+          if (c >= re[k].y && c <= re[k].z) {
+            const T* tp = vtaps + (size_t)(re[k].x + c - re[k].y) * 12;
+            T g0[4], g1[4], g2[4];
+            SmemVec<T>::ldg(tp, g0);
+            SmemVec<T>::ldg(tp + 4, g1);
+            SmemVec<T>::ldg(tp + 8, g2);
+#pragma unroll
+            for (int t = 0; t < 4; ++t) {
+              T c0 = 0, c1 = 0;
+#pragma unroll
+              for (int i = 0; i < XT; i += 2) {
+                c0 = fma(qr[k][i], win[i + t], c0);
+                c1 = fma(qr[k][i + 1], win[i + 1 + t], c1);
+              }
+              const T ct = c0 + c1;
+              e0[k] = fma(g0[t], ct, e0[k]);
+              e1[k] = fma(g1[t], ct, e1[k]);
+              e2[k] = fma(g2[t], ct, e2[k]);
+            }
+          }
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < ZT; ++k) {
+        const double fy = (double)dy, fz = (double)(zr - k);
+        const double d0 = (double)e0[k], d1 = (double)e1[k];
+        S[0] += (double)e2[k];
+        S[1] = fma(fy * fy, d0, S[1]);
+        S[2] = fma(fz * fz, d0, S[2]);
+        S[3] = fma(fy, d1, S[3]);
+        S[4] = fma(fz, d1, S[4]);
+        S[5] = fma(fy * fz, d0, S[5]);
+      }
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 6; ++k) {
+    double v = S[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (lane == 0) g.wpart[(size_t)cu.local * 6 + k] = v;
   }
 }
 

@@ -2,6 +2,7 @@
 // and every device buffer of a plan. See include/msm.h.
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -38,13 +39,30 @@ void* upload(msm_plan* p, const std::vector<double>& v) {
 
 int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
-// stencil row table + chunked taps of one tiled level (see conv.cuh)
+// balanced partition of n weighted items into S contiguous slices: bounds b[0..S]
+void balanced_bounds(const std::vector<double>& w, int S, unsigned char* b) {
+  const int n = (int)w.size();
+  double tot = 0;
+  for (double v : w) tot += v;
+  b[0] = 0;
+  int i = 0;
+  double run = 0;
+  for (int s = 1; s < S; ++s) {
+    const double target = tot * s / S;
+    while (i < n && run + 0.5 * w[i] < target && n - (i + 1) >= S - s) { run += w[i]; ++i; }
+    if (i < s) { while (i < s) { run += w[i]; ++i; } }   // at least one plane per slice
+    b[s] = (unsigned char)i;
+  }
+  b[S] = (unsigned char)n;
+}
+
+// stencil row tables + chunked taps of one tiled level (see conv.cuh)
 void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   const Level& lv = p->H->lev[l];
   LevelDev& d = p->lev[l];
   const SampledStencil st = sample_level_stencil(*p->H, *p->S, l);
   d.taps = st.taps;
-  ConvGeom& g = d.cg;
+  ConvLevel& g = p->conv.lev[l - 1];
   for (int ax = 0; ax < 3; ++ax) { g.M[ax] = lv.M[ax]; g.R[ax] = st.R[ax]; }
   g.X0 = round_up(st.R[0], 4);
   g.tiles[0] = (lv.M[0] + XT - 1) / XT;
@@ -58,16 +76,17 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   if (p->fp32) { pitch = round_up(pitch, 4); if (((pitch / 4) & 1) == 0) pitch += 4; }
   else { pitch = round_up(pitch, 2); if (((pitch / 2) & 1) == 0) pitch += 2; }
   g.pitch = pitch;
-  d.smem = (size_t)(32 + 2 * st.R[1]) * pitch * p->esz;
-  d.units = g.tiles[0] * g.tiles[1] * g.tiles[2];
+  g.ny = 2 * st.R[1] + 1;
+  p->conv_smem = std::max(p->conv_smem, (size_t)(32 + 2 * st.R[1]) * pitch * p->esz);
 
   const double A = std::ldexp(p->mp.a, l);
-  const int ny = 2 * st.R[1] + 1, nz = 2 * st.R[2] + 1;
-  std::vector<int4> rows((size_t)ny * nz);
-  std::vector<double> ts, tg;
-  for (int dz = -st.R[2]; dz <= st.R[2]; ++dz)
+  const int ny = g.ny, nz = 2 * st.R[2] + 1, Rz = st.R[2];
+  std::vector<int4> rows((size_t)ny * nz), vrows((size_t)ny * (Rz + 1));
+  std::vector<double> ts, tv;
+  std::vector<double> wz(nz, 0.0), wzv(Rz + 1, 0.0);     // chunks per tap plane (work weights)
+  for (int dz = -Rz; dz <= Rz; ++dz)
     for (int dy = -st.R[1]; dy <= st.R[1]; ++dy) {
-      int4& r = rows[(size_t)(dz + st.R[2]) * ny + (dy + st.R[1])];
+      int4& r = rows[(size_t)(dz + Rz) * ny + (dy + st.R[1])];
       const double y = dy * lv.h[1], z = dz * lv.h[2];
       const double rem = A * A - y * y - z * z;
       int Rx = -1;
@@ -75,24 +94,77 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
         Rx = std::min(st.R[0], (int)std::floor(std::sqrt(rem) / lv.h[0]));
         while (Rx >= 0 && (Rx * lv.h[0]) * (Rx * lv.h[0]) >= rem) --Rx;
       }
-      if (Rx < 0) { r = make_int4(0, 1, 0, 0); continue; }
-      const int clo = (-Rx + g.X0) / 4, chi = (Rx + g.X0) / 4;
-      r = make_int4((int)(ts.size() / 4), clo, chi, 0);
+      if (Rx < 0) { r = make_int4(0, 1, 0, 0); }
+      else {
+        const int clo = (-Rx + g.X0) / 4, chi = (Rx + g.X0) / 4;
+        r = make_int4((int)(ts.size() / 4), clo, chi, 0);
+        wz[dz + Rz] += chi - clo + 1 + 0.5;
+        for (int c = clo; c <= chi; ++c)
+          for (int t = 0; t < 4; ++t) {
+            const int dx = 4 * c - g.X0 + t;
+            ts.push_back(dx >= -Rx && dx <= Rx ? st.at(st.s, dx, dy, dz) : 0.0);
+          }
+      }
+      // virial: half space n > 0 (z, then y, then x), weight 2 (C(n) is even, reading V)
+      if (dz < 0) continue;
+      int4& v = vrows[(size_t)dz * ny + (dy + st.R[1])];
+      const bool whole = dz > 0 || dy > 0, centre = dz == 0 && dy == 0;
+      if (Rx < 0 || !(whole || centre) || (centre && Rx < 1)) { v = make_int4(0, 1, 0, 0); continue; }
+      const int xlo = centre ? 1 : -Rx;
+      const int clo = (xlo + g.X0) / 4, chi = (Rx + g.X0) / 4;
+      v = make_int4((int)(tv.size() / 12), clo, chi, 0);
+      wzv[dz] += chi - clo + 1 + 0.5;
       for (int c = clo; c <= chi; ++c)
-        for (int t = 0; t < 4; ++t) {
-          const int dx = 4 * c - g.X0 + t;
-          const bool in = dx >= -Rx && dx <= Rx;
-          ts.push_back(in ? st.at(st.s, dx, dy, dz) : 0.0);
-          tg.push_back(in ? st.at(st.g, dx, dy, dz) : 0.0);
-        }
+        for (int m = 0; m < 3; ++m)
+          for (int t = 0; t < 4; ++t) {
+            const int dx = 4 * c - g.X0 + t;
+            const double gv = dx >= xlo && dx <= Rx ? 2.0 * st.at(st.g, dx, dy, dz) : 0.0;
+            tv.push_back(m == 0 ? gv : m == 1 ? gv * dx : gv * dx * dx);
+          }
     }
-  d.rows = (int4*)dev_alloc(p, rows.size() * sizeof(int4));
-  if (cudaMemcpy(d.rows, rows.data(), rows.size() * sizeof(int4), cudaMemcpyHostToDevice) != cudaSuccess)
-    throw CudaFail();
-  d.staps = upload(p, ts);
-  d.gtaps = upload(p, tg);
+  auto up_rows = [&](const std::vector<int4>& r) {
+    int4* dptr = (int4*)dev_alloc(p, r.size() * sizeof(int4));
+    if (cudaMemcpy(dptr, r.data(), r.size() * sizeof(int4), cudaMemcpyHostToDevice) != cudaSuccess) throw CudaFail();
+    return dptr;
+  };
+  g.rows = up_rows(rows);
+  g.vrows = up_rows(vrows);
+  g.staps = upload(p, ts);
+  g.vtaps = upload(p, tv);
   d.pad = dev_alloc(p, (size_t)g.P[0] * g.P[1] * g.P[2] * p->esz);
-  d.wpart = (double*)dev_alloc(p, (size_t)d.units * 6 * sizeof(double));
+  g.pad = d.pad;
+  g.Q = d.Q;
+
+  // slices of the input planes, balanced by the taps each plane feeds into the ZT output planes
+  const int nplanes = 2 * Rz + ZT, vplanes = Rz + ZT;
+  std::vector<double> wp(nplanes, 0.0), wv(vplanes, 0.0);
+  for (int pz = 0; pz < nplanes; ++pz)
+    for (int k = 0; k < ZT; ++k) {
+      const int dz = pz - Rz - k;
+      if (dz >= -Rz && dz <= Rz) wp[pz] += wz[dz + Rz];
+      wp[pz] += 0.3;   // staging
+    }
+  for (int pz = 0; pz < vplanes; ++pz)
+    for (int k = 0; k < ZT; ++k) {
+      const int dz = pz - k;
+      if (dz >= 0 && dz <= Rz) wv[pz] += wzv[dz];
+      wv[pz] += 0.3;
+    }
+  const int tiles = g.tiles[0] * g.tiles[1] * g.tiles[2];
+  g.nslices = std::max(1, std::min({p->conv_slices, nplanes, kMaxConvSlices}));
+  g.vslices = std::max(1, std::min({(p->conv_slices + 1) / 2, vplanes, kMaxConvSlices}));
+  balanced_bounds(wp, g.nslices, g.pb);
+  balanced_bounds(wv, g.vslices, g.vb);
+  g.unit0 = p->conv.total_units;
+  g.vunit0 = p->conv.total_vunits;
+  p->conv.total_units += tiles * g.nslices;
+  p->conv.total_vunits += tiles * g.vslices;
+  if (g.nslices > 1) {
+    d.scratch = dev_alloc(p, (size_t)g.nslices * lv.points() * p->esz);
+    g.out = d.scratch;
+  } else {
+    g.out = d.E;
+  }
 }
 
 msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
@@ -124,6 +196,16 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   if (cudaSetDevice(prm->device) != cudaSuccess) return MSM_ERR_CUDA;
 
   // ---- grids
+  // slices per output tile of the convolution: enough one-warp units for ~3 resident waves
+  {
+    const int XTc = p->fp32 ? 16 : 8;
+    long long tiles = 0;
+    for (int l = 1; l < p->n_t; ++l)
+      tiles += (long long)((H.lev[l].M[0] + XTc - 1) / XTc) * ((H.lev[l].M[1] + 31) / 32) * ((H.lev[l].M[2] + 3) / 4);
+    const long long target = 148LL * 16 * 3;
+    p->conv_slices = tiles > 0 ? (int)std::max<long long>(1, std::min<long long>(kMaxConvSlices, (target + tiles - 1) / tiles)) : 1;
+    if (const char* e = std::getenv("MSM_CONV_SLICES")) p->conv_slices = std::max(1, std::atoi(e));
+  }
   size_t tmp_elems = 16;
   const int XT = p->fp32 ? 16 : 8, ZT = 4;
   for (int l = 1; l <= p->n_t; ++l) {
@@ -132,11 +214,22 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
     p->lev[l].E = dev_alloc(p, pts * p->esz);
     tmp_elems = std::max(tmp_elems, pts);
     if (l < p->n_t) {
+      if (l > kMaxConvLevels) return MSM_ERR_UNSUPPORTED;
       build_conv_tables(p, l, XT, ZT);
-      const ConvGeom& g = p->lev[l].cg;
+      const ConvLevel& g = p->conv.lev[l - 1];
       tmp_elems = std::max(tmp_elems, (size_t)g.P[0] * g.P[1] * g.P[2]);
-      if (p->lev[l].smem > 227 * 1024) return MSM_ERR_UNSUPPORTED;
+      if (p->conv_smem > 227 * 1024) return MSM_ERR_UNSUPPORTED;
     }
+  }
+  p->conv.nlev = p->n_t - 1;
+  if (p->conv.nlev > 0) {
+    p->conv_wpart = (double*)dev_alloc(p, (size_t)p->conv.total_vunits * 6 * sizeof(double));
+    for (int l = 1; l < p->n_t; ++l) {
+      ConvLevel& g = p->conv.lev[l - 1];
+      g.wpart = p->conv_wpart + (size_t)g.vunit0 * 6;
+    }
+    p->d_conv = (ConvTable*)dev_alloc(p, sizeof(ConvTable));
+    if (cudaMemcpy(p->d_conv, &p->conv, sizeof(ConvTable), cudaMemcpyHostToDevice) != cudaSuccess) throw CudaFail();
   }
   p->tmpA = dev_alloc(p, tmp_elems * p->esz);
   p->tmpB = dev_alloc(p, tmp_elems * p->esz);
@@ -204,10 +297,7 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
     if (cudaEventCreate(&p->ev[i]) != cudaSuccess) return MSM_ERR_CUDA;
   // stage list of msm_evaluate, in launch order
   for (const char* s : {"sort", "pair", "anterpolate", "restrict"}) p->stage_name_store.push_back(s);
-  for (int l = 1; l < p->n_t; ++l) {
-    p->stage_name_store.push_back("filter_l" + std::to_string(l));
-    p->stage_name_store.push_back("conv_l" + std::to_string(l));
-  }
+  for (const char* s : {"filter", "conv", "conv_virial"}) p->stage_name_store.push_back(s);
   for (const char* s : {"top", "prolongate", "interpolate", "reduce"}) p->stage_name_store.push_back(s);
   for (const std::string& s : p->stage_name_store) p->stage_names.push_back(s.c_str());
   p->n_stages = (int)p->stage_names.size();

@@ -165,7 +165,7 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
   FinalizeArgs fa;
   for (int l = 1; l < p->n_t; ++l) {
     LevelDev& d = p->lev[l];
-    const ConvGeom& g = d.cg;
+    const ConvLevel& g = p->conv.lev[l - 1];
     const Level& lv = H.lev[l];
     // omega' filter + halo, x then y then z
     const T* src = (const T*)d.Q;
@@ -184,25 +184,44 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
       src = dst;
       din[ax] = g.P[ax];
     }
-    mark();
+  }
+  mark();
+  if (p->conv.nlev > 0) {
     constexpr int XT = sizeof(T) == 4 ? 16 : 8, ZT = 4;
-    if (want_virial) {
-      auto kern = k_conv<T, XT, ZT, true>;
-      if (d.smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d.smem);
-      MSM_LAUNCH(p, (kern<<<d.units, 32, d.smem, st>>>(g, d.rows, (const T*)d.staps, (const T*)d.gtaps,
-                                                      (const T*)d.pad, (const T*)d.Q, (T*)d.E, d.wpart)));
-      Seg& s = fa.seg[nseg++];
-      s.ptr = d.wpart; s.count = d.units;
-      const double hx = lv.h[0], hy = lv.h[1], hz = lv.h[2];
-      const double sc[6] = {hx * hx, hy * hy, hz * hz, hx * hy, hx * hz, hy * hz};
-      for (int k = 0; k < 6; ++k) s.scale[k] = -0.5 * sc[k];
-    } else {
-      auto kern = k_conv<T, XT, ZT, false>;
-      if (d.smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d.smem);
-      MSM_LAUNCH(p, (kern<<<d.units, 32, d.smem, st>>>(g, d.rows, (const T*)d.staps, (const T*)d.gtaps,
-                                                      (const T*)d.pad, (const T*)d.Q, (T*)d.E, d.wpart)));
+    {
+      auto kern = k_conv<T, XT, ZT>;
+      if (p->conv_smem > 48 * 1024)
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
+      MSM_LAUNCH(p, (kern<<<p->conv.total_units, 32, p->conv_smem, st>>>(p->d_conv)));
+      for (int l = 1; l < p->n_t; ++l) {
+        const ConvLevel& g = p->conv.lev[l - 1];
+        if (g.nslices > 1) {
+          const size_t pts = H.lev[l].points();
+          MSM_LAUNCH(p, (k_sum_slices<T><<<blocks_for(pts, 256), 256, 0, st>>>(pts, g.nslices, (const T*)p->lev[l].scratch,
+                                                                               (T*)p->lev[l].E)));
+        }
+      }
     }
     mark();
+    if (want_virial) {
+      auto kern = k_conv_virial<T, XT, ZT>;
+      if (p->conv_smem > 48 * 1024)
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
+      MSM_LAUNCH(p, (kern<<<p->conv.total_vunits, 32, p->conv_smem, st>>>(p->d_conv)));
+      for (int l = 1; l < p->n_t; ++l) {
+        const ConvLevel& g = p->conv.lev[l - 1];
+        const Level& lv = H.lev[l];
+        Seg& s = fa.seg[nseg++];
+        s.ptr = g.wpart;
+        s.count = g.tiles[0] * g.tiles[1] * g.tiles[2] * g.vslices;
+        const double hx = lv.h[0], hy = lv.h[1], hz = lv.h[2];
+        const double sc[6] = {hx * hx, hy * hy, hz * hz, hx * hy, hx * hz, hy * hz};
+        for (int k = 0; k < 6; ++k) s.scale[k] = -0.5 * sc[k];
+      }
+    }
+    mark();
+  } else {
+    mark(); mark();
   }
 
   // ---------------- S6 top level

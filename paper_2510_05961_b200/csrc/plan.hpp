@@ -15,13 +15,8 @@ constexpr int kMaxStages = 2 * MSM_MAX_LEVELS + 16;   // sort pair anterpolate r
 
 struct LevelDev {
   void *Q = nullptr, *E = nullptr, *pad = nullptr;   // grid charge, potential, haloed filtered charge
-  ConvGeom cg{};
-  int4* rows = nullptr;
-  void *staps = nullptr, *gtaps = nullptr;
-  int units = 0;
-  double* wpart = nullptr;                           // units x 6
+  void* scratch = nullptr;                           // slice partials of the convolution (nslices > 1)
   int taps = 0;
-  size_t smem = 0;
 };
 
 }  // namespace msm
@@ -42,6 +37,11 @@ struct msm_plan {
 
   msm::LevelDev lev[MSM_MAX_LEVELS + 1];
   void *tmpA = nullptr, *tmpB = nullptr;
+  msm::ConvTable conv{};                             // host copy; conv.lev[l - 1] is level l
+  msm::ConvTable* d_conv = nullptr;
+  size_t conv_smem = 0;
+  int conv_slices = 1;                               // input-plane slices per output tile
+  double* conv_wpart = nullptr;                      // total_vunits x 6
 
   // top operator
   int G = 0;
