@@ -6,6 +6,7 @@
 #include <cstring>
 #include <new>
 
+#include "pair.cuh"
 #include "plan.hpp"
 
 using namespace msm;
@@ -284,7 +285,8 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   p->grec = dev_alloc(p, cap * 4 * p->esz);
   p->Fsr = dev_alloc(p, cap * 3 * p->esz);
   p->Vsr = dev_alloc(p, cap * p->esz);
-  p->pair_wpart = (double*)dev_alloc(p, (size_t)p->pair_rows * 6 * sizeof(double));
+  p->pair_ymax = (int)((cap / 32 + p->pair_rows) / p->pair_rows + 3) / 4 + 1;
+  p->pair_wpart = (double*)dev_alloc(p, (size_t)p->pair_rows * p->pair_ymax * kPairWarps * 6 * sizeof(double));
   p->n_eblocks = (int)((cap + 127) / 128);
   p->epart = (double*)dev_alloc(p, (size_t)p->n_eblocks * sizeof(double));
   p->results = (double*)dev_alloc(p, 8 * sizeof(double));

@@ -117,15 +117,22 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
     }
     (void)any_minimg;
     const double a = p->mp.a;
+    // fp32 scan: exact cutoff in fp32 mode (the drain repeats the same arithmetic); in fp64 mode a
+    // slack of 1e-4 relative covers the rounding of cell-relative coordinates (< 2^-24 * 8 edges)
+    pp.a2_scan = sizeof(T) == 4 ? (float)(a * a) : (float)(a * a * (1.0 + 1e-4));
     pp.a2 = (T)(a * a); pp.inv_a = (T)(1.0 / a); pp.inv_a2 = (T)(1.0 / (a * a)); pp.two_inv_a3 = (T)(2.0 / (a * a * a));
     for (int k = 0; k < 8; ++k) pp.c[k] = (T)p->S->c[k];
     pp.p = P;
-    if (want_virial)
-      MSM_LAUNCH(p, (k_pair<T, P, true><<<p->pair_rows, kPairWarps * 32, 0, st>>>(
-                        pp, p->pstart, (const V4*)p->prec, p->pcellx, p->porder, (T*)p->Fsr, (T*)p->Vsr, p->pair_wpart)));
-    else
-      MSM_LAUNCH(p, (k_pair<T, P, false><<<p->pair_rows, kPairWarps * 32, 0, st>>>(
-                        pp, p->pstart, (const V4*)p->prec, p->pcellx, p->porder, (T*)p->Fsr, (T*)p->Vsr, p->pair_wpart)));
+    // tiles of 32 particles per cell row, spread over gridDim.y blocks of kPairWarps warps
+    const int per_row = (n / 32 + p->pair_rows) / p->pair_rows;
+    const dim3 pgrid(p->pair_rows, std::max(1, std::min(p->pair_ymax, (per_row + kPairWarps - 1) / kPairWarps)));
+    p->pair_blocks = (int)(pgrid.x * pgrid.y);
+    const bool mi = pp.minimg[0] || pp.minimg[1] || pp.minimg[2];
+#define MSM_PAIR(V, M) MSM_LAUNCH(p, (k_pair<T, P, V, M><<<pgrid, kPairWarps * 32, 0, st>>>(           \
+    pp, p->pstart, (const V4*)p->prec, p->pcellx, p->porder, (T*)p->Fsr, (T*)p->Vsr, p->pair_wpart)))
+    if (want_virial) { if (mi) MSM_PAIR(true, true); else MSM_PAIR(true, false); }
+    else { if (mi) MSM_PAIR(false, true); else MSM_PAIR(false, false); }
+#undef MSM_PAIR
   }
   mark();
 
@@ -278,7 +285,7 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
   // ---------------- S9 reductions
   if (want_virial) {
     Seg& s = fa.seg[nseg++];
-    s.ptr = p->pair_wpart; s.count = p->pair_rows;
+    s.ptr = p->pair_wpart; s.count = p->pair_blocks * kPairWarps;
     for (int k = 0; k < 6; ++k) s.scale[k] = 1.0;
   }
   fa.nseg = nseg;

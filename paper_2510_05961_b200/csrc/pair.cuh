@@ -4,9 +4,23 @@
 // Cells have edge >= a/2, so the neighbourhood is 5x5x5 cells. An i-tile is up to 32 consecutive
 // sorted particles of one x-row of cells (lane = particle i); for each of the 25 neighbouring
 // rows the j-particles of cells [cx_first-2, cx_last+2] are contiguous in the sorted order and
-// are staged through shared memory 32 at a time, in a frame relative to the tile's first cell
-// (cell-relative coordinates keep fp32 differences accurate). -k_0'(r)/r = 1/r^3 + (2/a^3) g'(s),
-// s = r^2/a^2 - 1, so one rsqrt per pair inside the cutoff is the only special function.
+// are staged through shared memory kPairBatch at a time, in a frame relative to the tile's first
+// cell (cell-relative coordinates keep fp32 differences accurate).
+//
+// Only 17-27 % of the candidates are inside the cutoff, and a warp that branches per candidate
+// pays the full interaction whenever ANY lane hits. So the candidates of consecutive neighbour
+// rows are gathered into batches and each batch is processed in two phases:
+//   scan  -- every lane tests every candidate (one broadcast 16-byte shared load, 3 subtractions,
+//            3 multiply-adds, one compare, in fp32 on both precisions) and appends the index of
+//            each hit to its private list in shared memory; in fp64 mode the fp32 test uses a
+//            widened cutoff and the exact test is repeated in the drain;
+//   drain -- round r evaluates, on every lane that has one, the r-th hit of its list in full
+//            precision. Rounds = the largest hit count of any lane in the batch, so the expensive
+//            path runs at 60-70 % lane utilisation instead of ~20 %, with ~6 instructions of
+//            bookkeeping per round.
+// Every lane visits its hits in ascending candidate order, so the sums have a fixed order
+// (deterministic). -k_0'(r)/r = 1/r^3 + (2/a^3) g'(s), s = r^2/a^2 - 1: one rsqrt per pair is the
+// only special function.
 #pragma once
 #include "device_common.cuh"
 
@@ -20,44 +34,165 @@ template <typename T> struct PairParams {
   T edge[3];
   T box[3], inv_box[3];
   T a2, inv_a, inv_a2, two_inv_a3;
+  float a2_scan;          // cutoff^2 of the fp32 scan (widened by rounding slack in fp64 mode)
   T c[8];                 // binom(-1/2, k)
   int p;
 };
 
 constexpr int kPairWarps = 4;
 
-template <typename T, int P, bool VIRIAL>
+template <typename T> struct PairStage;       // shared-memory staging of one warp
+template <> struct PairStage<float> {
+  static constexpr int kBatch = 160;          // candidates per batch (multiple of 32)
+  float4 f[kBatch];                           // scan and drain read the same record
+  unsigned char list[kBatch * 32];            // hit r of lane l at [r * 32 + l]
+  __device__ __forceinline__ void put(int k, float4 r) { f[k] = r; }
+  __device__ __forceinline__ float4 full(int k) const { return f[k]; }
+};
+template <> struct PairStage<double> {
+  static constexpr int kBatch = 96;
+  float4 f[kBatch];                           // fp32 copy for the scan
+  double4 d[kBatch];                          // full precision for the drain
+  unsigned char list[kBatch * 32];
+  __device__ __forceinline__ void put(int k, double4 r) {
+    d[k] = r;
+    f[k] = make_float4((float)r.x, (float)r.y, (float)r.z, 0.f);
+  }
+  __device__ __forceinline__ double4 full(int k) const { return d[k]; }
+};
+
+__device__ __forceinline__ float rsqrt_fast(float x) {
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ double rsqrt_fast(double x) { return 1.0 / sqrt(x); }
+
+template <typename T, int P, bool VIRIAL, bool MI>
 __global__ void __launch_bounds__(kPairWarps * 32)
 k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>::type* __restrict__ prec,
        const int* __restrict__ pcellx, const int* __restrict__ porder, T* __restrict__ Fsr,
        T* __restrict__ Vsr, double* __restrict__ wpart) {
   using V4 = typename Vec4<T>::type;
-  __shared__ V4 sj[kPairWarps][32];
-  __shared__ double red[kPairWarps];
+  constexpr int B = PairStage<T>::kBatch;
+  __shared__ PairStage<T> stage[kPairWarps];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  const int row = blockIdx.x;                       // (cy, cz)
+  PairStage<T>& sj = stage[wid];
+  const int row = blockIdx.x;                       // (cy, cz); blockIdx.y strides over the row's tiles
   const int cy = row % prm.nc[1], cz = row / prm.nc[1];
   const int ncx = prm.nc[0];
   const int row_s = pstart[row * ncx], row_e = pstart[(row + 1) * ncx];
   const int ntile = (row_e - row_s + 31) >> 5;
+  const bool mix = MI && prm.minimg[0] != 0, miy = MI && prm.minimg[1] != 0, miz = MI && prm.minimg[2] != 0;
+  // a (sub-)tile may span at most span_max cells so that its +-2 neighbourhood never overlaps itself
+  const int span_max = prm.periodic[0] && !mix ? max(ncx - 5, 0) : (1 << 30);
+  const T a2 = prm.a2, inv_a = prm.inv_a, inv_a2 = prm.inv_a2, two_inv_a3 = prm.two_inv_a3;
+  const float a2_scan = prm.a2_scan;
+  T cf[P], cd[P];                                   // g(s) = sum cf[k] s^k, g'(s) = sum cd[k] s^(k-1)
+#pragma unroll
+  for (int k = 0; k < P; ++k) { cf[k] = prm.c[k]; cd[k] = (T)k * prm.c[k]; }
   double W[6] = {0, 0, 0, 0, 0, 0};
 
-  for (int tile = wid; tile < ntile; tile += kPairWarps) {
+  for (int tile = blockIdx.y * kPairWarps + wid; tile < ntile; tile += kPairWarps * gridDim.y) {
     const int ki = row_s + tile * 32 + lane;
-    const bool iv = ki < row_e;
+    const bool inrow = ki < row_e;
     V4 ri = make_vec4<T>(0, 0, 0, 0);
     int cxi = 0;
-    if (iv) { ri = ldg4(prec + ki); cxi = pcellx[ki]; }
+    if (inrow) { ri = ldg4(prec + ki); cxi = pcellx[ki]; }
     const int last = min(31, row_e - 1 - (row_s + tile * 32));
-    const int cxf = __shfl_sync(0xffffffffu, cxi, 0), cxl = __shfl_sync(0xffffffffu, cxi, last);
+   // sub-tiles: consecutive lanes whose cells span at most span_max (one pass unless the row is sparse)
+   for (int first = 0; first <= last;) {
+    const int cxf = __shfl_sync(0xffffffffu, cxi, first);
+    const unsigned fits = __ballot_sync(0xffffffffu, inrow && lane >= first && cxi - cxf <= span_max);
+    const int sub_last = 31 - __clz((int)fits);            // cells ascend with the lane
+    const bool iv = lane >= first && lane <= sub_last;
+    const int cxl = __shfl_sync(0xffffffffu, cxi, sub_last);
+    first = sub_last + 1;
     const T xi = ri.x + (T)(cxi - cxf) * prm.edge[0], yi = ri.y, zi = ri.z;
+    // fp32 copy for the scan; an idle lane sits far away and never hits
+    const float xs = iv ? (float)xi : 3e30f, ys = (float)yi, zs = (float)zi;
     // x-range of neighbour cells in unwrapped cell coordinates
     int xa = cxf - 2, xb = cxl + 2;
-    bool mix = prm.minimg[0] != 0;
     if (!prm.periodic[0]) { xa = max(xa, 0); xb = min(xb, ncx - 1); }
-    else if (xb - xa + 1 > ncx) { xa = 0; xb = ncx - 1; mix = true; }   // every cell once + min. image
+    else if (mix) { xa = 0; xb = ncx - 1; }                 // fewer than 5 cells: each once + min. image
+    constexpr bool anymi = MI;
     T ax = 0, ay = 0, az = 0, av = 0;
     T w0 = 0, w1 = 0, w2 = 0, w3 = 0, w4 = 0, w5 = 0;
+    int fill = 0;          // candidates staged in the current batch
+    int selfpos = -1;      // stage index of the lane's own particle, if it is in the batch
+
+    // ---- scan + drain of the staged batch
+    auto process = [&]() {
+      const int nw = (fill + 31) >> 5;
+      for (int k = fill + lane; k < nw * 32; k += 32) sj.put(k, make_vec4<T>((T)1e30, 0, 0, 0));   // pads: far away
+      __syncwarp();
+      unsigned char* const lp = sj.list + lane;
+      unsigned char* le = lp;                                 // end of this lane's hit list (stride 32)
+      for (int w = 0; w < nw; ++w) {
+        const float4* fp = sj.f + w * 32;
+        const int ib = w * 32;
+        if (!anymi) {
+#pragma unroll
+          for (int kk = 0; kk < 32; ++kk) {
+            const float4 pj = fp[kk];
+            const float dx = xs - pj.x, dy_ = ys - pj.y, dz_ = zs - pj.z;
+            const float r2 = fmaf(dx, dx, fmaf(dy_, dy_, dz_ * dz_));
+            if (r2 < a2_scan) { *le = (unsigned char)(ib + kk); le += 32; }
+          }
+        } else {
+#pragma unroll 4
+          for (int kk = 0; kk < 32; ++kk) {
+            const float4 pj = fp[kk];
+            float dx = xs - pj.x, dy_ = ys - pj.y, dz_ = zs - pj.z;
+            if (mix) dx -= (float)prm.box[0] * rintf(dx * (float)prm.inv_box[0]);
+            if (miy) dy_ -= (float)prm.box[1] * rintf(dy_ * (float)prm.inv_box[1]);
+            if (miz) dz_ -= (float)prm.box[2] * rintf(dz_ * (float)prm.inv_box[2]);
+            const float r2 = fmaf(dx, dx, fmaf(dy_, dy_, dz_ * dz_));
+            if (r2 < a2_scan) { *le = (unsigned char)(ib + kk); le += 32; }
+          }
+        }
+      }
+      const int n = (int)(le - lp) >> 5;                      // hits of this lane
+      int nmax = n;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) nmax = max(nmax, __shfl_xor_sync(0xffffffffu, nmax, o));
+      for (int r = 0; r < nmax; ++r) {
+        if (r < n) {
+          const int idx = lp[r * 32];
+          if (idx != selfpos) {                               // the particle itself, dropped by index
+            const V4 pj = sj.full(idx);
+            T dx = xi - pj.x, dy_ = yi - pj.y, dz_ = zi - pj.z;
+            if (anymi) {
+              if (mix) dx -= prm.box[0] * rint(dx * prm.inv_box[0]);
+              if (miy) dy_ -= prm.box[1] * rint(dy_ * prm.inv_box[1]);
+              if (miz) dz_ -= prm.box[2] * rint(dz_ * prm.inv_box[2]);
+            }
+            const T r2 = fma(dx, dx, fma(dy_, dy_, dz_ * dz_));
+            if (sizeof(T) == 4 || r2 < a2) {                  // fp32: the scan was already exact
+              const T rinv = rsqrt_fast(r2);
+              const T s = fma(r2, inv_a2, (T)-1);
+              T g = cf[P - 1], dg = cd[P - 1];
+#pragma unroll
+              for (int k = P - 2; k >= 0; --k) g = fma(g, s, cf[k]);
+#pragma unroll
+              for (int k = P - 2; k >= 1; --k) dg = fma(dg, s, cd[k]);
+              const T qj = pj.w;
+              av = fma(qj, fma(-g, inv_a, rinv), av);
+              const T fs = qj * fma(two_inv_a3, dg, rinv * rinv * rinv);
+              ax = fma(fs, dx, ax); ay = fma(fs, dy_, ay); az = fma(fs, dz_, az);
+              if (VIRIAL) {
+                const T fx = fs * dx, fy = fs * dy_, fz = fs * dz_;
+                w0 = fma(fx, dx, w0); w1 = fma(fy, dy_, w1); w2 = fma(fz, dz_, w2);
+                w3 = fma(fx, dy_, w3); w4 = fma(fx, dz_, w4); w5 = fma(fy, dz_, w5);
+              }
+            }
+          }
+        }
+      }
+      __syncwarp();
+      fill = 0;
+      selfpos = -1;
+    };
 
     for (int dz = prm.omin[2]; dz <= prm.omax[2]; ++dz) {
       int czj = cz + dz;
@@ -76,49 +211,27 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
           else if (seg == 1) { ca = max(xa, 0); cb = min(xb, ncx - 1); shift = 0; if (ca > cb) continue; }
           else { if (xb < ncx) continue; ca = max(xa, ncx) - ncx; cb = xb - ncx; shift = ncx; }
           const int js = pstart[rowbase + ca], je = pstart[rowbase + cb + 1];
-          for (int j0 = js; j0 < je; j0 += 32) {
-            const int kj = j0 + lane;
-            V4 rj = make_vec4<T>((T)1e30, 0, 0, 0);
-            if (kj < je) {
-              rj = ldg4(prec + kj);
+          for (int j = js; j < je;) {
+            // stage as many candidates of this segment as fit, in the tile's frame
+            const int take = min(je - j, B - fill);
+            for (int t = lane; t < take; t += 32) {
+              const int kj = j + t;
+              V4 rj = ldg4(prec + kj);
               rj.x += (T)(pcellx[kj] + shift - cxf) * prm.edge[0];
               rj.y += yoff;
               rj.z += zoff;
+              sj.put(fill + t, rj);
             }
-            __syncwarp();
-            sj[wid][lane] = rj;
-            __syncwarp();
-            const int cnt = min(32, je - j0);
-            for (int kk = 0; kk < cnt; ++kk) {
-              const V4 pj = sj[wid][kk];
-              T dx = xi - pj.x, dy_ = yi - pj.y, dz_ = zi - pj.z;
-              if (mix) dx -= prm.box[0] * rint(dx * prm.inv_box[0]);
-              if (prm.minimg[1]) dy_ -= prm.box[1] * rint(dy_ * prm.inv_box[1]);
-              if (prm.minimg[2]) dz_ -= prm.box[2] * rint(dz_ * prm.inv_box[2]);
-              const T r2 = fma(dx, dx, fma(dy_, dy_, dz_ * dz_));
-              if (r2 < prm.a2 && (j0 + kk) != ki && iv) {
-                const T rinv = rsqrt_t<T>(r2);
-                const T s = fma(r2, prm.inv_a2, (T)-1);
-                T g = prm.c[P - 1], dg = (T)(P - 1) * prm.c[P - 1];
-#pragma unroll
-                for (int k = P - 2; k >= 0; --k) g = fma(g, s, prm.c[k]);
-#pragma unroll
-                for (int k = P - 2; k >= 1; --k) dg = fma(dg, s, (T)k * prm.c[k]);
-                const T qj = pj.w;
-                av = fma(qj, rinv - g * prm.inv_a, av);
-                const T fs = qj * fma(prm.two_inv_a3, dg, rinv * rinv * rinv);
-                ax = fma(fs, dx, ax); ay = fma(fs, dy_, ay); az = fma(fs, dz_, az);
-                if (VIRIAL) {
-                  const T fx = fs * dx, fy = fs * dy_, fz = fs * dz_;
-                  w0 = fma(fx, dx, w0); w1 = fma(fy, dy_, w1); w2 = fma(fz, dz_, w2);
-                  w3 = fma(fx, dy_, w3); w4 = fma(fx, dz_, w4); w5 = fma(fy, dz_, w5);
-                }
-              }
-            }
+            if (ki >= j && ki < j + take) selfpos = fill + (ki - j);
+            fill += take;
+            j += take;
+            if (fill == B) process();
           }
         }
       }
     }
+    if (fill > 0) process();
+
     if (iv) {
       const int orig = porder[ki];
       const T qi = ri.w;
@@ -132,12 +245,15 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
         W[3] += hq * (double)w3; W[4] += hq * (double)w4; W[5] += hq * (double)w5;
       }
     }
+   }
   }
-  if (VIRIAL) {
+  if (VIRIAL) {   // one partial per warp, fixed shuffle order; no block barrier (warps finish at different times)
 #pragma unroll
     for (int k = 0; k < 6; ++k) {
-      const double r = block_reduce_sum<kPairWarps * 32>(W[k], red);
-      if (threadIdx.x == 0) wpart[(size_t)blockIdx.x * 6 + k] = r;
+      double v = W[k];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+      if (lane == 0) wpart[(((size_t)blockIdx.y * gridDim.x + blockIdx.x) * kPairWarps + wid) * 6 + k] = v;
     }
   }
 }

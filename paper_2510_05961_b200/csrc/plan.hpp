@@ -51,7 +51,7 @@ struct msm_plan {
   // particles
   int cap = 0;
   msm::BinGeom bg{};
-  int n_pcells = 0, n_gcells = 0, pair_rows = 0;
+  int n_pcells = 0, n_gcells = 0, pair_rows = 0, pair_ymax = 1, pair_blocks = 0;
   int* ibuf = nullptr;          // [phist(n_pcells+1) | ghist(n_gcells+1) | pfill | gfill | flag]
   size_t ibuf_count = 0;
   int *phist = nullptr, *ghist = nullptr, *pfill = nullptr, *gfill = nullptr, *flag = nullptr;
