@@ -27,22 +27,46 @@ __device__ __forceinline__ size_t lin(const int d[3], int x, int y, int z) {
   return ((size_t)z * d[1] + y) * d[0] + x;
 }
 
+// coordinates of output element t and the element stride of the working axis in the input array
+struct AxisPos {
+  int c[3];
+  size_t base;     // offset of the input line's element 0 (working-axis coordinate 0)
+  size_t stride;   // input stride along the working axis
+};
+__device__ __forceinline__ AxisPos axis_pos(const AxisDims& d, size_t t) {
+  AxisPos p;
+  p.c[0] = (int)(t % d.out[0]);
+  const size_t r = t / d.out[0];
+  p.c[1] = (int)(r % d.out[1]);
+  p.c[2] = (int)(r / d.out[1]);
+  int z[3] = {p.c[0], p.c[1], p.c[2]};
+  z[d.axis] = 0;
+  p.base = lin(d.in, z[0], z[1], z[2]);
+  p.stride = d.axis == 0 ? 1 : (d.axis == 1 ? (size_t)d.in[0] : (size_t)d.in[0] * d.in[1]);
+  return p;
+}
+
 // out[o] = sum_k w[k] in_logical[o - H - k]: omega' filter that also lays down the halo.
 // Logical input index i: periodic -> in[i mod M]; open -> in[i] inside [0, M), else 0.
+// One thread per output; the wrapped index is carried along the taps (one modulo per thread).
 template <typename T>
 __global__ void k_pad_filter(AxisDims d, int H, AxisTaps<T> w, const T* __restrict__ in, T* __restrict__ out) {
   const size_t total = (size_t)d.out[0] * d.out[1] * d.out[2];
   const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= total) return;
-  int c[3] = {(int)(t % d.out[0]), (int)((t / d.out[0]) % d.out[1]), (int)(t / ((size_t)d.out[0] * d.out[1]))};
-  const int g = c[d.axis] - H, M = d.in[d.axis], hw = w.n / 2;
+  const AxisPos p = axis_pos(d, t);
+  const int g = p.c[d.axis] - H, M = d.in[d.axis], hw = w.n / 2;
+  const T* line = in + p.base;
   T acc = 0;
-  for (int k = -hw; k <= hw; ++k) {
-    int i = g - k;
-    if (d.periodic) i = imod(i, M);
-    else if (i < 0 || i >= M) continue;
-    c[d.axis] = i;
-    acc = fma(w.c[k + hw], in[lin(d.in, c[0], c[1], c[2])], acc);
+  if (d.periodic) {
+    int i = imod(g + hw, M);                       // tap k = -hw reads logical index g + hw
+    for (int k = 0; k < w.n; ++k) {
+      acc = fma(w.c[k], line[(size_t)i * p.stride], acc);
+      if (--i < 0) i += M;
+    }
+  } else {
+    const int klo = max(0, g + hw - (M - 1)), khi = min(w.n - 1, g + hw);   // 0 <= g + hw - k < M
+    for (int k = klo; k <= khi; ++k) acc = fma(w.c[k], line[(size_t)(g + hw - k) * p.stride], acc);
   }
   out[t] = acc;
 }
@@ -54,16 +78,21 @@ __global__ void k_restrict_axis(AxisDims d, int lo_in, int lo_out, AxisTaps<T> J
   const size_t total = (size_t)d.out[0] * d.out[1] * d.out[2];
   const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= total) return;
-  int c[3] = {(int)(t % d.out[0]), (int)((t / d.out[0]) % d.out[1]), (int)(t / ((size_t)d.out[0] * d.out[1]))};
-  const int m = c[d.axis], M = d.in[d.axis], hw = J.n / 2;
-  if (d.periodic && M == 1) { out[t] = in[lin(d.in, c[0], c[1], c[2])]; return; }
+  const AxisPos p = axis_pos(d, t);
+  const int m = p.c[d.axis], M = d.in[d.axis], hw = J.n / 2;
+  const T* line = in + p.base;
+  if (d.periodic && M == 1) { out[t] = line[0]; return; }
   T acc = 0;
-  for (int n = -hw; n <= hw; ++n) {
-    int i = 2 * (m + lo_out) + n - lo_in;
-    if (d.periodic) i = imod(i, M);
-    else if (i < 0 || i >= M) continue;
-    c[d.axis] = i;
-    acc = fma(J.c[n + hw], in[lin(d.in, c[0], c[1], c[2])], acc);
+  const int i0 = 2 * (m + lo_out) - hw - lo_in;    // tap n = -hw
+  if (d.periodic) {
+    int i = imod(i0, M);
+    for (int k = 0; k < J.n; ++k) {
+      acc = fma(J.c[k], line[(size_t)i * p.stride], acc);
+      if (++i >= M) i -= M;
+    }
+  } else {
+    const int klo = max(0, -i0), khi = min(J.n - 1, M - 1 - i0);
+    for (int k = klo; k <= khi; ++k) acc = fma(J.c[k], line[(size_t)(i0 + k) * p.stride], acc);
   }
   out[t] = acc;
 }
@@ -75,26 +104,28 @@ __global__ void k_prolong_axis(AxisDims d, int lo_in, int lo_out, AxisTaps<T> J,
   const size_t total = (size_t)d.out[0] * d.out[1] * d.out[2];
   const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= total) return;
-  int c[3] = {(int)(t % d.out[0]), (int)((t / d.out[0]) % d.out[1]), (int)(t / ((size_t)d.out[0] * d.out[1]))};
-  const int i = c[d.axis], Mi = d.in[d.axis], Mo = d.out[d.axis], hw = J.n / 2;
+  const AxisPos p = axis_pos(d, t);
+  const int i = p.c[d.axis], Mi = d.in[d.axis], Mo = d.out[d.axis], hw = J.n / 2;
+  const T* line = in + p.base;
   T acc = 0;
   if (d.periodic && Mo == 1) {
-    acc = in[lin(d.in, c[0], c[1], c[2])];
+    acc = line[0];
+  } else if (d.periodic) {
+    // taps n with (i - n) even: n = n0, n0 + 2, ...; m = ((i - n) mod Mo) / 2 descends by one per tap
+    const int n0 = -hw + ((i + hw) & 1);
+    int m = imod(i - n0, Mo) >> 1;                 // Mo = 2 Mi
+    for (int n = n0; n <= hw; n += 2) {
+      acc = fma(J.c[n + hw], line[(size_t)m * p.stride], acc);
+      if (--m < 0) m += Mi;
+    }
   } else {
-    for (int n = -hw; n <= hw; ++n) {
-      int m;
-      if (d.periodic) {
-        const int v = imod(i - n, Mo);
-        if (v & 1) continue;
-        m = v >> 1;
-      } else {
-        const int v = i + lo_out - n;
-        if (v & 1) continue;
-        m = v / 2 - lo_in;            // v even (possibly negative): exact
-        if (m < 0 || m >= Mi) continue;
-      }
-      c[d.axis] = m;
-      acc = fma(J.c[n + hw], in[lin(d.in, c[0], c[1], c[2])], acc);
+    const int v0 = i + lo_out;                     // 2 (m + lo_in) = v0 - n
+    const int n0 = -hw + ((v0 + hw) & 1);
+    for (int n = n0; n <= hw; n += 2) {
+      const int v = v0 - n;                        // even (possibly negative): exact halving
+      const int m = v / 2 - lo_in;
+      if (m < 0 || m >= Mi) continue;
+      acc = fma(J.c[n + hw], line[(size_t)m * p.stride], acc);
     }
   }
   if (ADD) out[t] += acc; else out[t] = acc;

@@ -257,6 +257,17 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
     bg.h1[ax] = H.lev[1].h[ax];
     bg.ng[ax] = mp.periodic[ax] ? H.lev[1].M[ax] : (int)std::floor(prm->box[ax] / prm->h) + 1;
   }
+  // tiled anterpolation when each tile grid fits once into every periodic axis
+  {
+    p->at.D = kAT + prm->p - 1;
+    p->anterp_tiled = true;
+    for (int ax = 0; ax < 3; ++ax) {
+      p->at.nt[ax] = (bg.ng[ax] + kAT - 1) / kAT;
+      if (mp.periodic[ax] && H.lev[1].M[ax] < p->at.D) p->anterp_tiled = false;
+    }
+    if (p->anterp_tiled)
+      p->anterp_scratch = dev_alloc(p, (size_t)p->at.nt[0] * p->at.nt[1] * p->at.nt[2] * p->at.D * p->at.D * p->at.D * p->esz);
+  }
   const long long npc = (long long)bg.nc[0] * bg.nc[1] * bg.nc[2];
   const long long ngc = (long long)bg.ng[0] * bg.ng[1] * bg.ng[2];
   if (npc > (1ll << 28) || ngc > (1ll << 28)) return MSM_ERR_UNSUPPORTED;

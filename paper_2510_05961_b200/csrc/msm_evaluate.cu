@@ -143,8 +143,18 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
     gg.periodic[ax] = p->bg.periodic[ax];
   }
   const SplineTab<T, P> tab = make_tab<T, P>(*p->pieces);
-  MSM_LAUNCH(p, (k_anterpolate<T, P><<<blocks_for(H.lev[1].points(), 128), 128, 0, st>>>(
-                    gg, tab, p->gstart, (const V4*)p->grec, (T*)p->lev[1].Q)));
+  if (p->anterp_tiled) {
+    const int D3 = p->at.D * p->at.D * p->at.D;
+    const size_t sm = (size_t)(D3 + P * P) * sizeof(T);
+    const int ntiles = p->at.nt[0] * p->at.nt[1] * p->at.nt[2];
+    MSM_LAUNCH(p, (k_anterp_tiles<T, P><<<ntiles, 32, sm, st>>>(gg, p->at, tab, p->gstart, (const V4*)p->grec,
+                                                                 p->gcell_sorted, (T*)p->anterp_scratch)));
+    MSM_LAUNCH(p, (k_anterp_combine<T, P><<<blocks_for(H.lev[1].points(), 128), 128, 0, st>>>(
+                      gg, p->at, (const T*)p->anterp_scratch, (T*)p->lev[1].Q)));
+  } else {
+    MSM_LAUNCH(p, (k_anterpolate<T, P><<<blocks_for(H.lev[1].points(), 128), 128, 0, st>>>(
+                      gg, tab, p->gstart, (const V4*)p->grec, (T*)p->lev[1].Q)));
+  }
   mark();
 
   // ---------------- S4 restriction

@@ -6,6 +6,7 @@
 #include <vector>
 
 #include "../../include/msm.h"
+#include "anterp_tiled.cuh"
 #include "conv.cuh"
 #include "plan_math.hpp"
 
@@ -42,6 +43,11 @@ struct msm_plan {
   size_t conv_smem = 0;
   int conv_slices = 1;                               // input-plane slices per output tile
   double* conv_wpart = nullptr;                      // total_vunits x 6
+
+  // tiled anterpolation (anterp_tiled.cuh); false: gather kernel
+  bool anterp_tiled = false;
+  msm::AnterpTiles at{};
+  void* anterp_scratch = nullptr;
 
   // top operator
   int G = 0;
