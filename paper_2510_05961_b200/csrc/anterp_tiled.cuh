@@ -1,26 +1,25 @@
 // anterp_tiled.cuh -- S3 anterpolation (Eq. 9; Alg. 1) with warp-private shared-
 // memory grids reduced in a fixed order: scatter-free in global memory, no atomics, deterministic.
 //
-// A tile is a box of AT^3 level-1 grid cells owned by ONE warp. The warp walks the tile's particles
+// A tile is a box of T[0] x T[1] x T[2] level-1 grid cells owned by ONE warp. The warp walks the tile's particles
 // in the canonical sorted order (cell by cell, ascending original index inside a cell) and adds
-// each particle's p^3 contributions q_i phi_m(r_i) to its private (AT+p-1)^3 node grid in shared
+// each particle's p^3 contributions q_i phi_m(r_i) to its private (T+p-1)^3 node grid in shared
 // memory: lane t handles nodes t, t+32, ... of the p^3 block, so one particle's targets are all
 // distinct, and particles are processed one after the other, so every node sees its additions in a
 // fixed order. The 3p one-dimensional weights are evaluated once per particle (lane k < 3p
 // evaluates weight k) and handed round by shuffles. The tile grids go to a scratch array; a second
-// kernel sums, for every node, the (at most 27, typically 1-8) tiles that cover it in a fixed
-// order. Used when every periodic axis has at least AT + p - 1 nodes (each node then appears at
+// kernel sums, for every node, the (at most 8) tiles that cover it in a fixed order. Used when
+// every periodic axis has at least T + p - 1 nodes (each node then appears at
 // most once in a tile's grid); smaller grids use the gather kernel of particle_grid.cuh.
 #pragma once
 #include "particle_grid.cuh"
 
 namespace msm {
 
-constexpr int kAT = 8;   // tile edge in grid cells
-
 struct AnterpTiles {
+  int T[3];        // tile edge in grid cells per axis (each >= p - 1)
   int nt[3];       // tiles per axis
-  int D;           // AT + p - 1: tile grid edge in nodes
+  int D[3];        // T + p - 1: tile grid edge in nodes
 };
 
 template <typename T, int P>
@@ -31,14 +30,14 @@ k_anterp_tiles(GridGeom g, AnterpTiles at, SplineTab<T, P> tab, const int* __res
   using V4 = typename Vec4<T>::type;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* tg = reinterpret_cast<T*>(smem_raw);          // D^3 node grid
-  T* coef = tg + at.D * at.D * at.D;               // P x P spline piece coefficients
+  const int D3 = at.D[0] * at.D[1] * at.D[2], Dx = at.D[0], Dy = at.D[1];
+  T* coef = tg + D3;                               // P x P spline piece coefficients
   constexpr int NT = (P * P * P + 31) / 32;        // nodes per lane
   const int lane = threadIdx.x;
-  const int D = at.D, D3 = D * D * D;
   int tl = blockIdx.x;
   const int tx = tl % at.nt[0]; tl /= at.nt[0];
   const int ty = tl % at.nt[1], tz = tl / at.nt[1];
-  const int C0[3] = {tx * kAT, ty * kAT, tz * kAT};
+  const int C0[3] = {tx * at.T[0], ty * at.T[1], tz * at.T[2]};
   for (int i = lane; i < D3; i += 32) tg[i] = 0;
   for (int i = lane; i < P * P; i += 32) coef[i] = tab.c[i / P][i % P];
   // static node offsets of this lane inside a particle's p^3 block, and the lanes that hold its weights
@@ -47,24 +46,24 @@ k_anterp_tiles(GridGeom g, AnterpTiles at, SplineTab<T, P> tab, const int* __res
   for (int s = 0; s < NT; ++s) {
     const int t = min(lane + 32 * s, P * P * P - 1);
     const int jx = t % P, jy = (t / P) % P, jz = t / (P * P);
-    noff[s] = (jz * D + jy) * D + jx;
+    noff[s] = (jz * Dy + jy) * Dx + jx;
     lx[s] = jx; ly[s] = P + jy; lz[s] = 2 * P + jz;
   }
   __syncwarp();
-  const int czn = min(kAT, g.ng[2] - C0[2]), cyn = min(kAT, g.ng[1] - C0[1]), cxn = min(kAT, g.ng[0] - C0[0]);
+  const int czn = min(at.T[2], g.ng[2] - C0[2]), cyn = min(at.T[1], g.ng[1] - C0[1]),
+            cxn = min(at.T[0], g.ng[0] - C0[0]);
   for (int cz = 0; cz < czn; ++cz)
     for (int cy = 0; cy < cyn; ++cy) {
       const int rowbase = ((C0[2] + cz) * g.ng[1] + (C0[1] + cy)) * g.ng[0];
       const int ks = gstart[rowbase + C0[0]], ke = gstart[rowbase + C0[0] + cxn];
-      const int rowoff = (cz * D + cy) * D - C0[0];
+      const int rowoff = (cz * Dy + cy) * Dx - C0[0];
       for (int k0 = ks; k0 < ke; k0 += 32) {
         // coalesced load of up to 32 particles, then one after the other through shuffles
         V4 r = make_vec4<T>(0, 0, 0, 0);
         int cx = 0;
         if (k0 + lane < ke) { r = ldg4(grec + k0 + lane); cx = gcell_sorted[k0 + lane] - rowbase; }
         const int cnt = min(32, ke - k0);
-        // weight (axis a = lane / P, node offset j = lane % P) of MY particle's coordinate... is per
-        // particle, so it is evaluated inside the loop from the broadcast fractions
+        // per particle: lane k < 3P evaluates weight (axis k / P, node offset k % P)
         for (int i = 0; i < cnt; ++i) {
           const T fx = __shfl_sync(0xffffffffu, r.x, i), fy = __shfl_sync(0xffffffffu, r.y, i);
           const T fz = __shfl_sync(0xffffffffu, r.z, i), q = __shfl_sync(0xffffffffu, r.w, i);
@@ -97,7 +96,7 @@ k_anterp_tiles(GridGeom g, AnterpTiles at, SplineTab<T, P> tab, const int* __res
   for (int i = lane; i < D3; i += 32) out[i] = tg[i];
 }
 
-// Q[m] = sum over the tiles whose grid covers node m, tiles in ascending (z, y, x) visiting order
+// Q[m] = sum over the tiles whose grid covers node m (at most two per axis), in a fixed order
 template <typename T, int P>
 __global__ void __launch_bounds__(128)
 k_anterp_combine(GridGeom g, AnterpTiles at, const T* __restrict__ scratch, T* __restrict__ Q) {
@@ -106,38 +105,35 @@ k_anterp_combine(GridGeom g, AnterpTiles at, const T* __restrict__ scratch, T* _
   const int m = blockIdx.x * blockDim.x + threadIdx.x;
   if (m >= total) return;
   const int mi[3] = {m % g.M[0], (m / g.M[0]) % g.M[1], m / (g.M[0] * g.M[1])};
-  const int D = at.D;
-  // per axis: up to 3 (tile, local node index) candidates
-  int tix[3][3], lix[3][3], cnt[3];
+  int tix[3][2], lix[3][2], cnt[3];
 #pragma unroll
   for (int ax = 0; ax < 3; ++ax) {
-    const int n = mi[ax] + g.lo[ax];                 // node index
-    cnt[ax] = 0;
-    int prev = -1;
-#pragma unroll 1
-    for (int i = 0; i < P; ++i) {                    // cells n - HP .. n + HP - 1 touch node n
-      int c = n - HP + i;
-      if (g.periodic[ax]) c = imod(c, g.ng[ax]);
-      else if (c < 0 || c >= g.ng[ax]) continue;
-      const int t = c / kAT;
-      if (t == prev) continue;
-      prev = t;
-      // local index of node n in tile t's grid, whose first node is kAT * t - HP + 1
-      int ln = n - (kAT * t - HP + 1);
-      if (g.periodic[ax]) ln = imod(ln, g.M[ax]);
-      if (cnt[ax] < 3 && ln >= 0 && ln < D) {
-        bool dup = false;
-        for (int k = 0; k < cnt[ax]; ++k) dup |= tix[ax][k] == t;
-        if (!dup) { tix[ax][cnt[ax]] = t; lix[ax][cnt[ax]] = ln; ++cnt[ax]; }
-      }
+    const int n = mi[ax] + g.lo[ax];                 // node index; cells n - HP .. n + HP - 1 touch it
+    int c0 = n - HP, c1 = n + HP - 1;
+    if (g.periodic[ax]) {                            // -HP <= c0, c1 < M + HP and M >= D > P
+      if (c0 < 0) c0 += g.ng[ax];
+      if (c1 >= g.ng[ax]) c1 -= g.ng[ax];
+    } else {
+      c0 = max(c0, 0); c1 = min(c1, g.ng[ax] - 1);
     }
+    const int t0 = c0 / at.T[ax], t1 = c1 / at.T[ax];
+    // local index of node n in tile t's grid, whose first node is T * t - HP + 1
+    int l0 = n - (at.T[ax] * t0 - HP + 1), l1 = n - (at.T[ax] * t1 - HP + 1);
+    if (g.periodic[ax]) {
+      if (l0 < 0) l0 += g.M[ax]; else if (l0 >= g.M[ax]) l0 -= g.M[ax];
+      if (l1 < 0) l1 += g.M[ax]; else if (l1 >= g.M[ax]) l1 -= g.M[ax];
+    }
+    tix[ax][0] = t0; lix[ax][0] = l0;
+    tix[ax][1] = t1; lix[ax][1] = l1;
+    cnt[ax] = t1 != t0 ? 2 : 1;
   }
+  const size_t D3 = (size_t)at.D[0] * at.D[1] * at.D[2];
   T acc = 0;
   for (int a = 0; a < cnt[2]; ++a)
     for (int b = 0; b < cnt[1]; ++b)
       for (int c = 0; c < cnt[0]; ++c) {
         const size_t tile = ((size_t)tix[2][a] * at.nt[1] + tix[1][b]) * at.nt[0] + tix[0][c];
-        acc += scratch[tile * D * D * D + ((size_t)lix[2][a] * D + lix[1][b]) * D + lix[0][c]];
+        acc += scratch[tile * D3 + ((size_t)lix[2][a] * at.D[1] + lix[1][b]) * at.D[0] + lix[0][c]];
       }
   Q[m] = acc;
 }

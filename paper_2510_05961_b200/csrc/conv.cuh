@@ -126,7 +126,7 @@ __device__ __forceinline__ ConvUnit decode_unit(const ConvTable& tab, int u) {
 
 // ---------------------------------------------------------------------------------- potential
 template <typename T, int XT, int ZT>
-__global__ void __launch_bounds__(32)
+__global__ void __launch_bounds__(32, sizeof(T) == 4 ? 16 : 12)
 k_conv(const ConvTable* __restrict__ tabp) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* plane = reinterpret_cast<T*>(smem_raw);
@@ -172,15 +172,22 @@ k_conv(const ConvTable* __restrict__ tabp) {
           SmemVec<T>::load4(srow + 4 * c + j, t);
           win[j] = t[0]; win[j + 1] = t[1]; win[j + 2] = t[2]; win[j + 3] = t[3];
         }
+        // all tap quads of this chunk are requested before the first FMA (loads of inactive rows
+        // read the table's first quad and are not used)
+        T tp[ZT][4];
+        bool on[ZT];
 #pragma unroll
         for (int k = 0; k < ZT; ++k) {
-          if (c >= re[k].y && c <= re[k].z) {
-            T tp[4];
-            SmemVec<T>::ldg(staps + (re[k].x + c - re[k].y) * 4, tp);
+          on[k] = c >= re[k].y && c <= re[k].z;
+          SmemVec<T>::ldg(staps + (on[k] ? (re[k].x + c - re[k].y) * 4 : 0), tp[k]);
+        }
+#pragma unroll
+        for (int k = 0; k < ZT; ++k) {
+          if (on[k]) {
 #pragma unroll
             for (int t = 0; t < 4; ++t)
 #pragma unroll
-              for (int i = 0; i < XT; ++i) acc[k][i] = fma(tp[t], win[i + t], acc[k][i]);
+              for (int i = 0; i < XT; ++i) acc[k][i] = fma(tp[k][t], win[i + t], acc[k][i]);
           }
         }
       }

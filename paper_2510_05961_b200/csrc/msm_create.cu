@@ -257,16 +257,23 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
     bg.h1[ax] = H.lev[1].h[ax];
     bg.ng[ax] = mp.periodic[ax] ? H.lev[1].M[ax] : (int)std::floor(prm->box[ax] / prm->h) + 1;
   }
-  // tiled anterpolation when each tile grid fits once into every periodic axis
+  // tiled anterpolation when each tile grid fits once into every periodic axis and there are enough
+  // tiles (one warp each) to fill the GPU; otherwise the gather kernel
   {
-    p->at.D = kAT + prm->p - 1;
+    const int tdim[3] = {8, 4, 4};
     p->anterp_tiled = true;
+    long long ntiles = 1;
     for (int ax = 0; ax < 3; ++ax) {
-      p->at.nt[ax] = (bg.ng[ax] + kAT - 1) / kAT;
-      if (mp.periodic[ax] && H.lev[1].M[ax] < p->at.D) p->anterp_tiled = false;
+      p->at.T[ax] = prm->p - 1 <= tdim[ax] ? tdim[ax] : 8;   // power of two >= p - 1: divides periodic M, <= 2 tiles per node and axis
+      p->at.D[ax] = p->at.T[ax] + prm->p - 1;
+      p->at.nt[ax] = (bg.ng[ax] + p->at.T[ax] - 1) / p->at.T[ax];
+      ntiles *= p->at.nt[ax];
+      if (mp.periodic[ax] && H.lev[1].M[ax] < p->at.D[ax]) p->anterp_tiled = false;
     }
+    if (ntiles < 1024) p->anterp_tiled = false;
+    if (const char* e = std::getenv("MSM_ANTERP_TILED")) p->anterp_tiled = p->anterp_tiled && std::atoi(e) != 0;
     if (p->anterp_tiled)
-      p->anterp_scratch = dev_alloc(p, (size_t)p->at.nt[0] * p->at.nt[1] * p->at.nt[2] * p->at.D * p->at.D * p->at.D * p->esz);
+      p->anterp_scratch = dev_alloc(p, (size_t)ntiles * p->at.D[0] * p->at.D[1] * p->at.D[2] * p->esz);
   }
   const long long npc = (long long)bg.nc[0] * bg.nc[1] * bg.nc[2];
   const long long ngc = (long long)bg.ng[0] * bg.ng[1] * bg.ng[2];
@@ -300,6 +307,11 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   p->pair_wpart = (double*)dev_alloc(p, (size_t)p->pair_rows * p->pair_ymax * kPairWarps * 6 * sizeof(double));
   p->n_eblocks = (int)((cap + 127) / 128);
   p->epart = (double*)dev_alloc(p, (size_t)p->n_eblocks * sizeof(double));
+  {
+    const size_t rows = (size_t)p->pair_rows * p->pair_ymax * kPairWarps + p->conv.total_vunits + p->G + p->n_eblocks;
+    p->part_blocks = (int)(rows / 1024 + MSM_MAX_LEVELS + 8);
+    p->part = (double*)dev_alloc(p, (size_t)p->part_blocks * 7 * sizeof(double));
+  }
   p->results = (double*)dev_alloc(p, 8 * sizeof(double));
   p->in_pos = dev_alloc(p, cap * 3 * p->esz);
   p->in_q = dev_alloc(p, cap * p->esz);

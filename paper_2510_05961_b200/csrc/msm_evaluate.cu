@@ -14,35 +14,60 @@ namespace {
 
 struct Seg {
   const double* ptr;
-  int count;      // rows of 6 (or of 1 for the energy)
+  int count;      // rows of 6 doubles (width 6) or single doubles (width 1: energy partials)
+  int width;
+  int blk0;       // first block of this segment in k_partial_sums
   double scale[6];
 };
 constexpr int kMaxSegs = MSM_MAX_LEVELS + 4;
+constexpr int kRowsPerBlock = 1024;
 struct FinalizeArgs {
-  int nseg;
+  int nseg, nblk;
   Seg seg[kMaxSegs];
-  const double* epart;
-  int ne;
 };
 
-// S9: U = sum of the block partials; W = sum over segments of scale_k * partial_k. One block,
-// fixed order -> deterministic.
-__global__ void __launch_bounds__(256) k_finalize(FinalizeArgs a, const int* __restrict__ flag,
-                                                  double* __restrict__ results) {
+// S9, stage 1: every block sums kRowsPerBlock rows of one segment (thread t takes rows t, t+256,
+// ... then a fixed-order block reduction) into part[block][0..5] (scaled virial) / part[block][6]
+// (energy). Stage 2 (k_finalize, one block) adds the block partials in block order. Both orders are
+// fixed -> deterministic.
+__global__ void __launch_bounds__(256) k_partial_sums(FinalizeArgs a, double* __restrict__ part) {
   __shared__ double red[8];
-  double e = 0.0;
-  for (int i = threadIdx.x; i < a.ne; i += 256) e += a.epart[i];
-  e = block_reduce_sum<256>(e, red);
-  if (threadIdx.x == 0) results[0] = e;
+  int s = 0;
+  for (int k = 1; k < a.nseg; ++k)
+    if ((int)blockIdx.x >= a.seg[k].blk0) s = k;
+  const Seg& sg = a.seg[s];
+  const int r0 = ((int)blockIdx.x - sg.blk0) * kRowsPerBlock, r1 = min(r0 + kRowsPerBlock, sg.count);
+  double v[6] = {0, 0, 0, 0, 0, 0};
+  if (sg.width == 6) {
+    for (int i = r0 + threadIdx.x; i < r1; i += 256)
+#pragma unroll
+      for (int k = 0; k < 6; ++k) v[k] += sg.ptr[(size_t)i * 6 + k];
+  } else {
+    for (int i = r0 + threadIdx.x; i < r1; i += 256) v[0] += sg.ptr[i];
+  }
+#pragma unroll
   for (int k = 0; k < 6; ++k) {
-    double w = 0.0;
-    for (int s = 0; s < a.nseg; ++s) {
-      double t = 0.0;
-      for (int i = threadIdx.x; i < a.seg[s].count; i += 256) t += a.seg[s].ptr[(size_t)i * 6 + k];
-      w += a.seg[s].scale[k] * t;
+    const double r = block_reduce_sum<256>(v[k], red);
+    if (threadIdx.x == 0) {
+      if (sg.width == 6) part[(size_t)blockIdx.x * 7 + k] = sg.scale[k] * r;
+      else if (k == 0) part[(size_t)blockIdx.x * 7 + 6] = r;
     }
+  }
+  if (threadIdx.x == 0) {
+    if (sg.width == 6) part[(size_t)blockIdx.x * 7 + 6] = 0.0;
+    else
+      for (int k = 0; k < 6; ++k) part[(size_t)blockIdx.x * 7 + k] = 0.0;
+  }
+}
+
+__global__ void __launch_bounds__(256) k_finalize(int nblk, const double* __restrict__ part,
+                                                  const int* __restrict__ flag, double* __restrict__ results) {
+  __shared__ double red[8];
+  for (int k = 0; k < 7; ++k) {
+    double w = 0.0;
+    for (int i = threadIdx.x; i < nblk; i += 256) w += part[(size_t)i * 7 + k];
     w = block_reduce_sum<256>(w, red);
-    if (threadIdx.x == 0) results[1 + k] = w;
+    if (threadIdx.x == 0) results[k == 6 ? 0 : 1 + k] = w;
   }
   if (threadIdx.x == 0) results[7] = (double)(*flag);
 }
@@ -144,7 +169,7 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
   }
   const SplineTab<T, P> tab = make_tab<T, P>(*p->pieces);
   if (p->anterp_tiled) {
-    const int D3 = p->at.D * p->at.D * p->at.D;
+    const int D3 = p->at.D[0] * p->at.D[1] * p->at.D[2];
     const size_t sm = (size_t)(D3 + P * P) * sizeof(T);
     const int ntiles = p->at.nt[0] * p->at.nt[1] * p->at.nt[2];
     MSM_LAUNCH(p, (k_anterp_tiles<T, P><<<ntiles, 32, sm, st>>>(gg, p->at, tab, p->gstart, (const V4*)p->grec,
@@ -229,7 +254,7 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
         const ConvLevel& g = p->conv.lev[l - 1];
         const Level& lv = H.lev[l];
         Seg& s = fa.seg[nseg++];
-        s.ptr = g.wpart;
+        s.ptr = g.wpart; s.width = 6;
         s.count = g.tiles[0] * g.tiles[1] * g.tiles[2] * g.vslices;
         const double hx = lv.h[0], hy = lv.h[1], hz = lv.h[2];
         const double sc[6] = {hx * hx, hy * hy, hz * hz, hx * hy, hx * hz, hy * hz};
@@ -249,7 +274,7 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
       MSM_LAUNCH(p, (k_top_dense<T, true><<<nb, 128, 0, st>>>(p->G, (const T*)p->topT, (const T*)p->topTD,
                                                              (const T*)d.Q, (T*)d.E, p->top_wrow)));
       Seg& s = fa.seg[nseg++];
-      s.ptr = p->top_wrow; s.count = p->G;
+      s.ptr = p->top_wrow; s.count = p->G; s.width = 6;
       for (int k = 0; k < 6; ++k) s.scale[k] = 1.0;
     } else {
       MSM_LAUNCH(p, (k_top_dense<T, false><<<nb, 128, 0, st>>>(p->G, (const T*)p->topT, (const T*)p->topTD,
@@ -295,12 +320,24 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
   // ---------------- S9 reductions
   if (want_virial) {
     Seg& s = fa.seg[nseg++];
-    s.ptr = p->pair_wpart; s.count = p->pair_blocks * kPairWarps;
+    s.ptr = p->pair_wpart; s.count = p->pair_blocks * kPairWarps; s.width = 6;
     for (int k = 0; k < 6; ++k) s.scale[k] = 1.0;
   }
+  {
+    Seg& s = fa.seg[nseg++];
+    s.ptr = p->epart; s.count = neb; s.width = 1;
+    for (int k = 0; k < 6; ++k) s.scale[k] = 0.0;
+  }
   fa.nseg = nseg;
-  fa.epart = p->epart; fa.ne = neb;
-  MSM_LAUNCH(p, (k_finalize<<<1, 256, 0, st>>>(fa, p->flag, p->results)));
+  int nblk = 0;
+  for (int k = 0; k < nseg; ++k) {
+    fa.seg[k].blk0 = nblk;
+    nblk += (fa.seg[k].count + kRowsPerBlock - 1) / kRowsPerBlock;
+  }
+  fa.nblk = nblk;
+  if (nblk > p->part_blocks) return MSM_ERR_CUDA;   // sized at plan creation; cannot happen
+  if (nblk > 0) MSM_LAUNCH(p, (k_partial_sums<<<nblk, 256, 0, st>>>(fa, p->part)));
+  MSM_LAUNCH(p, (k_finalize<<<1, 256, 0, st>>>(nblk, p->part, p->flag, p->results)));
   mark();
   cudaMemcpyAsync(p->h_results, p->results, 8 * sizeof(double), cudaMemcpyDeviceToHost, st);
   if (cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }

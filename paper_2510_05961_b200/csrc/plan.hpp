@@ -67,6 +67,8 @@ struct msm_plan {
   void *prec = nullptr, *grec = nullptr, *Fsr = nullptr, *Vsr = nullptr;
   double *pair_wpart = nullptr, *epart = nullptr, *results = nullptr;
   int n_eblocks = 0;
+  double* part = nullptr;       // block partials of the final reductions, part_blocks x 7
+  int part_blocks = 0;
   double* h_results = nullptr;  // pinned: U, W[6], flag
   // staging for msm_evaluate_host
   void *in_pos = nullptr, *in_q = nullptr, *out_F = nullptr, *out_V = nullptr;
