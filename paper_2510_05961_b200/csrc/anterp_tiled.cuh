@@ -16,6 +16,8 @@
 
 namespace msm {
 
+constexpr int kMaxAnterpRows = 64;   // T[1] * T[2]
+
 struct AnterpTiles {
   int T[3];        // tile edge in grid cells per axis (each >= p - 1)
   int nt[3];       // tiles per axis
@@ -52,46 +54,71 @@ k_anterp_tiles(GridGeom g, AnterpTiles at, SplineTab<T, P> tab, const int* __res
   __syncwarp();
   const int czn = min(at.T[2], g.ng[2] - C0[2]), cyn = min(at.T[1], g.ng[1] - C0[1]),
             cxn = min(at.T[0], g.ng[0] - C0[0]);
-  for (int cz = 0; cz < czn; ++cz)
-    for (int cy = 0; cy < cyn; ++cy) {
+  // the tile's particles are one contiguous run per (cz, cy) row of cells: fetch all row bounds at
+  // once and walk the concatenation of the runs (row-major, so the canonical order is kept)
+  const int nrows = czn * cyn;
+  int* rks = reinterpret_cast<int*>(coef + P * P);   // first particle of row r
+  int* roff = rks + kMaxAnterpRows;                  // particles before row r; roff[nrows] = total
+  for (int r = lane; r < nrows; r += 32) {
+    const int cz = r / cyn, cy = r - cz * cyn;
+    const int rowbase = ((C0[2] + cz) * g.ng[1] + (C0[1] + cy)) * g.ng[0];
+    const int ks = gstart[rowbase + C0[0]], ke = gstart[rowbase + C0[0] + cxn];
+    rks[r] = ks;
+    roff[r + 1] = ke - ks;
+  }
+  __syncwarp();
+  if (lane == 0) {
+    roff[0] = 0;
+    for (int r = 0; r < nrows; ++r) roff[r + 1] += roff[r];
+  }
+  __syncwarp();
+  const int total = roff[nrows];
+  for (int k0 = 0; k0 < total; k0 += 32) {
+    // coalesced (per row) load of up to 32 particles, then one after the other through shuffles
+    V4 r = make_vec4<T>(0, 0, 0, 0);
+    int mybase = 0;
+    const int flat = k0 + lane;
+    if (flat < total) {
+      int lo = 0, hi = nrows - 1;                     // last row with roff[row] <= flat
+      while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (roff[mid] <= flat) lo = mid; else hi = mid - 1;
+      }
+      const int cz = lo / cyn, cy = lo - cz * cyn;
       const int rowbase = ((C0[2] + cz) * g.ng[1] + (C0[1] + cy)) * g.ng[0];
-      const int ks = gstart[rowbase + C0[0]], ke = gstart[rowbase + C0[0] + cxn];
-      const int rowoff = (cz * Dy + cy) * Dx - C0[0];
-      for (int k0 = ks; k0 < ke; k0 += 32) {
-        // coalesced load of up to 32 particles, then one after the other through shuffles
-        V4 r = make_vec4<T>(0, 0, 0, 0);
-        int cx = 0;
-        if (k0 + lane < ke) { r = ldg4(grec + k0 + lane); cx = gcell_sorted[k0 + lane] - rowbase; }
-        const int cnt = min(32, ke - k0);
-        // per particle: lane k < 3P evaluates weight (axis k / P, node offset k % P)
-        for (int i = 0; i < cnt; ++i) {
-          const T fx = __shfl_sync(0xffffffffu, r.x, i), fy = __shfl_sync(0xffffffffu, r.y, i);
-          const T fz = __shfl_sync(0xffffffffu, r.z, i), q = __shfl_sync(0xffffffffu, r.w, i);
-          const int base = rowoff + __shfl_sync(0xffffffffu, cx, i);
-          const int a = lane / P, j = lane - a * P;
-          const T f = a == 0 ? fx : (a == 1 ? fy : fz);
-          T w = 0;
-          if (lane < 3 * P) {
-            const T* c = coef + j * P;
-            w = c[P - 1];
+      const int k = rks[lo] + (flat - roff[lo]);
+      r = ldg4(grec + k);
+      mybase = (cz * Dy + cy) * Dx - C0[0] + (gcell_sorted[k] - rowbase);
+    }
+    const int cnt = min(32, total - k0);
+    // per particle: lane k < 3P evaluates weight (axis k / P, node offset k % P)
+    for (int i = 0; i < cnt; ++i) {
+      const T fx = __shfl_sync(0xffffffffu, r.x, i), fy = __shfl_sync(0xffffffffu, r.y, i);
+      const T fz = __shfl_sync(0xffffffffu, r.z, i), q = __shfl_sync(0xffffffffu, r.w, i);
+      const int base = __shfl_sync(0xffffffffu, mybase, i);
+      const int a = lane / P, j = lane - a * P;
+      const T f = a == 0 ? fx : (a == 1 ? fy : fz);
+      T w = 0;
+      if (lane < 3 * P) {
+        const T* c = coef + j * P;
+        w = c[P - 1];
 #pragma unroll
-            for (int k = P - 2; k >= 0; --k) w = fma(w, f, c[k]);
-            if (a == 2) w *= q;
-          }
+        for (int k = P - 2; k >= 0; --k) w = fma(w, f, c[k]);
+        if (a == 2) w *= q;
+      }
 #pragma unroll
-          for (int s = 0; s < NT; ++s) {
-            const T wx = __shfl_sync(0xffffffffu, w, lx[s]);
-            const T wy = __shfl_sync(0xffffffffu, w, ly[s]);
-            const T wz = __shfl_sync(0xffffffffu, w, lz[s]);
-            if (lane + 32 * s < P * P * P) {
-              T* dst = tg + base + noff[s];
-              *dst = fma(wz * wy, wx, *dst);
-            }
-          }
-          __syncwarp();
+      for (int s = 0; s < NT; ++s) {
+        const T wx = __shfl_sync(0xffffffffu, w, lx[s]);
+        const T wy = __shfl_sync(0xffffffffu, w, ly[s]);
+        const T wz = __shfl_sync(0xffffffffu, w, lz[s]);
+        if (lane + 32 * s < P * P * P) {
+          T* dst = tg + base + noff[s];
+          *dst = fma(wz * wy, wx, *dst);
         }
       }
+      __syncwarp();
     }
+  }
   T* out = scratch + (size_t)blockIdx.x * D3;
   for (int i = lane; i < D3; i += 32) out[i] = tg[i];
 }

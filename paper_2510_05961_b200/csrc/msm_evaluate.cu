@@ -170,7 +170,7 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
   const SplineTab<T, P> tab = make_tab<T, P>(*p->pieces);
   if (p->anterp_tiled) {
     const int D3 = p->at.D[0] * p->at.D[1] * p->at.D[2];
-    const size_t sm = (size_t)(D3 + P * P) * sizeof(T);
+    const size_t sm = (size_t)(D3 + P * P) * sizeof(T) + (2 * kMaxAnterpRows + 2) * sizeof(int);
     const int ntiles = p->at.nt[0] * p->at.nt[1] * p->at.nt[2];
     MSM_LAUNCH(p, (k_anterp_tiles<T, P><<<ntiles, 32, sm, st>>>(gg, p->at, tab, p->gstart, (const V4*)p->grec,
                                                                  p->gcell_sorted, (T*)p->anterp_scratch)));
