@@ -57,7 +57,12 @@ class ClockSampler:
     def __init__(self, index: int):
         self.rows, self.proc, self.index = [], None, index
 
+    def mark(self):
+        time.sleep(0.25)              # let nvidia-smi deliver at least one sample under load
+        self.first = len(self.rows)
+
     def start(self):
+        self.first = 0
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
                                           "--format=csv,noheader,nounits", "-lms", "100"],
@@ -80,7 +85,7 @@ class ClockSampler:
         except Exception:
             self.proc.kill()
         sm, mx, reasons = [], [], set()
-        for r in self.rows:
+        for r in self.rows[min(self.first, max(len(self.rows) - 1, 0)):]:
             try:
                 sm.append(float(r[0])); mx.append(float(r[1]))
             except Exception:
@@ -144,6 +149,21 @@ def stage_work(stage: str, w, plan, esz: int, pairs: float):
     return "byte", n * esz * 2.0                              # reduce
 
 
+def max_over_ranks(ms_total: float, ms_e2e: float, world: int, dev):
+    """Device-timed step sums of this rank -> the maximum over all ranks (MAX all-reduce)."""
+    import torch
+    t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device=dev)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t[0]), float(t[1])
+
+
+def whole_job_value(world: int, particles: int, steps: int, ms_total: float) -> float:
+    """Replicas: every rank evaluated `particles` particles `steps` times in `ms_total` (max over ranks)."""
+    return world * particles * steps / (ms_total * 1e-3)
+
+
 def run_ours(args, rank: int, world: int):
     import numpy as np
     import torch
@@ -161,7 +181,6 @@ def run_ours(args, rank: int, world: int):
     esz = 4 if prec == "fp32" else 8
     plan = msm.Plan.for_workload(w, prec, device=local)
     dt = plan.torch_dtype
-    npdt = np.float32 if prec == "fp32" else np.float64
     pos = torch.tensor(w.positions, dtype=dt, device=dev).contiguous()
     q = torch.tensor(w.charges, dtype=dt, device=dev).contiguous()
     F = torch.zeros((w.n, 3), dtype=dt, device=dev)
@@ -176,11 +195,13 @@ def run_ours(args, rank: int, world: int):
 
     # ---- device-resident arm (value)
     plan.set_profiling(True)          # one cudaEventRecord between stages: per-stage times, live
-    for _ in range(args.warmup):
-        plan.evaluate(pos, q, F, V)
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+    for _ in range(args.warmup):
+        plan.evaluate(pos, q, F, V)
+    if rank == 0:
+        sampler.mark()                # only samples taken from here on (the timed region) count
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     stage_sum, launches, energy = {}, 0, 0.0
     barrier()
@@ -215,11 +236,7 @@ def run_ours(args, rank: int, world: int):
     barrier()
     ms_e2e = sum(a.elapsed_time(b) for a, b in ev2)
 
-    t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device=dev)
-    if world > 1:
-        import torch.distributed as dist
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total, ms_e2e = float(t[0]), float(t[1])
+    ms_total, ms_e2e = max_over_ranks(ms_total, ms_e2e, world, dev)
     if rank != 0:
         return None
 
@@ -249,7 +266,7 @@ def run_ours(args, rank: int, world: int):
                 if d["bound"] == "alu" else f"{peak_src} MEASURED_PEAKS.json hbm_gbs",
                 "measured_fma_tflops": round(fma_meas, 2), "share_of_step": round(d["ms"] / (ms_total / args.steps), 4)}
     out = {
-        "metric": METRIC, "value": world * w.n * args.steps / (ms_total * 1e-3), "unit": UNIT,
+        "metric": METRIC, "value": whole_job_value(world, w.n, args.steps, ms_total), "unit": UNIT,
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
         "config": {"workload": args.workload, "particles": w.n, "box": list(w.box), "periodic": list(w.periodic),
@@ -257,7 +274,7 @@ def run_ours(args, rank: int, world: int):
                    "grids": [list(plan.info.grid_dims[i]) for i in range(plan.info.n_tiled)],
                    "outputs": "energy+forces+potentials+virial", "parallelism": "replicas" if world > 1 else "1gpu",
                    "l2": "256 MiB fill between steps (outside the per-step event pairs)"},
-        "e2e": {"value": world * w.n * args.steps / (ms_e2e * 1e-3), "unit": UNIT,
+        "e2e": {"value": whole_job_value(world, w.n, args.steps, ms_e2e), "unit": UNIT,
                 "h2d_bytes_per_step": w.n * 4 * esz, "d2h_bytes_per_step": w.n * 4 * esz + 64,
                 "ms_per_step": ms_e2e / args.steps},
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "stages": stages,
