@@ -6,8 +6,11 @@
 // each particle's p^3 contributions q_i phi_m(r_i) to its private (T+p-1)^3 node grid in shared
 // memory: lane t handles nodes t, t+32, ... of the p^3 block, so one particle's targets are all
 // distinct, and particles are processed one after the other, so every node sees its additions in a
-// fixed order. The 3p one-dimensional weights are evaluated once per particle (lane k < 3p
-// evaluates weight k) and handed round by shuffles. The tile grids go to a scratch array; a second
+// fixed order. When p divides 32 every lane's nodes keep the same (jx, jy) and a fixed set of jz, so
+// the lane holds the spline pieces of its own rows in registers and evaluates its weights itself
+// (no shuffles: the shared-memory/shuffle pipe is the bottleneck of this kernel); otherwise the 3p
+// one-dimensional weights are evaluated once per particle (lane k < 3p evaluates weight k) and
+// handed round by shuffles. The batch of particle records is broadcast from shared memory. The tile grids go to a scratch array; a second
 // kernel sums, for every node, the (at most 8) tiles that cover it in a fixed order. Used when
 // every periodic axis has at least T + p - 1 nodes (each node then appears at
 // most once in a tile's grid); smaller grids use the gather kernel of particle_grid.cuh.
@@ -23,6 +26,13 @@ struct AnterpTiles {
   int nt[3];       // tiles per axis
   int D[3];        // T + p - 1: tile grid edge in nodes
 };
+
+// dynamic shared memory of k_anterp_tiles: node grid, spline pieces (padded so that the int arrays
+// and the 32-byte records that follow stay aligned), row tables, batch staging
+template <typename T, int P> inline size_t anterp_smem_bytes(int D3) {
+  const size_t grid_elems = ((size_t)D3 + P * P + 7) / 8 * 8;
+  return grid_elems * sizeof(T) + (2 * kMaxAnterpRows + 2 + 32 + 6) * sizeof(int) + 32 * 4 * sizeof(T);
+}
 
 template <typename T, int P>
 __global__ void __launch_bounds__(32)
@@ -51,14 +61,29 @@ k_anterp_tiles(GridGeom g, AnterpTiles at, SplineTab<T, P> tab, const int* __res
     noff[s] = (jz * Dy + jy) * Dx + jx;
     lx[s] = jx; ly[s] = P + jy; lz[s] = 2 * P + jz;
   }
+  constexpr bool kRegRows = (32 % P) == 0;
+  T cxr[P], cyr[P], czr[kRegRows ? NT : 1][P];       // spline pieces of this lane's rows
+  if (kRegRows) {
+    const int jx = lane % P, jy = (lane / P) % P;
+#pragma unroll
+    for (int k = 0; k < P; ++k) { cxr[k] = tab.c[jx][k]; cyr[k] = tab.c[jy][k]; }
+#pragma unroll
+    for (int s2 = 0; s2 < NT; ++s2) {
+      const int jz = min((lane + 32 * s2) / (P * P), P - 1);
+#pragma unroll
+      for (int k = 0; k < P; ++k) czr[s2][k] = tab.c[jz][k];
+    }
+  }
   __syncwarp();
   const int czn = min(at.T[2], g.ng[2] - C0[2]), cyn = min(at.T[1], g.ng[1] - C0[1]),
             cxn = min(at.T[0], g.ng[0] - C0[0]);
   // the tile's particles are one contiguous run per (cz, cy) row of cells: fetch all row bounds at
   // once and walk the concatenation of the runs (row-major, so the canonical order is kept)
   const int nrows = czn * cyn;
-  int* rks = reinterpret_cast<int*>(coef + P * P);   // first particle of row r
+  int* rks = reinterpret_cast<int*>(tg + (D3 + P * P + 7) / 8 * 8);   // first particle of row r
   int* roff = rks + kMaxAnterpRows;                  // particles before row r; roff[nrows] = total
+  int* sbase = roff + kMaxAnterpRows + 2;            // node offset of each particle of the batch
+  V4* srec = reinterpret_cast<V4*>(sbase + 32 + 6);  // the batch's records (offset is a multiple of 32 B)
   for (int r = lane; r < nrows; r += 32) {
     const int cz = r / cyn, cy = r - cz * cyn;
     const int rowbase = ((C0[2] + cz) * g.ng[1] + (C0[1] + cy)) * g.ng[0];
@@ -91,29 +116,48 @@ k_anterp_tiles(GridGeom g, AnterpTiles at, SplineTab<T, P> tab, const int* __res
       mybase = (cz * Dy + cy) * Dx - C0[0] + (gcell_sorted[k] - rowbase);
     }
     const int cnt = min(32, total - k0);
-    // per particle: lane k < 3P evaluates weight (axis k / P, node offset k % P)
+    srec[lane] = r;
+    sbase[lane] = mybase;
+    __syncwarp();
     for (int i = 0; i < cnt; ++i) {
-      const T fx = __shfl_sync(0xffffffffu, r.x, i), fy = __shfl_sync(0xffffffffu, r.y, i);
-      const T fz = __shfl_sync(0xffffffffu, r.z, i), q = __shfl_sync(0xffffffffu, r.w, i);
-      const int base = __shfl_sync(0xffffffffu, mybase, i);
-      const int a = lane / P, j = lane - a * P;
-      const T f = a == 0 ? fx : (a == 1 ? fy : fz);
-      T w = 0;
-      if (lane < 3 * P) {
-        const T* c = coef + j * P;
-        w = c[P - 1];
+      const V4 pr = srec[i];                          // broadcast
+      const int base = sbase[i];
+      if (kRegRows) {
+        T wx = cxr[P - 1], wy = cyr[P - 1];
 #pragma unroll
-        for (int k = P - 2; k >= 0; --k) w = fma(w, f, c[k]);
-        if (a == 2) w *= q;
-      }
+        for (int k = P - 2; k >= 0; --k) { wx = fma(wx, pr.x, cxr[k]); wy = fma(wy, pr.y, cyr[k]); }
+        const T wxy = wx * wy * pr.w;
 #pragma unroll
-      for (int s = 0; s < NT; ++s) {
-        const T wx = __shfl_sync(0xffffffffu, w, lx[s]);
-        const T wy = __shfl_sync(0xffffffffu, w, ly[s]);
-        const T wz = __shfl_sync(0xffffffffu, w, lz[s]);
-        if (lane + 32 * s < P * P * P) {
-          T* dst = tg + base + noff[s];
-          *dst = fma(wz * wy, wx, *dst);
+        for (int s2 = 0; s2 < NT; ++s2) {
+          T wz = czr[s2][P - 1];
+#pragma unroll
+          for (int k = P - 2; k >= 0; --k) wz = fma(wz, pr.z, czr[s2][k]);
+          if (lane + 32 * s2 < P * P * P) {
+            T* dst = tg + base + noff[s2];
+            *dst = fma(wz, wxy, *dst);
+          }
+        }
+      } else {
+        // lane k < 3P evaluates weight (axis k / P, node offset k % P)
+        const int a = lane / P, j = lane - a * P;
+        const T f = a == 0 ? pr.x : (a == 1 ? pr.y : pr.z);
+        T w = 0;
+        if (lane < 3 * P) {
+          const T* c = coef + j * P;
+          w = c[P - 1];
+#pragma unroll
+          for (int k = P - 2; k >= 0; --k) w = fma(w, f, c[k]);
+          if (a == 2) w *= pr.w;
+        }
+#pragma unroll
+        for (int s2 = 0; s2 < NT; ++s2) {
+          const T wx = __shfl_sync(0xffffffffu, w, lx[s2]);
+          const T wy = __shfl_sync(0xffffffffu, w, ly[s2]);
+          const T wz = __shfl_sync(0xffffffffu, w, lz[s2]);
+          if (lane + 32 * s2 < P * P * P) {
+            T* dst = tg + base + noff[s2];
+            *dst = fma(wz * wy, wx, *dst);
+          }
         }
       }
       __syncwarp();

@@ -222,7 +222,7 @@ __global__ void k_sum_slices(size_t n, int nslices, const T* __restrict__ part, 
 
 // ------------------------------------------------------------------------------------- virial
 template <typename T, int XT, int ZT>
-__global__ void __launch_bounds__(32)
+__global__ void __launch_bounds__(32, sizeof(T) == 4 ? 16 : 9)
 k_conv_virial(const ConvTable* __restrict__ tabp) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* plane = reinterpret_cast<T*>(smem_raw);

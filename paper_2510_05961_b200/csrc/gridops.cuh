@@ -27,18 +27,33 @@ __device__ __forceinline__ size_t lin(const int d[3], int x, int y, int z) {
   return ((size_t)z * d[1] + y) * d[0] + x;
 }
 
-// coordinates of output element t and the element stride of the working axis in the input array
+// Launch shape of the separable kernels: one thread per output element, consecutive threads along
+// x (coalesced across rows); arrays hold fewer than 2^31 elements, so the index maths is 32-bit.
+constexpr int kAxisThreads = 256;
+inline unsigned axis_grid(const AxisDims& d) {
+  const size_t total = (size_t)d.out[0] * d.out[1] * d.out[2];
+  return (unsigned)((total + kAxisThreads - 1) / kAxisThreads);
+}
+inline unsigned axis_block() { return kAxisThreads; }
+
+// coordinates of this thread's output element, its linear index, and the working-axis stride
 struct AxisPos {
   int c[3];
+  bool valid;
+  size_t t;        // linear index in the output array
   size_t base;     // offset of the input line's element 0 (working-axis coordinate 0)
   size_t stride;   // input stride along the working axis
 };
-__device__ __forceinline__ AxisPos axis_pos(const AxisDims& d, size_t t) {
+__device__ __forceinline__ AxisPos axis_pos(const AxisDims& d) {
   AxisPos p;
-  p.c[0] = (int)(t % d.out[0]);
-  const size_t r = t / d.out[0];
-  p.c[1] = (int)(r % d.out[1]);
-  p.c[2] = (int)(r / d.out[1]);
+  const unsigned t = blockIdx.x * kAxisThreads + threadIdx.x;
+  const unsigned total = (unsigned)d.out[0] * (unsigned)d.out[1] * (unsigned)d.out[2];
+  p.valid = t < total;
+  p.t = t;
+  const unsigned r = t / (unsigned)d.out[0];
+  p.c[0] = (int)(t - r * (unsigned)d.out[0]);
+  p.c[2] = (int)(r / (unsigned)d.out[1]);
+  p.c[1] = (int)(r - (unsigned)p.c[2] * (unsigned)d.out[1]);
   int z[3] = {p.c[0], p.c[1], p.c[2]};
   z[d.axis] = 0;
   p.base = lin(d.in, z[0], z[1], z[2]);
@@ -51,10 +66,9 @@ __device__ __forceinline__ AxisPos axis_pos(const AxisDims& d, size_t t) {
 // One thread per output; the wrapped index is carried along the taps (one modulo per thread).
 template <typename T>
 __global__ void k_pad_filter(AxisDims d, int H, AxisTaps<T> w, const T* __restrict__ in, T* __restrict__ out) {
-  const size_t total = (size_t)d.out[0] * d.out[1] * d.out[2];
-  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= total) return;
-  const AxisPos p = axis_pos(d, t);
+  const AxisPos p = axis_pos(d);
+  if (!p.valid) return;
+  const size_t t = p.t;
   const int g = p.c[d.axis] - H, M = d.in[d.axis], hw = w.n / 2;
   const T* line = in + p.base;
   T acc = 0;
@@ -75,10 +89,9 @@ __global__ void k_pad_filter(AxisDims d, int H, AxisTaps<T> w, const T* __restri
 template <typename T>
 __global__ void k_restrict_axis(AxisDims d, int lo_in, int lo_out, AxisTaps<T> J, const T* __restrict__ in,
                                 T* __restrict__ out) {
-  const size_t total = (size_t)d.out[0] * d.out[1] * d.out[2];
-  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= total) return;
-  const AxisPos p = axis_pos(d, t);
+  const AxisPos p = axis_pos(d);
+  if (!p.valid) return;
+  const size_t t = p.t;
   const int m = p.c[d.axis], M = d.in[d.axis], hw = J.n / 2;
   const T* line = in + p.base;
   if (d.periodic && M == 1) { out[t] = line[0]; return; }
@@ -101,10 +114,9 @@ __global__ void k_restrict_axis(AxisDims d, int lo_in, int lo_out, AxisTaps<T> J
 template <typename T, bool ADD>
 __global__ void k_prolong_axis(AxisDims d, int lo_in, int lo_out, AxisTaps<T> J, const T* __restrict__ in,
                                T* __restrict__ out) {
-  const size_t total = (size_t)d.out[0] * d.out[1] * d.out[2];
-  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= total) return;
-  const AxisPos p = axis_pos(d, t);
+  const AxisPos p = axis_pos(d);
+  if (!p.valid) return;
+  const size_t t = p.t;
   const int i = p.c[d.axis], Mi = d.in[d.axis], Mo = d.out[d.axis], hw = J.n / 2;
   const T* line = in + p.base;
   T acc = 0;

@@ -282,17 +282,17 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   p->pair_rows = bg.nc[1] * bg.nc[2];
   p->cap = prm->max_particles;
   const size_t cap = (size_t)p->cap;
-  p->ibuf_count = (size_t)2 * p->n_pcells + 2 * p->n_gcells + 8;
+  p->ibuf_count = (size_t)p->n_pcells + p->n_gcells + 8;
   p->ibuf = (int*)dev_alloc(p, p->ibuf_count * sizeof(int));
   p->phist = p->ibuf;
   p->ghist = p->phist + p->n_pcells;
-  p->pfill = p->ghist + p->n_gcells;
-  p->gfill = p->pfill + p->n_pcells;
-  p->flag = p->gfill + p->n_gcells;
+  p->flag = p->ghist + p->n_gcells;
   p->pstart = (int*)dev_alloc(p, ((size_t)p->n_pcells + 1) * sizeof(int));
   p->gstart = (int*)dev_alloc(p, ((size_t)p->n_gcells + 1) * sizeof(int));
   p->ptotals = (int*)dev_alloc(p, ((size_t)p->n_pcells / 4096 + 2) * sizeof(int));
   p->gtotals = (int*)dev_alloc(p, ((size_t)p->n_gcells / 4096 + 2) * sizeof(int));
+  p->pslot = (int*)dev_alloc(p, cap * sizeof(int));
+  p->gslot = (int*)dev_alloc(p, cap * sizeof(int));
   p->pcell = (int*)dev_alloc(p, cap * sizeof(int));
   p->gcell = (int*)dev_alloc(p, cap * sizeof(int));
   p->porder = (int*)dev_alloc(p, cap * sizeof(int));

@@ -105,7 +105,7 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
   // ---------------- S1 sort
   cudaMemsetAsync(p->ibuf, 0, p->ibuf_count * sizeof(int), st);
   MSM_LAUNCH(p, (k_bin<T><<<blocks_for(n, 256), 256, 0, st>>>(n, pos, p->bg, p->pcell, p->gcell, p->phist,
-                                                               p->ghist, p->flag)));
+                                                               p->ghist, p->pslot, p->gslot, p->flag)));
   {
     const int tp = (p->n_pcells + kScanTile - 1) / kScanTile, tg = (p->n_gcells + kScanTile - 1) / kScanTile;
     MSM_LAUNCH(p, (k_scan_tiles<<<tp, kScanThreads, 0, st>>>(p->n_pcells, p->phist, p->pstart, p->ptotals)));
@@ -116,7 +116,7 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
     MSM_LAUNCH(p, (k_scan_add<<<blocks_for(p->n_gcells, 256), 256, 0, st>>>(p->n_gcells, p->gstart, p->gtotals, n)));
   }
   MSM_LAUNCH(p, (k_scatter<<<blocks_for(n, 256), 256, 0, st>>>(n, p->pcell, p->gcell, p->pstart, p->gstart,
-                                                                 p->pfill, p->gfill, p->porder, p->gorder)));
+                                                                 p->pslot, p->gslot, p->porder, p->gorder)));
   MSM_LAUNCH(p, (k_sort_cells<<<blocks_for(p->n_pcells, 128), 128, 0, st>>>(p->n_pcells, p->pstart, p->porder)));
   MSM_LAUNCH(p, (k_sort_cells<<<blocks_for(p->n_gcells, 128), 128, 0, st>>>(p->n_gcells, p->gstart, p->gorder)));
   MSM_LAUNCH(p, (k_build_records<T><<<blocks_for(n, 256), 256, 0, st>>>(
@@ -170,7 +170,7 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
   const SplineTab<T, P> tab = make_tab<T, P>(*p->pieces);
   if (p->anterp_tiled) {
     const int D3 = p->at.D[0] * p->at.D[1] * p->at.D[2];
-    const size_t sm = (size_t)(D3 + P * P) * sizeof(T) + (2 * kMaxAnterpRows + 2) * sizeof(int);
+    const size_t sm = anterp_smem_bytes<T, P>(D3);
     const int ntiles = p->at.nt[0] * p->at.nt[1] * p->at.nt[2];
     MSM_LAUNCH(p, (k_anterp_tiles<T, P><<<ntiles, 32, sm, st>>>(gg, p->at, tab, p->gstart, (const V4*)p->grec,
                                                                  p->gcell_sorted, (T*)p->anterp_scratch)));
@@ -194,8 +194,7 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
       d.out[ax] = c.M[ax];
       d.axis = ax; d.periodic = p->bg.periodic[ax];
       T* dst = ax == 2 ? (T*)p->lev[l + 1].Q : (T*)(ax == 0 ? p->tmpA : p->tmpB);
-      const size_t tot = (size_t)d.out[0] * d.out[1] * d.out[2];
-      MSM_LAUNCH(p, (k_restrict_axis<T><<<blocks_for(tot, 256), 256, 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
+      MSM_LAUNCH(p, (k_restrict_axis<T><<<axis_grid(d), axis_block(), 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
       src = dst;
       din[ax] = c.M[ax];
     }
@@ -219,10 +218,9 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
       ad.out[ax] = g.P[ax];
       ad.axis = ax; ad.periodic = p->bg.periodic[ax];
       T* dst = ax == 2 ? (T*)d.pad : (T*)(ax == 0 ? p->tmpA : p->tmpB);
-      const size_t tot = (size_t)ad.out[0] * ad.out[1] * ad.out[2];
       // along the filtered axis the logical size is the grid's, not the (already padded) array's
       ad.in[ax] = lv.M[ax];
-      MSM_LAUNCH(p, (k_pad_filter<T><<<blocks_for(tot, 256), 256, 0, st>>>(ad, halo[ax], Wt, src, dst)));
+      MSM_LAUNCH(p, (k_pad_filter<T><<<axis_grid(ad), axis_block(), 0, st>>>(ad, halo[ax], Wt, src, dst)));
       src = dst;
       din[ax] = g.P[ax];
     }
@@ -295,13 +293,12 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
       for (int k = 0; k < 3; ++k) { d.in[k] = din[k]; d.out[k] = din[k]; }
       d.out[ax] = f.M[ax];
       d.axis = ax; d.periodic = p->bg.periodic[ax];
-      const size_t tot = (size_t)d.out[0] * d.out[1] * d.out[2];
       if (s3 < 2) {
         T* dst = (T*)(s3 == 0 ? p->tmpA : p->tmpB);
-        MSM_LAUNCH(p, (k_prolong_axis<T, false><<<blocks_for(tot, 256), 256, 0, st>>>(d, c.lo[ax], f.lo[ax], Jt, src, dst)));
+        MSM_LAUNCH(p, (k_prolong_axis<T, false><<<axis_grid(d), axis_block(), 0, st>>>(d, c.lo[ax], f.lo[ax], Jt, src, dst)));
         src = dst;
       } else {
-        MSM_LAUNCH(p, (k_prolong_axis<T, true><<<blocks_for(tot, 256), 256, 0, st>>>(d, c.lo[ax], f.lo[ax], Jt, src,
+        MSM_LAUNCH(p, (k_prolong_axis<T, true><<<axis_grid(d), axis_block(), 0, st>>>(d, c.lo[ax], f.lo[ax], Jt, src,
                                                                                     (T*)p->lev[l].E)));
       }
       din[ax] = f.M[ax];

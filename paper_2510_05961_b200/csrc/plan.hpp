@@ -58,10 +58,11 @@ struct msm_plan {
   int cap = 0;
   msm::BinGeom bg{};
   int n_pcells = 0, n_gcells = 0, pair_rows = 0, pair_ymax = 1, pair_blocks = 0;
-  int* ibuf = nullptr;          // [phist(n_pcells+1) | ghist(n_gcells+1) | pfill | gfill | flag]
+  int* ibuf = nullptr;          // [phist(n_pcells) | ghist(n_gcells) | flag]: zeroed per call
   size_t ibuf_count = 0;
-  int *phist = nullptr, *ghist = nullptr, *pfill = nullptr, *gfill = nullptr, *flag = nullptr;
+  int *phist = nullptr, *ghist = nullptr, *flag = nullptr;
   int *pstart = nullptr, *gstart = nullptr, *ptotals = nullptr, *gtotals = nullptr;
+  int *pslot = nullptr, *gslot = nullptr;
   int *pcell = nullptr, *gcell = nullptr, *porder = nullptr, *gorder = nullptr, *pcellx = nullptr,
       *gcell_sorted = nullptr;
   void *prec = nullptr, *grec = nullptr, *Fsr = nullptr, *Vsr = nullptr;

@@ -20,7 +20,7 @@ __device__ __forceinline__ double wrap_coord(double x, double L, int periodic) {
 template <typename T>
 __global__ void k_bin(int n, const T* __restrict__ pos, BinGeom g, int* __restrict__ pcell,
                       int* __restrict__ gcell, int* __restrict__ phist, int* __restrict__ ghist,
-                      int* __restrict__ flag) {
+                      int* __restrict__ pslot, int* __restrict__ gslot, int* __restrict__ flag) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   int pc[3], gc[3];
@@ -41,8 +41,8 @@ __global__ void k_bin(int n, const T* __restrict__ pos, BinGeom g, int* __restri
   const int gci = (gc[2] * g.ng[1] + gc[1]) * g.ng[0] + gc[0];
   pcell[i] = pci;
   gcell[i] = gci;
-  atomicAdd(&phist[pci], 1);
-  atomicAdd(&ghist[gci], 1);
+  pslot[i] = atomicAdd(&phist[pci], 1);   // arrival rank inside the cell (any order: k_sort_cells fixes it)
+  gslot[i] = atomicAdd(&ghist[gci], 1);
 }
 
 // exclusive scan, three kernels: per-block scan of 4096-element tiles, scan of the tile totals,
@@ -131,16 +131,15 @@ __global__ void k_scan_add(int m, int* __restrict__ out, const int* __restrict__
   if (i == 0) out[m] = n_total;
 }
 
-// pass 2: scatter original indices into their cell's segment (slot order arbitrary here)
+// pass 2: scatter original indices into their cell's segment (slot = arrival rank from pass 1)
 __global__ void k_scatter(int n, const int* __restrict__ pcell, const int* __restrict__ gcell,
                           const int* __restrict__ pstart, const int* __restrict__ gstart,
-                          int* __restrict__ pfill, int* __restrict__ gfill, int* __restrict__ porder,
+                          const int* __restrict__ pslot, const int* __restrict__ gslot, int* __restrict__ porder,
                           int* __restrict__ gorder) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  const int pc = pcell[i], gc = gcell[i];
-  porder[pstart[pc] + atomicAdd(&pfill[pc], 1)] = i;
-  gorder[gstart[gc] + atomicAdd(&gfill[gc], 1)] = i;
+  porder[pstart[pcell[i]] + pslot[i]] = i;
+  gorder[gstart[gcell[i]] + gslot[i]] = i;
 }
 
 // pass 3: canonical order inside each cell (ascending original index): insertion sort per cell
