@@ -301,14 +301,14 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   p->gcell_sorted = (int*)dev_alloc(p, cap * sizeof(int));
   p->prec = dev_alloc(p, cap * 4 * p->esz);
   p->grec = dev_alloc(p, cap * 4 * p->esz);
-  p->Fsr = dev_alloc(p, cap * 3 * p->esz);
-  p->Vsr = dev_alloc(p, cap * p->esz);
+  p->Fsr = dev_alloc(p, (size_t)kPairMaxSplit * cap * 3 * p->esz);   // per-split partials of the pair kernel
+  p->Vsr = dev_alloc(p, (size_t)kPairMaxSplit * cap * p->esz);
   p->pair_ymax = (int)((cap / 32 + p->pair_rows) / p->pair_rows + 3) / 4 + 1;
-  p->pair_wpart = (double*)dev_alloc(p, (size_t)p->pair_rows * p->pair_ymax * kPairWarps * 6 * sizeof(double));
+  p->pair_wpart = (double*)dev_alloc(p, (size_t)p->pair_rows * p->pair_ymax * kPairMaxSplit * kPairWarps * 6 * sizeof(double));
   p->n_eblocks = (int)((cap + 127) / 128);
   p->epart = (double*)dev_alloc(p, (size_t)p->n_eblocks * sizeof(double));
   {
-    const size_t rows = (size_t)p->pair_rows * p->pair_ymax * kPairWarps + p->conv.total_vunits + p->G + p->n_eblocks;
+    const size_t rows = (size_t)p->pair_rows * p->pair_ymax * kPairMaxSplit * kPairWarps + p->conv.total_vunits + p->G + p->n_eblocks;
     p->part_blocks = (int)(rows / 1024 + MSM_MAX_LEVELS + 8);
     p->part = (double*)dev_alloc(p, (size_t)p->part_blocks * 7 * sizeof(double));
   }

@@ -1,5 +1,6 @@
 // msm_evaluate.cu -- msm_evaluate: enqueues the whole hot path (S1..S9 of DESIGN.md) on one stream.
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 
 #include "gridops.cuh"
@@ -150,8 +151,15 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
     pp.p = P;
     // tiles of 32 particles per cell row, spread over gridDim.y blocks of kPairWarps warps
     const int per_row = (n / 32 + p->pair_rows) / p->pair_rows;
-    const dim3 pgrid(p->pair_rows, std::max(1, std::min(p->pair_ymax, (per_row + kPairWarps - 1) / kPairWarps)));
-    p->pair_blocks = (int)(pgrid.x * pgrid.y);
+    // few tiles (small systems): deal the dz planes of the neighbourhood to separate blocks
+    const int nplanes = pp.omax[2] - pp.omin[2] + 1;
+    static const int split_tiles = std::getenv("MSM_PAIR_SPLIT_TILES") ? std::atoi(std::getenv("MSM_PAIR_SPLIT_TILES")) : 8192;
+    pp.nsplit = n / 32 < split_tiles ? std::min(nplanes, kPairMaxSplit) : 1;
+    pp.part_stride = (size_t)p->cap;
+    p->pair_nsplit = pp.nsplit;
+    const dim3 pgrid(p->pair_rows, std::max(1, std::min(p->pair_ymax, (per_row + kPairWarps - 1) / kPairWarps)),
+                     pp.nsplit);
+    p->pair_blocks = (int)(pgrid.x * pgrid.y * pgrid.z);
     const bool mi = pp.minimg[0] || pp.minimg[1] || pp.minimg[2];
 #define MSM_PAIR(V, M) MSM_LAUNCH(p, (k_pair<T, P, V, M><<<pgrid, kPairWarps * 32, 0, st>>>(           \
     pp, p->pstart, (const V4*)p->prec, p->pcellx, p->porder, (T*)p->Fsr, (T*)p->Vsr, p->pair_wpart)))
@@ -309,7 +317,7 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
   // ---------------- S8 interpolation + outputs
   const int neb = (int)blocks_for(n, 128);
   MSM_LAUNCH(p, (k_interpolate<T, P><<<neb, 128, 0, st>>>(
-                    n, gg, tab, (T)(1.0 / H.lev[1].h[0]), (T)(1.0 / H.lev[1].h[1]), (T)(1.0 / H.lev[1].h[2]),
+                    n, p->pair_nsplit, (size_t)p->cap, gg, tab, (T)(1.0 / H.lev[1].h[0]), (T)(1.0 / H.lev[1].h[1]), (T)(1.0 / H.lev[1].h[2]),
                     (T)(p->S->gamma0() / p->mp.a), (const V4*)p->grec, p->gcell_sorted, p->gorder,
                     (const T*)p->lev[1].E, (const T*)p->Fsr, (const T*)p->Vsr, (T*)d_F, (T*)d_V, p->epart)));
   mark();

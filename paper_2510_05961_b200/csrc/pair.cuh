@@ -18,6 +18,8 @@
 //            precision. Rounds = the largest hit count of any lane in the batch, so the expensive
 //            path runs at 60-70 % lane utilisation instead of ~20 %, with ~6 instructions of
 //            bookkeeping per round.
+// Small systems have too few tiles to fill the GPU: the dz planes of the neighbourhood are then
+// dealt to up to kPairMaxSplit blocks (blockIdx.z) whose partial sums k_interpolate adds in order.
 // Every lane visits its hits in ascending candidate order, so the sums have a fixed order
 // (deterministic). -k_0'(r)/r = 1/r^3 + (2/a^3) g'(s), s = r^2/a^2 - 1: one rsqrt per pair is the
 // only special function.
@@ -37,9 +39,12 @@ template <typename T> struct PairParams {
   float a2_scan;          // cutoff^2 of the fp32 scan (widened by rounding slack in fp64 mode)
   T c[8];                 // binom(-1/2, k)
   int p;
+  int nsplit;             // the dz planes of the neighbourhood are dealt to nsplit blocks (blockIdx.z)
+  size_t part_stride;     // elements between the per-split partial outputs (capacity)
 };
 
 constexpr int kPairWarps = 4;
+constexpr int kPairMaxSplit = 5;
 
 template <typename T> struct PairStage;       // shared-memory staging of one warp
 template <> struct PairStage<float> {
@@ -194,7 +199,7 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
       selfpos = -1;
     };
 
-    for (int dz = prm.omin[2]; dz <= prm.omax[2]; ++dz) {
+    for (int dz = prm.omin[2] + (int)blockIdx.z; dz <= prm.omax[2]; dz += prm.nsplit) {
       int czj = cz + dz;
       if (prm.periodic[2]) czj = imod(czj, prm.nc[2]);
       else if (czj < 0 || czj >= prm.nc[2]) continue;
@@ -235,10 +240,11 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
     if (iv) {
       const int orig = porder[ki];
       const T qi = ri.w;
-      Fsr[3 * (size_t)orig + 0] = qi * ax;
-      Fsr[3 * (size_t)orig + 1] = qi * ay;
-      Fsr[3 * (size_t)orig + 2] = qi * az;
-      Vsr[orig] = av;
+      T* Fp = Fsr + (size_t)blockIdx.z * 3 * prm.part_stride;   // partial of this split
+      Fp[3 * (size_t)orig + 0] = qi * ax;
+      Fp[3 * (size_t)orig + 1] = qi * ay;
+      Fp[3 * (size_t)orig + 2] = qi * az;
+      Vsr[(size_t)blockIdx.z * prm.part_stride + orig] = av;
       if (VIRIAL) {
         const double hq = 0.5 * (double)qi;   // every pair is visited from both ends
         W[0] += hq * (double)w0; W[1] += hq * (double)w1; W[2] += hq * (double)w2;
@@ -253,7 +259,8 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
       double v = W[k];
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-      if (lane == 0) wpart[(((size_t)blockIdx.y * gridDim.x + blockIdx.x) * kPairWarps + wid) * 6 + k] = v;
+      if (lane == 0)
+        wpart[((((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * kPairWarps + wid) * 6 + k] = v;
     }
   }
 }

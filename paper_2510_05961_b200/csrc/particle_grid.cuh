@@ -64,7 +64,8 @@ k_anterpolate(GridGeom g, SplineTab<T, P> tab, const int* __restrict__ gstart,
 // and the block's share of U = 1/2 sum_i q_i potential_i (fp64, fixed order).
 template <typename T, int P>
 __global__ void __launch_bounds__(128)
-k_interpolate(int n, GridGeom g, SplineTab<T, P> tab, T inv_h0, T inv_h1, T inv_h2, T self_coef,
+k_interpolate(int n, int nsplit, size_t part_stride, GridGeom g, SplineTab<T, P> tab, T inv_h0, T inv_h1, T inv_h2,
+              T self_coef,
               const typename Vec4<T>::type* __restrict__ grec, const int* __restrict__ gcell_sorted,
               const int* __restrict__ gorder, const T* __restrict__ E, const T* __restrict__ Fsr,
               const T* __restrict__ Vsr, T* __restrict__ F_out, T* __restrict__ V_out,
@@ -115,12 +116,19 @@ k_interpolate(int n, GridGeom g, SplineTab<T, P> tab, T inv_h0, T inv_h1, T inv_
     }
     const int orig = gorder[k];
     const T q = r.w;
-    const T pot = Vsr[orig] + v - q * self_coef;
+    // short-range partials of the pair kernel's splits, added in split order
+    T vs = Vsr[orig], fsx = Fsr[3 * (size_t)orig + 0], fsy = Fsr[3 * (size_t)orig + 1], fsz = Fsr[3 * (size_t)orig + 2];
+    for (int s = 1; s < nsplit; ++s) {
+      vs += Vsr[s * part_stride + orig];
+      const T* Fp = Fsr + s * 3 * part_stride;
+      fsx += Fp[3 * (size_t)orig + 0]; fsy += Fp[3 * (size_t)orig + 1]; fsz += Fp[3 * (size_t)orig + 2];
+    }
+    const T pot = vs + v - q * self_coef;
     if (V_out) V_out[orig] = pot;
     if (F_out) {
-      F_out[3 * (size_t)orig + 0] = Fsr[3 * (size_t)orig + 0] - q * gx * inv_h0;
-      F_out[3 * (size_t)orig + 1] = Fsr[3 * (size_t)orig + 1] - q * gy * inv_h1;
-      F_out[3 * (size_t)orig + 2] = Fsr[3 * (size_t)orig + 2] - q * gz * inv_h2;
+      F_out[3 * (size_t)orig + 0] = fsx - q * gx * inv_h0;
+      F_out[3 * (size_t)orig + 1] = fsy - q * gy * inv_h1;
+      F_out[3 * (size_t)orig + 2] = fsz - q * gz * inv_h2;
     }
     e_i = 0.5 * (double)q * (double)pot;
   }

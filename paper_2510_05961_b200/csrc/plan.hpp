@@ -57,7 +57,7 @@ struct msm_plan {
   // particles
   int cap = 0;
   msm::BinGeom bg{};
-  int n_pcells = 0, n_gcells = 0, pair_rows = 0, pair_ymax = 1, pair_blocks = 0;
+  int n_pcells = 0, n_gcells = 0, pair_rows = 0, pair_ymax = 1, pair_blocks = 0, pair_nsplit = 1;
   int* ibuf = nullptr;          // [phist(n_pcells) | ghist(n_gcells) | flag]: zeroed per call
   size_t ibuf_count = 0;
   int *phist = nullptr, *ghist = nullptr, *flag = nullptr;
