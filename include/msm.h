@@ -97,8 +97,12 @@ msm_status_t msm_plan_info(const msm_plan_t *plan, msm_plan_info_t *info_out);
  *   h_virial     host, 6 doubles xx yy zz xy xz yz of -dU/d eps_ab (number of grid points and a
  *                fixed, reading V); may be NULL (the strain-derivative work is then skipped).
  * The caller owns all six buffers; the plan owns every scratch buffer and msm_evaluate allocates
- * nothing.  Device outputs are stream-ordered; the call synchronises the stream before returning
- * (it always reads back the status flag, the energy and the virial in one small copy).
+ * nothing.  The work is ordered after everything already enqueued on cuda_stream, and the call
+ * returns only when it is complete (it always reads back the status flag, the energy and the virial
+ * in one small copy).  From the second consecutive call with identical arguments on, the launch
+ * sequence is captured into a CUDA graph and replayed on a plan-owned stream (a small system is
+ * otherwise bound by its ~40-60 dependent kernel launches); results are bit-identical either way.
+ * MSM_NO_GRAPH=1 in the environment at plan creation disables this.
  * Neutrality is assumed on periodic axes: the single-point top level contributes zero (reading
  * T2), which for a non-neutral input is the neutralising-background convention. */
 msm_status_t msm_evaluate(msm_plan_t *plan, int n, const void *d_positions, const void *d_charges,

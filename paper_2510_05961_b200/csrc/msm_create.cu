@@ -320,6 +320,10 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   if (cudaMallocHost((void**)&p->h_results, 8 * sizeof(double)) != cudaSuccess) return MSM_ERR_NOMEM;
   for (int i = 0; i <= kMaxStages; ++i)
     if (cudaEventCreate(&p->ev[i]) != cudaSuccess) return MSM_ERR_CUDA;
+  if (cudaStreamCreateWithFlags(&p->gstream, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->gev, cudaEventDisableTiming) != cudaSuccess)
+    return MSM_ERR_CUDA;
+  if (const char* e = std::getenv("MSM_NO_GRAPH")) p->graph_enabled = std::atoi(e) == 0;
   // stage list of msm_evaluate, in launch order
   for (const char* s : {"sort", "pair", "anterpolate", "restrict"}) p->stage_name_store.push_back(s);
   for (const char* s : {"filter", "conv", "conv_virial"}) p->stage_name_store.push_back(s);
@@ -336,6 +340,9 @@ extern "C" {
 void msm_plan_destroy(msm_plan_t* p) {
   if (!p) return;
   for (void* d : p->allocs) cudaFree(d);
+  if (p->gexec) cudaGraphExecDestroy(p->gexec);
+  if (p->gstream) cudaStreamDestroy(p->gstream);
+  if (p->gev) cudaEventDestroy(p->gev);
   if (p->h_results) cudaFreeHost(p->h_results);
   for (int i = 0; i <= kMaxStages; ++i)
     if (p->ev[i]) cudaEventDestroy(p->ev[i]);

@@ -92,14 +92,21 @@ template <typename T, int P> SplineTab<T, P> make_tab(const SplinePieces& sp) {
 #define MSM_LAUNCH(plan, ...) do { __VA_ARGS__; ++(plan)->launches; } while (0)
 
 template <typename T, int P>
-msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, void* d_F, void* d_V,
-                        bool want_virial, cudaStream_t st) {
+msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, void* d_F, void* d_V,
+                       bool want_virial, cudaStream_t st, bool capturing) {
   using V4 = typename Vec4<T>::type;
   const Hierarchy& H = *p->H;
   const T* pos = (const T*)d_pos;
   const T* q = (const T*)d_q;
   int evi = 0;
-  auto mark = [&]() { if (p->profiling) cudaEventRecord(p->ev[evi], st); ++evi; };
+  // stage events; inside a stream capture they become external event-record nodes of the graph
+  auto mark = [&]() {
+    if (p->profiling) {
+      if (capturing) cudaEventRecordWithFlags(p->ev[evi], st, cudaEventRecordExternal);
+      else cudaEventRecord(p->ev[evi], st);
+    }
+    ++evi;
+  };
   p->launches = 0;
   mark();
 
@@ -153,7 +160,7 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
     const int per_row = (n / 32 + p->pair_rows) / p->pair_rows;
     // few tiles (small systems): deal the dz planes of the neighbourhood to separate blocks
     const int nplanes = pp.omax[2] - pp.omin[2] + 1;
-    static const int split_tiles = std::getenv("MSM_PAIR_SPLIT_TILES") ? std::atoi(std::getenv("MSM_PAIR_SPLIT_TILES")) : 8192;
+    static const int split_tiles = std::getenv("MSM_PAIR_SPLIT_TILES") ? std::atoi(std::getenv("MSM_PAIR_SPLIT_TILES")) : 16384;
     pp.nsplit = n / 32 < split_tiles ? std::min(nplanes, kPairMaxSplit) : 1;
     pp.part_stride = (size_t)p->cap;
     p->pair_nsplit = pp.nsplit;
@@ -345,6 +352,23 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
   MSM_LAUNCH(p, (k_finalize<<<1, 256, 0, st>>>(nblk, p->part, p->flag, p->results)));
   mark();
   cudaMemcpyAsync(p->h_results, p->results, 8 * sizeof(double), cudaMemcpyDeviceToHost, st);
+  return MSM_OK;
+}
+
+msm_status_t enqueue(msm_plan* p, int n, const void* pos, const void* q, void* F, void* V, bool wv, cudaStream_t st,
+                     bool capturing) {
+#define MSM_CASE(TT, PP) return enqueue_t<TT, PP>(p, n, pos, q, F, V, wv, st, capturing)
+  if (p->fp32) {
+    switch (p->P) { case 4: MSM_CASE(float, 4); case 6: MSM_CASE(float, 6); case 8: MSM_CASE(float, 8); }
+  } else {
+    switch (p->P) { case 4: MSM_CASE(double, 4); case 6: MSM_CASE(double, 6); case 8: MSM_CASE(double, 8); }
+  }
+#undef MSM_CASE
+  return MSM_ERR_UNSUPPORTED;
+}
+
+// wait for the evaluation enqueued on st, then read the stage times
+msm_status_t finish(msm_plan* p, cudaStream_t st) {
   if (cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }
   if (cudaGetLastError() != cudaSuccess) return MSM_ERR_CUDA;
   if (p->profiling)
@@ -352,14 +376,44 @@ msm_status_t evaluate_t(msm_plan* p, int n, const void* d_pos, const void* d_q, 
   return MSM_OK;
 }
 
-template <typename T>
-msm_status_t evaluate_p(msm_plan* p, int n, const void* pos, const void* q, void* F, void* V, bool wv, cudaStream_t st) {
-  switch (p->P) {
-    case 4: return evaluate_t<T, 4>(p, n, pos, q, F, V, wv, st);
-    case 6: return evaluate_t<T, 6>(p, n, pos, q, F, V, wv, st);
-    case 8: return evaluate_t<T, 8>(p, n, pos, q, F, V, wv, st);
+void drop_graph(msm_plan* p) {
+  if (p->gexec) { cudaGraphExecDestroy(p->gexec); p->gexec = nullptr; }
+}
+
+// One evaluation. The ~40-60 dependent launches of a small system cost more than their work, so the
+// second consecutive call with the same arguments captures the launch sequence into a CUDA graph
+// (on a plan-owned stream) and later calls replay it; any change of arguments, or any failure of
+// the capture, falls back to direct launches on the caller's stream.
+msm_status_t run(msm_plan* p, int n, const void* pos, const void* q, void* F, void* V, bool wv, cudaStream_t st) {
+  const msm::GraphKey key{n, pos, q, F, V, wv, p->profiling};
+  if (p->graph_enabled && p->gstream && key == p->gkey) {
+    if (!p->gexec) {
+      cudaGraph_t g = nullptr;
+      if (cudaStreamBeginCapture(p->gstream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+        const msm_status_t es = enqueue(p, n, pos, q, F, V, wv, p->gstream, true);
+        const cudaError_t ce = cudaStreamEndCapture(p->gstream, &g);
+        if (es == MSM_OK && ce == cudaSuccess && g && cudaGraphInstantiate(&p->gexec, g, 0) != cudaSuccess)
+          p->gexec = nullptr;
+        if (g) cudaGraphDestroy(g);
+      }
+      if (!p->gexec) { cudaGetLastError(); p->graph_enabled = false; }   // never try again on this plan
+    }
+    if (p->gexec) {
+      // order the replay after the caller's stream; the call synchronises before it returns
+      if (cudaEventRecord(p->gev, st) == cudaSuccess && cudaStreamWaitEvent(p->gstream, p->gev, 0) == cudaSuccess &&
+          cudaGraphLaunch(p->gexec, p->gstream) == cudaSuccess)
+        return finish(p, p->gstream);
+      cudaGetLastError();
+      drop_graph(p);
+      p->graph_enabled = false;
+    }
+  } else if (!(key == p->gkey)) {
+    p->gkey = key;
+    drop_graph(p);
   }
-  return MSM_ERR_UNSUPPORTED;
+  const msm_status_t es = enqueue(p, n, pos, q, F, V, wv, st, false);
+  if (es != MSM_OK) return es;
+  return finish(p, st);
 }
 
 }  // namespace
@@ -373,8 +427,7 @@ msm_status_t msm_evaluate(msm_plan_t* p, int n, const void* d_positions, const v
   if (cudaSetDevice(p->prm.device) != cudaSuccess) return MSM_ERR_CUDA;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const bool wv = h_virial != nullptr;
-  const msm_status_t s = p->fp32 ? evaluate_p<float>(p, n, d_positions, d_charges, d_forces, d_potentials, wv, st)
-                                 : evaluate_p<double>(p, n, d_positions, d_charges, d_forces, d_potentials, wv, st);
+  const msm_status_t s = run(p, n, d_positions, d_charges, d_forces, d_potentials, wv, st);
   if (s != MSM_OK) return s;
   if (h_energy) *h_energy = p->h_results[0];
   if (h_virial) std::memcpy(h_virial, p->h_results + 1, 6 * sizeof(double));

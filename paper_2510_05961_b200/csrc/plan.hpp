@@ -20,6 +20,17 @@ struct LevelDev {
   int taps = 0;
 };
 
+// arguments of one msm_evaluate: a captured CUDA graph is replayed only for an identical call
+struct GraphKey {
+  int n = -1;
+  const void *pos = nullptr, *q = nullptr;
+  void *F = nullptr, *V = nullptr;
+  bool virial = false, profiling = false;
+  bool operator==(const GraphKey& o) const {
+    return n == o.n && pos == o.pos && q == o.q && F == o.F && V == o.V && virial == o.virial && profiling == o.profiling;
+  }
+};
+
 }  // namespace msm
 
 struct msm_plan {
@@ -73,6 +84,13 @@ struct msm_plan {
   double* h_results = nullptr;  // pinned: U, W[6], flag
   // staging for msm_evaluate_host
   void *in_pos = nullptr, *in_q = nullptr, *out_F = nullptr, *out_V = nullptr;
+
+  // CUDA graph of the launch sequence (msm_evaluate.cu: run)
+  bool graph_enabled = true;
+  msm::GraphKey gkey{};
+  cudaStream_t gstream = nullptr;
+  cudaGraphExec_t gexec = nullptr;
+  cudaEvent_t gev = nullptr;
 
   // profiling
   bool profiling = false;
