@@ -137,7 +137,7 @@ void msm_plan_destroy(msm_plan_t *plan);
 const char *msm_status_string(msm_status_t s);
 
 /* Microbenchmarks used for the roofline denominators the driver does not provide (FP32 / FP64
- * FMA peak of the CUDA cores).  kind 0: FFMA, 1: DFMA.  Returns TFLOP/s (2 flops per FMA) through
+ * FMA peak of the CUDA cores).  kind 0: FFMA, 1: DFMA, 2: FFMA2 (packed fma.rn.f32x2).  Returns TFLOP/s (2 flops per FMA) through
  * *tflops, timed with CUDA events on the given device. */
 msm_status_t msm_measure_fma_peak(int device, int kind, double *tflops);
 

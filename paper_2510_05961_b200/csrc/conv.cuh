@@ -47,6 +47,8 @@ struct ConvLevel {
   const int4* rows;           // (tap chunk offset, first chunk, last chunk, -) per (dz, dy)
   const int4* vrows;          // same for the half-space virial taps
   const void* staps;          // s_l in 4-tap chunks
+  const int4* rows2;          // fp32 packed path: per (d, dy), d = -R[2] .. R[2]+1, rows d and d-1 merged
+  const void* taps2;          // per chunk 8 floats: (s_d[t], s_{d-1}[t]) for the chunk's 4 taps
   const void* vtaps;          // per chunk: 4 x 2g, 4 x 2g dx, 4 x 2g dx^2
   const void* pad;            // omega'-filtered haloed grid charge
   const void* Q;              // grid charge (virial)
@@ -70,6 +72,11 @@ template <> struct SmemVec<float> {
     const float4 t = __ldg(reinterpret_cast<const float4*>(p));
     v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
   }
+  // streaming load that does not allocate in L1 (the L1 is kept for the tap tables)
+  static __device__ __forceinline__ void ldcg(const float* p, float (&v)[4]) {
+    const float4 t = __ldcg(reinterpret_cast<const float4*>(p));
+    v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+  }
 };
 template <> struct SmemVec<double> {
   static __device__ __forceinline__ void load4(const double* p, double (&v)[4]) {
@@ -80,6 +87,11 @@ template <> struct SmemVec<double> {
   static __device__ __forceinline__ void ldg(const double* p, double (&v)[4]) {
     const double2 a = __ldg(reinterpret_cast<const double2*>(p));
     const double2 b = __ldg(reinterpret_cast<const double2*>(p + 2));
+    v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+  }
+  static __device__ __forceinline__ void ldcg(const double* p, double (&v)[4]) {
+    const double2 a = __ldcg(reinterpret_cast<const double2*>(p));
+    const double2 b = __ldcg(reinterpret_cast<const double2*>(p + 2));
     v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
   }
 };
@@ -94,7 +106,7 @@ __device__ __forceinline__ void stage_plane(const ConvLevel& g, const T* __restr
   for (int v = lane; v < nvec; v += 32) {
     const int r = v / vper, cx = (v - r * vper) * 4;
     T t[4];
-    SmemVec<T>::ldg(src + (size_t)r * g.P[0] + cx, t);
+    SmemVec<T>::ldcg(src + (size_t)r * g.P[0] + cx, t);
     T* dst = plane + r * g.pitch + cx;
     dst[0] = t[0]; dst[1] = t[1]; dst[2] = t[2]; dst[3] = t[3];
   }
@@ -205,6 +217,121 @@ k_conv(const ConvTable* __restrict__ tabp) {
 #pragma unroll
         for (int i = 0; i < XT; ++i)
           if (X + i < g.M[0]) dst[i] = acc[k][i];
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------- potential, fp32 with packed FMAs
+// Blackwell's fma.rn.f32x2 (SASS FFMA2) does two fp32 multiply-adds per instruction and lane at the
+// same flop rate as FFMA, i.e. with half the issue slots -- and this kernel is bound by instruction
+// issue (71 % of its instructions are FMAs). The pair is taken along z: the accumulators of output
+// planes (2kp, 2kp+1) form one 64-bit register pair, the window value is the scalar (broadcast)
+// operand, and the taps of the two stencil rows dz = d and d - 1 that feed those planes from one
+// input plane are stored interleaved (taps2), so one FFMA2 replaces two FFMAs with no extra moves.
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2(unsigned long long v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+// acc += s * pair (s broadcast to both halves; ptxas folds the duplicate into a scalar operand)
+__device__ __forceinline__ void ffma2_bcast(unsigned long long& acc, float s, unsigned long long pair) {
+  asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(pack2(s, s)), "l"(pair));
+}
+
+template <int XT>
+__global__ void __launch_bounds__(32, 16)
+k_conv_f2(const ConvTable* __restrict__ tabp) {
+  constexpr int ZT = 4, ZP = 2;                       // two pairs of output planes
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float* plane = reinterpret_cast<float*>(smem_raw);
+  const ConvTable& tab = *tabp;
+  const int lane = threadIdx.x;
+  const ConvUnit cu = decode_unit<false, XT, ZT>(tab, blockIdx.x);
+  const ConvLevel& g = tab.lev[cu.lev];
+  const int X = cu.X, Y = cu.Y, Z = cu.Z;
+  const int Ry = g.R[1], Rz = g.R[2];
+  const int nrow = 32 + 2 * Ry;
+  const int WX = XT + 2 * g.X0 + 4;
+  const int ny = g.ny;
+  const int4* __restrict__ rows2 = g.rows2;
+  const float4* __restrict__ taps2 = reinterpret_cast<const float4*>(g.taps2);
+  const float* __restrict__ qpad = reinterpret_cast<const float*>(g.pad);
+
+  unsigned long long acc[ZP][XT];                     // (plane 2kp, plane 2kp + 1) of output x + i
+#pragma unroll
+  for (int k = 0; k < ZP; ++k)
+#pragma unroll
+    for (int i = 0; i < XT; ++i) acc[k][i] = 0ull;
+
+  const int p0 = g.pb[cu.slice], p1 = g.pb[cu.slice + 1];
+  for (int pz = p0; pz < p1; ++pz) {
+    const int zr = pz - Rz;                           // input plane z = Z + zr
+    stage_plane<float>(g, qpad, plane, Z + pz, X, Y, nrow, WX, lane);
+    for (int dy = -Ry; dy <= Ry; ++dy) {
+      int4 re[ZP];
+      int cl = 1 << 30, ch = -1;
+#pragma unroll
+      for (int k = 0; k < ZP; ++k) {
+        const int d = zr - 2 * k;                     // planes (2k, 2k+1) take stencil rows (d, d - 1)
+        if (d >= -Rz && d <= Rz + 1) re[k] = __ldg(rows2 + (d + Rz) * ny + (dy + Ry));
+        else re[k] = make_int4(0, 1, 0, 0);           // empty
+        if (re[k].y <= re[k].z) { cl = min(cl, re[k].y); ch = max(ch, re[k].z); }
+      }
+      const float* srow = plane + (lane + dy + Ry) * g.pitch;
+      for (int c = cl; c <= ch; ++c) {
+        float win[XT + 4];
+#pragma unroll
+        for (int j = 0; j < XT + 4; j += 4) {
+          const float4 t = *reinterpret_cast<const float4*>(srow + 4 * c + j);
+          win[j] = t.x; win[j + 1] = t.y; win[j + 2] = t.z; win[j + 3] = t.w;
+        }
+        float4 tq[ZP][2];
+        bool on[ZP];
+#pragma unroll
+        for (int k = 0; k < ZP; ++k) {
+          on[k] = c >= re[k].y && c <= re[k].z;
+          const float4* tp = taps2 + (on[k] ? (re[k].x + c - re[k].y) * 2 : 0);
+          tq[k][0] = __ldg(tp);
+          tq[k][1] = __ldg(tp + 1);
+        }
+#pragma unroll
+        for (int k = 0; k < ZP; ++k) {
+          if (on[k]) {
+            const unsigned long long t0 = pack2(tq[k][0].x, tq[k][0].y), t1 = pack2(tq[k][0].z, tq[k][0].w);
+            const unsigned long long t2 = pack2(tq[k][1].x, tq[k][1].y), t3 = pack2(tq[k][1].z, tq[k][1].w);
+#pragma unroll
+            for (int i = 0; i < XT; ++i) {
+              ffma2_bcast(acc[k][i], win[i], t0);
+              ffma2_bcast(acc[k][i], win[i + 1], t1);
+              ffma2_bcast(acc[k][i], win[i + 2], t2);
+              ffma2_bcast(acc[k][i], win[i + 3], t3);
+            }
+          }
+        }
+      }
+    }
+  }
+  // outputs (slice partial or the final value)
+  const int y = Y + lane;
+  if (y < g.M[1]) {
+    float* out = reinterpret_cast<float*>(g.out) + (size_t)cu.slice * g.M[0] * g.M[1] * g.M[2];
+#pragma unroll
+    for (int k = 0; k < ZP; ++k) {
+      float* d0 = out + ((size_t)(Z + 2 * k) * g.M[1] + y) * g.M[0] + X;
+      float* d1 = d0 + (size_t)g.M[1] * g.M[0];
+      const bool z0 = Z + 2 * k < g.M[2], z1 = Z + 2 * k + 1 < g.M[2];
+#pragma unroll
+      for (int i = 0; i < XT; ++i) {
+        float lo, hi;
+        unpack2(acc[k][i], lo, hi);
+        if (X + i < g.M[0]) {
+          if (z0) d0[i] = lo;
+          if (z1) d1[i] = hi;
+        }
       }
     }
   }

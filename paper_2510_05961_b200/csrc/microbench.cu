@@ -23,7 +23,33 @@ __global__ void __launch_bounds__(256) k_fma_chain(T* out, int iters, T a, T b) 
   out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
-template <typename T> msm_status_t measure(double* tflops) {
+// packed pairs: fma.rn.f32x2 (SASS FFMA2) does two fp32 multiply-adds per instruction and lane
+__global__ void __launch_bounds__(256) k_fma2_chain(float* out, int iters, float a, float b) {
+  unsigned long long x[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const float2 v = make_float2((threadIdx.x + i) * 1e-3f, (threadIdx.x + i) * 2e-3f);
+    x[i] = *reinterpret_cast<const unsigned long long*>(&v);
+  }
+  const float2 av = make_float2(a, a), bv = make_float2(b, b);
+  const unsigned long long aa = *reinterpret_cast<const unsigned long long*>(&av);
+  const unsigned long long bb = *reinterpret_cast<const unsigned long long*>(&bv);
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r)
+#pragma unroll
+      for (int i = 0; i < 8; ++i) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(x[i]) : "l"(aa), "l"(bb));
+  }
+  float s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const float2 v = *reinterpret_cast<const float2*>(&x[i]);
+    s += v.x + v.y;
+  }
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+template <typename T> msm_status_t measure(double* tflops, bool packed = false) {
   int sms = 0, dev = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -35,7 +61,8 @@ template <typename T> msm_status_t measure(double* tflops) {
   double best = 0.0;
   for (int rep = 0; rep < 5; ++rep) {
     cudaEventRecord(e0);
-    k_fma_chain<T><<<blocks, threads>>>(out, iters, (T)0.999, (T)1e-4);
+    if (packed) k_fma2_chain<<<blocks, threads>>>((float*)out, iters, 0.999f, 1e-4f);
+    else k_fma_chain<T><<<blocks, threads>>>(out, iters, (T)0.999, (T)1e-4);
     cudaEventRecord(e1);
     if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(out); return MSM_ERR_CUDA; }
     float ms = 0;
@@ -52,7 +79,8 @@ template <typename T> msm_status_t measure(double* tflops) {
 }  // namespace
 
 extern "C" msm_status_t msm_measure_fma_peak(int device, int kind, double* tflops) {
-  if (!tflops || (kind != 0 && kind != 1)) return MSM_ERR_INVALID_ARG;
+  if (!tflops || kind < 0 || kind > 2) return MSM_ERR_INVALID_ARG;
   if (cudaSetDevice(device) != cudaSuccess) return MSM_ERR_CUDA;
+  if (kind == 2) return measure<float>(tflops, true);
   return kind == 0 ? measure<float>(tflops) : measure<double>(tflops);
 }

@@ -132,6 +132,39 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   g.vrows = up_rows(vrows);
   g.staps = upload(p, ts);
   g.vtaps = upload(p, tv);
+  g.rows2 = nullptr;
+  g.taps2 = nullptr;
+  if (p->fp32) {
+    // packed path (k_conv_f2): stencil rows d and d - 1 merged, taps interleaved per tap
+    auto row_rx = [&](int dz, int dy) {               // x half-width of row (dz, dy), -1 if empty
+      if (dz < -Rz || dz > Rz) return -1;
+      const int4& r = rows[(size_t)(dz + Rz) * ny + (dy + st.R[1])];
+      if (r.y > r.z) return -1;
+      const double y = dy * lv.h[1], z = dz * lv.h[2];
+      const double rem = A * A - y * y - z * z;
+      int Rx = std::min(st.R[0], (int)std::floor(std::sqrt(rem) / lv.h[0]));
+      while (Rx >= 0 && (Rx * lv.h[0]) * (Rx * lv.h[0]) >= rem) --Rx;
+      return Rx;
+    };
+    std::vector<int4> r2((size_t)ny * (nz + 1));
+    std::vector<double> t2;
+    for (int d = -Rz; d <= Rz + 1; ++d)
+      for (int dy = -st.R[1]; dy <= st.R[1]; ++dy) {
+        const int ra = row_rx(d, dy), rb = row_rx(d - 1, dy), Rx = std::max(ra, rb);
+        int4& r = r2[(size_t)(d + Rz) * ny + (dy + st.R[1])];
+        if (Rx < 0) { r = make_int4(0, 1, 0, 0); continue; }
+        const int clo = (-Rx + g.X0) / 4, chi = (Rx + g.X0) / 4;
+        r = make_int4((int)(t2.size() / 8), clo, chi, 0);
+        for (int c = clo; c <= chi; ++c)
+          for (int t = 0; t < 4; ++t) {
+            const int dx = 4 * c - g.X0 + t;
+            t2.push_back(ra >= 0 && dx >= -ra && dx <= ra ? st.at(st.s, dx, dy, d) : 0.0);
+            t2.push_back(rb >= 0 && dx >= -rb && dx <= rb ? st.at(st.s, dx, dy, d - 1) : 0.0);
+          }
+      }
+    g.rows2 = up_rows(r2);
+    g.taps2 = upload(p, t2);
+  }
   d.pad = dev_alloc(p, (size_t)g.P[0] * g.P[1] * g.P[2] * p->esz);
   g.pad = d.pad;
   g.Q = d.Q;

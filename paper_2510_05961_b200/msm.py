@@ -72,9 +72,9 @@ def lib():
 
 
 def measure_fma_peak(kind: str = "fp32", device: int = 0) -> float:
-    """TFLOP/s of back-to-back FFMA ("fp32") or DFMA ("fp64") on the CUDA cores."""
+    """TFLOP/s of back-to-back FFMA ("fp32"), DFMA ("fp64") or packed FFMA2 ("fp32x2") on the CUDA cores."""
     out = C.c_double(0.0)
-    st = lib().msm_measure_fma_peak(device, 0 if kind == "fp32" else 1, C.byref(out))
+    st = lib().msm_measure_fma_peak(device, {"fp32": 0, "fp64": 1, "fp32x2": 2}[kind], C.byref(out))
     if st:
         raise MsmError(st, "msm_measure_fma_peak")
     return out.value
