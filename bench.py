@@ -30,6 +30,7 @@ if ROOT not in sys.path:
 METRIC = "msm_energy_forces_particles_per_s"
 UNIT = "particles/s"
 FLOP_PER_PAIR = 30.0          # r^2, rsqrt, Horner g and g', 4 accumulations
+FLOP_PER_CANDIDATE = 9.0      # distance test of a cell-list candidate (pair row)
 SM_COUNT, FP32_LANES, SM_MAX_GHZ = 148, 128, 1.965
 
 
@@ -127,7 +128,16 @@ def stage_work(stage: str, w, plan, esz: int, pairs: float):
         return d[0] * d[1] * d[2]
     nt = info.n_tiled
     if stage == "pair":
-        return "flop", FLOP_PER_PAIR * pairs
+        # 30 flop per in-cutoff directed pair + 9 flop per candidate of the a/2 cell
+        # scheme (the other particles of the 5^3 cells around a particle's cell)
+        nc = info.pair_cells
+        cells = 1
+        reach = 1
+        for ax in range(3):
+            cells *= nc[ax]
+            reach *= min(5, nc[ax])
+        candidates = n * max(reach * n / cells - 1.0, 0.0)
+        return "flop", FLOP_PER_PAIR * pairs + FLOP_PER_CANDIDATE * candidates
     if stage == "conv":                                       # 2 T_s flop per grid point and level
         return "flop", sum(2.0 * info.stencil_taps[l - 1] * G(l) for l in range(1, nt))
     if stage == "conv_virial":                                # correlation over the half space of taps

@@ -242,6 +242,15 @@ __device__ __forceinline__ void ffma2_bcast(unsigned long long& acc, float s, un
   asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(pack2(s, s)), "l"(pair));
 }
 
+// read-only 16-byte load that the compiler may not move (it would otherwise sink the tap loads into
+// the branch that uses them, right in front of the first dependent FMA)
+__device__ __forceinline__ float4 ldg_pinned(const float4* p) {
+  float4 v;
+  asm volatile("ld.global.nc.L1::evict_last.v4.f32 {%0, %1, %2, %3}, [%4];"
+               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+  return v;
+}
+
 template <int XT>
 __global__ void __launch_bounds__(32, 16)
 k_conv_f2(const ConvTable* __restrict__ tabp) {
@@ -278,7 +287,7 @@ k_conv_f2(const ConvTable* __restrict__ tabp) {
       for (int k = 0; k < ZP; ++k) {
         const int d = zr - 2 * k;                     // planes (2k, 2k+1) take stencil rows (d, d - 1)
         if (d >= -Rz && d <= Rz + 1) re[k] = __ldg(rows2 + (d + Rz) * ny + (dy + Ry));
-        else re[k] = make_int4(0, 1, 0, 0);           // empty
+        else re[k] = make_int4(0, 0, -1, 0);          // empty
         if (re[k].y <= re[k].z) { cl = min(cl, re[k].y); ch = max(ch, re[k].z); }
       }
       const float* srow = plane + (lane + dy + Ry) * g.pitch;
@@ -294,9 +303,11 @@ k_conv_f2(const ConvTable* __restrict__ tabp) {
 #pragma unroll
         for (int k = 0; k < ZP; ++k) {
           on[k] = c >= re[k].y && c <= re[k].z;
-          const float4* tp = taps2 + (on[k] ? (re[k].x + c - re[k].y) * 2 : 0);
-          tq[k][0] = __ldg(tp);
-          tq[k][1] = __ldg(tp + 1);
+          // unconditional address (clamped into the row; an empty row reads the guard chunk in front
+          // of the table), so the loads are not tied to the branch below
+          const float4* tp = taps2 + (re[k].x + min(max(c, re[k].y), re[k].z) - re[k].y) * 2;
+          tq[k][0] = ldg_pinned(tp);
+          tq[k][1] = ldg_pinned(tp + 1);
         }
 #pragma unroll
         for (int k = 0; k < ZP; ++k) {

@@ -147,14 +147,14 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
       return Rx;
     };
     std::vector<int4> r2((size_t)ny * (nz + 1));
-    std::vector<double> t2;
+    std::vector<double> t2(8, 0.0);                  // guard chunk in front of the table (index -1)
     for (int d = -Rz; d <= Rz + 1; ++d)
       for (int dy = -st.R[1]; dy <= st.R[1]; ++dy) {
         const int ra = row_rx(d, dy), rb = row_rx(d - 1, dy), Rx = std::max(ra, rb);
         int4& r = r2[(size_t)(d + Rz) * ny + (dy + st.R[1])];
-        if (Rx < 0) { r = make_int4(0, 1, 0, 0); continue; }
+        if (Rx < 0) { r = make_int4(0, 0, -1, 0); continue; }   // empty: clamps to chunk -1
         const int clo = (-Rx + g.X0) / 4, chi = (Rx + g.X0) / 4;
-        r = make_int4((int)(t2.size() / 8), clo, chi, 0);
+        r = make_int4((int)(t2.size() / 8) - 1, clo, chi, 0);
         for (int c = clo; c <= chi; ++c)
           for (int t = 0; t < 4; ++t) {
             const int dx = 4 * c - g.X0 + t;
@@ -163,7 +163,7 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
           }
       }
     g.rows2 = up_rows(r2);
-    g.taps2 = upload(p, t2);
+    g.taps2 = (const char*)upload(p, t2) + 8 * p->esz;   // chunk 0 of the table follows the guard chunk
   }
   d.pad = dev_alloc(p, (size_t)g.P[0] * g.P[1] * g.P[2] * p->esz);
   g.pad = d.pad;
