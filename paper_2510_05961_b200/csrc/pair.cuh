@@ -123,6 +123,11 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
     constexpr bool anymi = MI;
     T ax = 0, ay = 0, az = 0, av = 0;
     T w0 = 0, w1 = 0, w2 = 0, w3 = 0, w4 = 0, w5 = 0;
+    // fp32 drains two hits per lane and round with packed f32x2 arithmetic (FADD2/FMUL2/FFMA2: two
+    // results per instruction and lane, half the issue slots); the halves are added at the end
+    constexpr bool kPacked = sizeof(T) == 4 && !MI;
+    float2 ax2 = {0.f, 0.f}, ay2 = {0.f, 0.f}, az2 = {0.f, 0.f}, av2 = {0.f, 0.f};
+    float2 u0 = {0.f, 0.f}, u1 = {0.f, 0.f}, u2 = {0.f, 0.f}, u3 = {0.f, 0.f}, u4 = {0.f, 0.f}, u5 = {0.f, 0.f};
     int fill = 0;          // candidates staged in the current batch
     int selfpos = -1;      // stage index of the lane's own particle, if it is in the batch
 
@@ -161,6 +166,44 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
       int nmax = n;
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) nmax = max(nmax, __shfl_xor_sync(0xffffffffu, nmax, o));
+      if constexpr (kPacked) {
+        const float* sf = reinterpret_cast<const float*>(sj.f);
+        const float xf = (float)xi, yf = (float)yi, zf = (float)zi;
+        for (int r = 0; r < nmax; r += 2) {
+          if (r < n) {
+            // hits r and r + 1 of this lane; a missing second hit repeats the first with charge 0,
+            // the particle itself gets charge 0 and a harmless distance
+            const bool two = r + 1 < n;
+            const int ia = lp[r * 32], ib = two ? lp[(r + 1) * 32] : ia;
+            const float* pa = sf + ia * 4;
+            const float* pb = sf + ib * 4;
+            const float2 xj = make_float2(pa[0], pb[0]), yj = make_float2(pa[1], pb[1]), zj = make_float2(pa[2], pb[2]);
+            const float2 qj = make_float2(ia != selfpos ? pa[3] : 0.f, (two && ib != selfpos) ? pb[3] : 0.f);
+            const float2 dx = __fadd2_rn(make_float2(xf, xf), make_float2(-xj.x, -xj.y));
+            const float2 dy_ = __fadd2_rn(make_float2(yf, yf), make_float2(-yj.x, -yj.y));
+            const float2 dz_ = __fadd2_rn(make_float2(zf, zf), make_float2(-zj.x, -zj.y));
+            float2 r2 = __ffma2_rn(dx, dx, __ffma2_rn(dy_, dy_, __fmul2_rn(dz_, dz_)));
+            r2.x = fmaxf(r2.x, 1e-20f); r2.y = fmaxf(r2.y, 1e-20f);       // only the self pair is this close
+            const float2 rinv = make_float2(rsqrt_fast(r2.x), rsqrt_fast(r2.y));
+            const float2 sv = __ffma2_rn(r2, make_float2((float)inv_a2, (float)inv_a2), make_float2(-1.f, -1.f));
+            float2 g = make_float2((float)cf[P - 1], (float)cf[P - 1]), dg = make_float2((float)cd[P - 1], (float)cd[P - 1]);
+#pragma unroll
+            for (int k = P - 2; k >= 0; --k) g = __ffma2_rn(g, sv, make_float2((float)cf[k], (float)cf[k]));
+#pragma unroll
+            for (int k = P - 2; k >= 1; --k) dg = __ffma2_rn(dg, sv, make_float2((float)cd[k], (float)cd[k]));
+            const float nia = -(float)inv_a, t3 = (float)two_inv_a3;
+            av2 = __ffma2_rn(qj, __ffma2_rn(g, make_float2(nia, nia), rinv), av2);
+            const float2 rinv3 = __fmul2_rn(__fmul2_rn(rinv, rinv), rinv);
+            const float2 fs = __fmul2_rn(qj, __ffma2_rn(make_float2(t3, t3), dg, rinv3));
+            ax2 = __ffma2_rn(fs, dx, ax2); ay2 = __ffma2_rn(fs, dy_, ay2); az2 = __ffma2_rn(fs, dz_, az2);
+            if (VIRIAL) {
+              const float2 fx = __fmul2_rn(fs, dx), fy = __fmul2_rn(fs, dy_), fz = __fmul2_rn(fs, dz_);
+              u0 = __ffma2_rn(fx, dx, u0); u1 = __ffma2_rn(fy, dy_, u1); u2 = __ffma2_rn(fz, dz_, u2);
+              u3 = __ffma2_rn(fx, dy_, u3); u4 = __ffma2_rn(fx, dz_, u4); u5 = __ffma2_rn(fy, dz_, u5);
+            }
+          }
+        }
+      } else {
       for (int r = 0; r < nmax; ++r) {
         if (r < n) {
           const int idx = lp[r * 32];
@@ -193,6 +236,7 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
             }
           }
         }
+      }
       }
       __syncwarp();
       fill = 0;
@@ -236,6 +280,11 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
       }
     }
     if (fill > 0) process();
+    if (kPacked) {
+      ax += (T)(ax2.x + ax2.y); ay += (T)(ay2.x + ay2.y); az += (T)(az2.x + az2.y); av += (T)(av2.x + av2.y);
+      w0 += (T)(u0.x + u0.y); w1 += (T)(u1.x + u1.y); w2 += (T)(u2.x + u2.y);
+      w3 += (T)(u3.x + u3.y); w4 += (T)(u4.x + u4.y); w5 += (T)(u5.x + u5.y);
+    }
 
     if (iv) {
       const int orig = porder[ki];
