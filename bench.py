@@ -246,6 +246,19 @@ def run_ours(args, rank: int, world: int):
     barrier()
     ms_e2e = sum(a.elapsed_time(b) for a, b in ev2)
 
+    # ---- context: the same step without the virial (energy + forces + potentials only)
+    plan.set_profiling(False)
+    for _ in range(3):
+        plan.evaluate(pos, q, F, V, True, False)
+    ev3 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for s in range(args.steps):
+        flush.fill_(s & 0xFF)
+        ev3[s][0].record()
+        plan.evaluate(pos, q, F, V, True, False)
+        ev3[s][1].record()
+        torch.cuda.synchronize()
+    ms_nov = sum(a.elapsed_time(b) for a, b in ev3)
+
     ms_total, ms_e2e = max_over_ranks(ms_total, ms_e2e, world, dev)
     if rank != 0:
         return None
@@ -287,6 +300,8 @@ def run_ours(args, rank: int, world: int):
         "e2e": {"value": whole_job_value(world, w.n, args.steps, ms_e2e), "unit": UNIT,
                 "h2d_bytes_per_step": w.n * 4 * esz, "d2h_bytes_per_step": w.n * 4 * esz + 64,
                 "ms_per_step": ms_e2e / args.steps},
+        "without_virial": {"value": w.n * args.steps / (ms_nov * 1e-3), "unit": UNIT, "ms_per_step": ms_nov / args.steps,
+                           "note": "rank 0, energy+forces+potentials only; context, not the metric"},
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "stages": stages,
         "energy": energy,
     }
