@@ -50,6 +50,8 @@ struct ConvLevel {
   const int4* rows2;          // fp32 packed path: per (d, dy), d = -R[2] .. R[2]+1, rows d and d-1 merged
   const void* taps2;          // per chunk 8 floats: (s_d[t], s_{d-1}[t]) for the chunk's 4 taps
   const void* vtaps;          // per chunk: 4 x 2g, 4 x 2g dx, 4 x 2g dx^2
+  const int4* vrows2;         // fp32 packed virial: half-space rows d and d - 1 merged, d = 0 .. R[2]+1
+  const void* vtaps2;         // per chunk 24 floats: for 2g, 2g dx, 2g dx^2: 4 taps x (row d, row d - 1)
   const void* pad;            // omega'-filtered haloed grid charge
   const void* Q;              // grid charge (virial)
   void* out;                  // E^l if nslices == 1, else scratch [slice][z][y][x]
@@ -450,6 +452,132 @@ k_conv_virial(const ConvTable* __restrict__ tabp) {
         S[3] = fma(fy, d1, S[3]);
         S[4] = fma(fz, d1, S[4]);
         S[5] = fma(fy * fz, d0, S[5]);
+      }
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 6; ++k) {
+    double v = S[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (lane == 0) g.wpart[(size_t)cu.local * 6 + k] = v;
+  }
+}
+
+// ------------------------------------------------------------------ virial, fp32 with packed FMAs
+// Same pairing as k_conv_f2: output planes (2k, 2k+1) share one register pair. The correlation
+// c_t = sum_i q_i win[i + t] of both planes is one FFMA2 chain (window value = scalar operand,
+// (q_2k, q_2k+1) = pair operand); the x-moments multiply by the interleaved taps of the half-space
+// rows d and d - 1.
+__device__ __forceinline__ void ffma2_pp(unsigned long long& acc, unsigned long long a, unsigned long long b) {
+  asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b));
+}
+__device__ __forceinline__ unsigned long long fadd2_pp(unsigned long long a, unsigned long long b) {
+  unsigned long long r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+
+template <int XT>
+__global__ void __launch_bounds__(32, 16)
+k_conv_virial_f2(const ConvTable* __restrict__ tabp) {
+  constexpr int ZT = 4, ZP = 2;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float* plane = reinterpret_cast<float*>(smem_raw);
+  const ConvTable& tab = *tabp;
+  const int lane = threadIdx.x;
+  const ConvUnit cu = decode_unit<true, XT, ZT>(tab, blockIdx.x);
+  const ConvLevel& g = tab.lev[cu.lev];
+  const int X = cu.X, Y = cu.Y, Z = cu.Z;
+  const int Ry = g.R[1], Rz = g.R[2];
+  const int nrow = 32 + 2 * Ry;
+  const int WX = XT + 2 * g.X0 + 4;
+  const int ny = g.ny;
+  const int4* __restrict__ rows = g.vrows2;
+  const float4* __restrict__ vtaps = reinterpret_cast<const float4*>(g.vtaps2);
+  const float* __restrict__ qpad = reinterpret_cast<const float*>(g.pad);
+  const float* __restrict__ Q = reinterpret_cast<const float*>(g.Q);
+
+  unsigned long long qr[ZP][XT];                      // (Q of plane 2k, Q of plane 2k + 1)
+#pragma unroll
+  for (int k = 0; k < ZP; ++k)
+#pragma unroll
+    for (int i = 0; i < XT; ++i) {
+      const int x = X + i, y = Y + lane, z = Z + 2 * k;
+      const bool in = x < g.M[0] && y < g.M[1];
+      const float lo = in && z < g.M[2] ? Q[((size_t)z * g.M[1] + y) * g.M[0] + x] : 0.f;
+      const float hi = in && z + 1 < g.M[2] ? Q[((size_t)(z + 1) * g.M[1] + y) * g.M[0] + x] : 0.f;
+      qr[k][i] = pack2(lo, hi);
+    }
+  double S[6] = {0, 0, 0, 0, 0, 0};
+
+  const int p0 = g.vb[cu.slice], p1 = g.vb[cu.slice + 1];
+  for (int zr = p0; zr < p1; ++zr) {                  // input plane z = Z + zr, only dz >= 0
+    stage_plane<float>(g, qpad, plane, Z + zr + Rz, X, Y, nrow, WX, lane);
+    for (int dy = -Ry; dy <= Ry; ++dy) {
+      int4 re[ZP];
+      int cl = 1 << 30, ch = -1;
+#pragma unroll
+      for (int k = 0; k < ZP; ++k) {
+        const int d = zr - 2 * k;                     // planes (2k, 2k+1) take rows (d, d - 1)
+        if (d >= 0 && d <= Rz + 1) re[k] = __ldg(rows + d * ny + (dy + Ry));
+        else re[k] = make_int4(0, 1, 0, 0);
+        if (re[k].y <= re[k].z) { cl = min(cl, re[k].y); ch = max(ch, re[k].z); }
+      }
+      if (ch < cl) continue;
+      unsigned long long e0[ZP], e1[ZP], e2[ZP];
+#pragma unroll
+      for (int k = 0; k < ZP; ++k) { e0[k] = 0ull; e1[k] = 0ull; e2[k] = 0ull; }
+      const float* srow = plane + (lane + dy + Ry) * g.pitch;
+      for (int c = cl; c <= ch; ++c) {
+        float win[XT + 4];
+#pragma unroll
+        for (int j = 0; j < XT + 4; j += 4) {
+          const float4 t = *reinterpret_cast<const float4*>(srow + 4 * c + j);
+          win[j] = t.x; win[j + 1] = t.y; win[j + 2] = t.z; win[j + 3] = t.w;
+        }
+#pragma unroll
+        for (int k = 0; k < ZP; ++k) {
+          if (c >= re[k].y && c <= re[k].z) {
+            const float4* tp = vtaps + (size_t)(re[k].x + c - re[k].y) * 6;
+            float4 gq[6];
+#pragma unroll
+            for (int m = 0; m < 6; ++m) gq[m] = __ldg(tp + m);
+#pragma unroll
+            for (int t = 0; t < 4; ++t) {
+              unsigned long long c0 = 0ull, c1 = 0ull;
+#pragma unroll
+              for (int i = 0; i < XT; i += 2) {
+                ffma2_bcast(c0, win[i + t], qr[k][i]);
+                ffma2_bcast(c1, win[i + 1 + t], qr[k][i + 1]);
+              }
+              const unsigned long long ct = fadd2_pp(c0, c1);
+              // taps of moment m, tap t: floats (2t, 2t+1) of quads 2m, 2m+1
+              const float4 a0 = gq[t >> 1], a1 = gq[2 + (t >> 1)], a2 = gq[4 + (t >> 1)];
+              const bool up = (t & 1) != 0;
+              ffma2_pp(e0[k], up ? pack2(a0.z, a0.w) : pack2(a0.x, a0.y), ct);
+              ffma2_pp(e1[k], up ? pack2(a1.z, a1.w) : pack2(a1.x, a1.y), ct);
+              ffma2_pp(e2[k], up ? pack2(a2.z, a2.w) : pack2(a2.x, a2.y), ct);
+            }
+          }
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < ZP; ++k) {
+        float e0l, e0h, e1l, e1h, e2l, e2h;
+        unpack2(e0[k], e0l, e0h); unpack2(e1[k], e1l, e1h); unpack2(e2[k], e2l, e2h);
+        const double fy = (double)dy;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {                 // lower half: plane 2k (dz = d), upper: 2k+1 (dz = d - 1)
+          const double fz = (double)(zr - 2 * k - h);
+          const double d0 = (double)(h ? e0h : e0l), d1 = (double)(h ? e1h : e1l);
+          S[0] += (double)(h ? e2h : e2l);
+          S[1] = fma(fy * fy, d0, S[1]);
+          S[2] = fma(fz * fz, d0, S[2]);
+          S[3] = fma(fy, d1, S[3]);
+          S[4] = fma(fz, d1, S[4]);
+          S[5] = fma(fy * fz, d0, S[5]);
+        }
       }
     }
   }

@@ -134,6 +134,8 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   g.vtaps = upload(p, tv);
   g.rows2 = nullptr;
   g.taps2 = nullptr;
+  g.vrows2 = nullptr;
+  g.vtaps2 = nullptr;
   if (p->fp32) {
     // packed path (k_conv_f2): stencil rows d and d - 1 merged, taps interleaved per tap
     auto row_rx = [&](int dz, int dy) {               // x half-width of row (dz, dy), -1 if empty
@@ -162,6 +164,41 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
             t2.push_back(rb >= 0 && dx >= -rb && dx <= rb ? st.at(st.s, dx, dy, d - 1) : 0.0);
           }
       }
+    // virial, packed: half-space rows d and d - 1 merged, per chunk 24 floats (2g, 2g dx, 2g dx^2)
+    // x 4 taps x (row d, row d - 1)
+    auto vrange = [&](int dz, int dy, int& xlo, int& xhi) {          // taps of half-space row (dz, dy)
+      if (dz < 0 || dz > Rz) return false;
+      const int Rx = row_rx(dz, dy);
+      const bool whole = dz > 0 || dy > 0, centre = dz == 0 && dy == 0;
+      if (Rx < 0 || !(whole || centre) || (centre && Rx < 1)) return false;
+      xlo = centre ? 1 : -Rx; xhi = Rx;
+      return true;
+    };
+    std::vector<int4> vr2((size_t)ny * (Rz + 2));
+    std::vector<double> tv2;
+    for (int d = 0; d <= Rz + 1; ++d)
+      for (int dy = -st.R[1]; dy <= st.R[1]; ++dy) {
+        int alo = 0, ahi = -1, blo = 0, bhi = -1;
+        const bool ha = vrange(d, dy, alo, ahi), hb = vrange(d - 1, dy, blo, bhi);
+        int4& r = vr2[(size_t)d * ny + (dy + st.R[1])];
+        if (!ha && !hb) { r = make_int4(0, 1, 0, 0); continue; }
+        const int xlo = ha && hb ? std::min(alo, blo) : (ha ? alo : blo);
+        const int xhi = ha && hb ? std::max(ahi, bhi) : (ha ? ahi : bhi);
+        const int clo = (xlo + g.X0) / 4, chi = (xhi + g.X0) / 4;
+        r = make_int4((int)(tv2.size() / 24), clo, chi, 0);
+        for (int c = clo; c <= chi; ++c)
+          for (int m = 0; m < 3; ++m)
+            for (int t = 0; t < 4; ++t) {
+              const int dx = 4 * c - g.X0 + t;
+              const double ga = ha && dx >= alo && dx <= ahi ? 2.0 * st.at(st.g, dx, dy, d) : 0.0;
+              const double gb = hb && dx >= blo && dx <= bhi ? 2.0 * st.at(st.g, dx, dy, d - 1) : 0.0;
+              const double f = m == 0 ? 1.0 : m == 1 ? (double)dx : (double)dx * dx;
+              tv2.push_back(ga * f);
+              tv2.push_back(gb * f);
+            }
+      }
+    g.vrows2 = up_rows(vr2);
+    g.vtaps2 = upload(p, tv2);
     g.rows2 = up_rows(r2);
     g.taps2 = (const char*)upload(p, t2) + 8 * p->esz;   // chunk 0 of the table follows the guard chunk
   }
@@ -303,7 +340,10 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
       ntiles *= p->at.nt[ax];
       if (mp.periodic[ax] && H.lev[1].M[ax] < p->at.D[ax]) p->anterp_tiled = false;
     }
-    if (ntiles < 1024) p->anterp_tiled = false;
+    {
+      const char* e = std::getenv("MSM_ANTERP_MIN_TILES");
+      if (ntiles < (e ? std::atoi(e) : 128)) p->anterp_tiled = false;
+    }
     if (const char* e = std::getenv("MSM_ANTERP_TILED")) p->anterp_tiled = p->anterp_tiled && std::atoi(e) != 0;
     if (p->anterp_tiled)
       p->anterp_scratch = dev_alloc(p, (size_t)ntiles * p->at.D[0] * p->at.D[1] * p->at.D[2] * p->esz);
@@ -336,7 +376,7 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   p->grec = dev_alloc(p, cap * 4 * p->esz);
   p->Fsr = dev_alloc(p, (size_t)kPairMaxSplit * cap * 3 * p->esz);   // per-split partials of the pair kernel
   p->Vsr = dev_alloc(p, (size_t)kPairMaxSplit * cap * p->esz);
-  p->pair_ymax = (int)((cap / 32 + p->pair_rows) / p->pair_rows + 3) / 4 + 1;
+  p->pair_ymax = (int)((cap / 32 + p->pair_rows) / p->pair_rows + kPairWarps - 1) / kPairWarps + 1;
   p->pair_wpart = (double*)dev_alloc(p, (size_t)p->pair_rows * p->pair_ymax * kPairMaxSplit * kPairWarps * 6 * sizeof(double));
   p->n_eblocks = (int)((cap + 127) / 128);
   p->epart = (double*)dev_alloc(p, (size_t)p->n_eblocks * sizeof(double));

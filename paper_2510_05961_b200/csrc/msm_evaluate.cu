@@ -266,10 +266,17 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     }
     mark();
     if (want_virial) {
-      auto kern = k_conv_virial<T, XT, ZT>;
-      if (p->conv_smem > 48 * 1024)
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
-      MSM_LAUNCH(p, (kern<<<p->conv.total_vunits, 32, p->conv_smem, st>>>(p->d_conv)));
+      if constexpr (sizeof(T) == 4) {
+        auto kern = k_conv_virial_f2<XT>;             // packed FMAs (FFMA2)
+        if (p->conv_smem > 48 * 1024)
+          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
+        MSM_LAUNCH(p, (kern<<<p->conv.total_vunits, 32, p->conv_smem, st>>>(p->d_conv)));
+      } else {
+        auto kern = k_conv_virial<T, XT, ZT>;
+        if (p->conv_smem > 48 * 1024)
+          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
+        MSM_LAUNCH(p, (kern<<<p->conv.total_vunits, 32, p->conv_smem, st>>>(p->d_conv)));
+      }
       for (int l = 1; l < p->n_t; ++l) {
         const ConvLevel& g = p->conv.lev[l - 1];
         const Level& lv = H.lev[l];

@@ -43,7 +43,7 @@ template <typename T> struct PairParams {
   size_t part_stride;     // elements between the per-split partial outputs (capacity)
 };
 
-constexpr int kPairWarps = 4;
+constexpr int kPairWarps = 1;
 constexpr int kPairMaxSplit = 5;
 
 template <typename T> struct PairStage;       // shared-memory staging of one warp
