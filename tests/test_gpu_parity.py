@@ -280,3 +280,81 @@ def test_graph_replay_matches_direct_launches():
         U, W = plan.evaluate(pos, q, F, V)
     st = plan.stage_times()
     assert U == U2 and all(v >= 0 for v in st.values()) and 0.0 < sum(st.values()) < 50.0
+
+
+def _custom(name, pos, q, box, periodic, h, a, p, levels, precision="fp64"):
+    from paper_2510_05961_b200.workloads import Workload
+    return Workload(name, np.asarray(pos, dtype=np.float64), np.asarray(q, dtype=np.float64), tuple(box),
+                    tuple(periodic), h=h, a=a, p=p, levels=levels).as_precision(precision)
+
+
+@pytest.mark.parametrize("periodic,box,p,precision", [
+    ((0, 0, 0), (61.0, 37.0, 45.0), 4, "fp64"),      # open, partial anterpolation tiles on every axis
+    ((0, 0, 0), (61.0, 37.0, 45.0), 6, "fp64"),
+    ((1, 1, 0), (32.0, 32.0, 45.0), 4, "fp64"),      # slab
+    ((1, 1, 1), (40.0, 24.0, 32.0), 4, "fp64"),      # periodic, non-cubic box (unequal spacings)
+    ((1, 1, 1), (40.0, 24.0, 32.0), 4, "fp32"),
+    ((0, 0, 0), (61.0, 37.0, 45.0), 4, "fp32"),
+])
+def test_tiled_anterpolation_shapes(periodic, box, p, precision):
+    """Grids large enough for the tiled anterpolation kernel (>= 128 tiles), with partial tiles,
+    open faces and unequal periodic spacings."""
+    rng = np.random.default_rng(77)
+    n = 3001
+    pos = rng.random((n, 3)) * np.array(box)
+    q = rng.uniform(-1, 1, n); q -= q.mean()
+    levels = 3 if all(periodic) else 4                # open axes: keep the dense top grid under 4096 points
+    w = _custom(f"tiled_{''.join(map(str, periodic))}_p{p}_{precision}", pos, q, box, periodic, 1.0, 4.0, p, levels,
+                precision)
+    from paper_2510_05961_b200 import msm
+    gpu = run_gpu(w, precision=precision)
+    ref = run_oracle(w)
+    _log(w.name, compare(w, gpu, ref, precision))
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_clustered_particles(precision):
+    """A dense blob in a large periodic box: cells with > 100 particles (several candidate batches
+    per neighbour row, many tiles per cell row) next to empty cells."""
+    rng = np.random.default_rng(5)
+    n = 3000
+    box = (48.0, 48.0, 48.0)
+    pos = 24.0 + rng.normal(0.0, 3.0, (n, 3))
+    pos = np.mod(pos, 48.0)
+    q = rng.uniform(-1, 1, n); q -= q.mean()
+    w = _custom(f"blob_{precision}", pos, q, box, (1, 1, 1), 1.5, 6.0, 4, 2, precision)
+    gpu = run_gpu(w, precision=precision)
+    ref = run_oracle(w)
+    errs = compare(w, gpu, ref, precision)
+    _log(w.name, errs)
+
+
+def test_sparse_particles_long_tiles():
+    """Very few particles in a large periodic box: one tile spans a whole row of cells, so the pair
+    kernel must cut it into sub-tiles whose neighbourhoods do not wrap onto themselves."""
+    rng = np.random.default_rng(11)
+    n = 24
+    box = (40.0, 40.0, 40.0)                       # 16 pair cells per row; one tile holds the whole row
+    pos = rng.random((n, 3)) * np.array(box)
+    pos[:, 1] = 10.0 + 0.5 * rng.random(n)        # all in one (y, z) row of cells
+    pos[:, 2] = 10.0 + 0.5 * rng.random(n)
+    q = np.where(np.arange(n) % 2 == 0, 1.0, -1.0)
+    w = _custom("sparse_row", pos, q, box, (1, 1, 1), 2.5, 5.0, 4, 2)
+    gpu = run_gpu(w)
+    ref = run_oracle(w)
+    _log(w.name, compare(w, gpu, ref, "fp64"))
+
+
+def test_tiny_periodic_box_minimum_image():
+    """Fewer than five pair cells per axis: the explicit minimum-image instance of the pair kernel,
+    with the neighbourhood planes split over blocks."""
+    rng = np.random.default_rng(13)
+    n = 257
+    box = (13.0, 11.0, 12.5)
+    pos = rng.random((n, 3)) * np.array(box)
+    q = rng.uniform(-1, 1, n); q -= q.mean()
+    for prec in ("fp64", "fp32"):
+        w = _custom(f"tinybox_{prec}", pos, q, box, (1, 1, 1), 1.5, 5.0, 4, 2, prec)
+        gpu = run_gpu(w, precision=prec)
+        ref = run_oracle(w)
+        _log(w.name, compare(w, gpu, ref, prec))
