@@ -102,7 +102,9 @@ msm_status_t msm_plan_info(const msm_plan_t *plan, msm_plan_info_t *info_out);
  * in one small copy).  From the second consecutive call with identical arguments on, the launch
  * sequence is captured into a CUDA graph and replayed on a plan-owned stream (a small system is
  * otherwise bound by its ~40-60 dependent kernel launches); results are bit-identical either way.
- * MSM_NO_GRAPH=1 in the environment at plan creation disables this.
+ * MSM_NO_GRAPH=1 in the environment at plan creation disables this.  The short-range pair kernel
+ * runs on a second plan-owned stream beside the grid pipeline and joins before the interpolation
+ * (not while per-stage profiling is on; MSM_NO_OVERLAP=1 disables it).
  * Neutrality is assumed on periodic axes: the single-point top level contributes zero (reading
  * T2), which for a non-neutral input is the neutralising-background convention. */
 msm_status_t msm_evaluate(msm_plan_t *plan, int n, const void *d_positions, const void *d_charges,

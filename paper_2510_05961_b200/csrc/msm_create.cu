@@ -397,6 +397,11 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
       cudaEventCreateWithFlags(&p->gev, cudaEventDisableTiming) != cudaSuccess)
     return MSM_ERR_CUDA;
   if (const char* e = std::getenv("MSM_NO_GRAPH")) p->graph_enabled = std::atoi(e) == 0;
+  if (cudaStreamCreateWithFlags(&p->pstream, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->fork_ev, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->join_ev, cudaEventDisableTiming) != cudaSuccess)
+    return MSM_ERR_CUDA;
+  if (const char* e = std::getenv("MSM_NO_OVERLAP")) p->overlap = std::atoi(e) == 0;
   // stage list of msm_evaluate, in launch order
   for (const char* s : {"sort", "pair", "anterpolate", "restrict"}) p->stage_name_store.push_back(s);
   for (const char* s : {"filter", "conv", "conv_virial"}) p->stage_name_store.push_back(s);
@@ -413,6 +418,9 @@ extern "C" {
 void msm_plan_destroy(msm_plan_t* p) {
   if (!p) return;
   for (void* d : p->allocs) cudaFree(d);
+  if (p->pstream) cudaStreamDestroy(p->pstream);
+  if (p->fork_ev) cudaEventDestroy(p->fork_ev);
+  if (p->join_ev) cudaEventDestroy(p->join_ev);
   if (p->gexec) cudaGraphExecDestroy(p->gexec);
   if (p->gstream) cudaStreamDestroy(p->gstream);
   if (p->gev) cudaEventDestroy(p->gev);

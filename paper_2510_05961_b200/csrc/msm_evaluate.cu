@@ -133,6 +133,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   mark();
 
   // ---------------- S2 pair
+  bool forked = false;
   {
     PairParams<T> pp;
     bool any_minimg = false;
@@ -168,11 +169,23 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
                      pp.nsplit);
     p->pair_blocks = (int)(pgrid.x * pgrid.y * pgrid.z);
     const bool mi = pp.minimg[0] || pp.minimg[1] || pp.minimg[2];
-#define MSM_PAIR(V, M) MSM_LAUNCH(p, (k_pair<T, P, V, M><<<pgrid, kPairWarps * 32, 0, st>>>(           \
+    // The pair sum does not depend on the grid pipeline (S3..S7): it runs on the plan's second
+    // stream beside it and joins before the interpolation, so that the two latency-bound halves of
+    // the evaluation fill each other's idle issue slots. With per-stage profiling on, everything
+    // stays on one stream (the stage times would otherwise overlap).
+    cudaStream_t ps = st;
+    if (p->overlap && !p->profiling && p->pstream) {
+      cudaEventRecord(p->fork_ev, st);
+      cudaStreamWaitEvent(p->pstream, p->fork_ev, 0);
+      ps = p->pstream;
+    }
+#define MSM_PAIR(V, M) MSM_LAUNCH(p, (k_pair<T, P, V, M><<<pgrid, kPairWarps * 32, 0, ps>>>(           \
     pp, p->pstart, (const V4*)p->prec, p->pcellx, p->porder, (T*)p->Fsr, (T*)p->Vsr, p->pair_wpart)))
     if (want_virial) { if (mi) MSM_PAIR(true, true); else MSM_PAIR(true, false); }
     else { if (mi) MSM_PAIR(false, true); else MSM_PAIR(false, false); }
 #undef MSM_PAIR
+    if (ps != st) cudaEventRecord(p->join_ev, ps);
+    forked = ps != st;
   }
   mark();
 
@@ -336,6 +349,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   mark();
 
   // ---------------- S8 interpolation + outputs
+  if (forked) cudaStreamWaitEvent(st, p->join_ev, 0);
   const int neb = (int)blocks_for(n, 128);
   MSM_LAUNCH(p, (k_interpolate<T, P><<<neb, 128, 0, st>>>(
                     n, p->pair_nsplit, (size_t)p->cap, gg, tab, (T)(1.0 / H.lev[1].h[0]), (T)(1.0 / H.lev[1].h[1]), (T)(1.0 / H.lev[1].h[2]),

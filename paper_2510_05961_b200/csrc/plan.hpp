@@ -92,6 +92,11 @@ struct msm_plan {
   cudaGraphExec_t gexec = nullptr;
   cudaEvent_t gev = nullptr;
 
+  // second stream for the pair kernel (runs beside the grid pipeline)
+  bool overlap = true;
+  cudaStream_t pstream = nullptr;
+  cudaEvent_t fork_ev = nullptr, join_ev = nullptr;
+
   // profiling
   bool profiling = false;
   cudaEvent_t ev[msm::kMaxStages + 1]{};
