@@ -399,7 +399,10 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   if (const char* e = std::getenv("MSM_NO_GRAPH")) p->graph_enabled = std::atoi(e) == 0;
   if (cudaStreamCreateWithFlags(&p->pstream, cudaStreamNonBlocking) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->fork_ev, cudaEventDisableTiming) != cudaSuccess ||
-      cudaEventCreateWithFlags(&p->join_ev, cudaEventDisableTiming) != cudaSuccess)
+      cudaEventCreateWithFlags(&p->join_ev, cudaEventDisableTiming) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&p->vstream, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->fork2_ev, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->join2_ev, cudaEventDisableTiming) != cudaSuccess)
     return MSM_ERR_CUDA;
   if (const char* e = std::getenv("MSM_NO_OVERLAP")) p->overlap = std::atoi(e) == 0;
   // stage list of msm_evaluate, in launch order
@@ -419,6 +422,9 @@ void msm_plan_destroy(msm_plan_t* p) {
   if (!p) return;
   for (void* d : p->allocs) cudaFree(d);
   if (p->pstream) cudaStreamDestroy(p->pstream);
+  if (p->vstream) cudaStreamDestroy(p->vstream);
+  if (p->fork2_ev) cudaEventDestroy(p->fork2_ev);
+  if (p->join2_ev) cudaEventDestroy(p->join2_ev);
   if (p->fork_ev) cudaEventDestroy(p->fork_ev);
   if (p->join_ev) cudaEventDestroy(p->join_ev);
   if (p->gexec) cudaGraphExecDestroy(p->gexec);

@@ -133,7 +133,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   mark();
 
   // ---------------- S2 pair
-  bool forked = false;
+  bool forked = false, forked_v = false;
   {
     PairParams<T> pp;
     bool any_minimg = false;
@@ -256,6 +256,28 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   mark();
   if (p->conv.nlev > 0) {
     constexpr int XT = sizeof(T) == 4 ? 16 : 8, ZT = 4;
+    auto launch_virial = [&](cudaStream_t vs) {
+      if constexpr (sizeof(T) == 4) {
+        auto kern = k_conv_virial_f2<XT>;             // packed FMAs (FFMA2)
+        if (p->conv_smem > 48 * 1024)
+          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
+        MSM_LAUNCH(p, (kern<<<p->conv.total_vunits, 32, p->conv_smem, vs>>>(p->d_conv)));
+      } else {
+        auto kern = k_conv_virial<T, XT, ZT>;
+        if (p->conv_smem > 48 * 1024)
+          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
+        MSM_LAUNCH(p, (kern<<<p->conv.total_vunits, 32, p->conv_smem, vs>>>(p->d_conv)));
+      }
+    };
+    // the virial correlation only needs the filtered grid charge: it runs on a third stream beside
+    // the potential convolution (not with per-stage profiling on) and joins before the reductions
+    if (want_virial && p->overlap && !p->profiling && p->vstream) {
+      cudaEventRecord(p->fork2_ev, st);
+      cudaStreamWaitEvent(p->vstream, p->fork2_ev, 0);
+      launch_virial(p->vstream);
+      cudaEventRecord(p->join2_ev, p->vstream);
+      forked_v = true;
+    }
     {
       if constexpr (sizeof(T) == 4) {
         auto kern = k_conv_f2<XT>;                    // packed FMAs (FFMA2)
@@ -279,17 +301,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     }
     mark();
     if (want_virial) {
-      if constexpr (sizeof(T) == 4) {
-        auto kern = k_conv_virial_f2<XT>;             // packed FMAs (FFMA2)
-        if (p->conv_smem > 48 * 1024)
-          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
-        MSM_LAUNCH(p, (kern<<<p->conv.total_vunits, 32, p->conv_smem, st>>>(p->d_conv)));
-      } else {
-        auto kern = k_conv_virial<T, XT, ZT>;
-        if (p->conv_smem > 48 * 1024)
-          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
-        MSM_LAUNCH(p, (kern<<<p->conv.total_vunits, 32, p->conv_smem, st>>>(p->d_conv)));
-      }
+      if (!forked_v) launch_virial(st);
       for (int l = 1; l < p->n_t; ++l) {
         const ConvLevel& g = p->conv.lev[l - 1];
         const Level& lv = H.lev[l];
@@ -376,6 +388,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   }
   fa.nblk = nblk;
   if (nblk > p->part_blocks) return MSM_ERR_CUDA;   // sized at plan creation; cannot happen
+  if (forked_v) cudaStreamWaitEvent(st, p->join2_ev, 0);
   if (nblk > 0) MSM_LAUNCH(p, (k_partial_sums<<<nblk, 256, 0, st>>>(fa, p->part)));
   MSM_LAUNCH(p, (k_finalize<<<1, 256, 0, st>>>(nblk, p->part, p->flag, p->results)));
   mark();

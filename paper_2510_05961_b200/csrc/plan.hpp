@@ -94,8 +94,8 @@ struct msm_plan {
 
   // second stream for the pair kernel (runs beside the grid pipeline)
   bool overlap = true;
-  cudaStream_t pstream = nullptr;
-  cudaEvent_t fork_ev = nullptr, join_ev = nullptr;
+  cudaStream_t pstream = nullptr, vstream = nullptr;
+  cudaEvent_t fork_ev = nullptr, join_ev = nullptr, fork2_ev = nullptr, join2_ev = nullptr;
 
   // profiling
   bool profiling = false;
