@@ -1,5 +1,5 @@
-// gridops.cuh -- S4 restriction and S7 prolongation (Eq. 19, separable, one axis at a
-// time), and the omega' pre-filter that writes the haloed (padded) copy of a level's grid
+// gridops.cuh -- S4 restriction (Eq. 19 line 1, separable, one axis at a time; the
+// prolongation is in gridops_fused.cuh), and the omega' pre-filter that writes the haloed (padded) copy of a level's grid
 // charge which the stencil convolution reads (Eq. 20's omega' factors moved from the stencil to the
 // grid charge: K * q = s * (omega' (x) omega' (x) omega' * q)).
 //
@@ -108,39 +108,6 @@ __global__ void k_restrict_axis(AxisDims d, int lo_in, int lo_out, AxisTaps<T> J
     for (int k = klo; k <= khi; ++k) acc = fma(J.c[k], line[(size_t)(i0 + k) * p.stride], acc);
   }
   out[t] = acc;
-}
-
-// out[i] (+)= sum_n J_n in[m], 2(m + lo_in) + n = i + lo_out   (prolongation = exact transpose)
-template <typename T, bool ADD>
-__global__ void k_prolong_axis(AxisDims d, int lo_in, int lo_out, AxisTaps<T> J, const T* __restrict__ in,
-                               T* __restrict__ out) {
-  const AxisPos p = axis_pos(d);
-  if (!p.valid) return;
-  const size_t t = p.t;
-  const int i = p.c[d.axis], Mi = d.in[d.axis], Mo = d.out[d.axis], hw = J.n / 2;
-  const T* line = in + p.base;
-  T acc = 0;
-  if (d.periodic && Mo == 1) {
-    acc = line[0];
-  } else if (d.periodic) {
-    // taps n with (i - n) even: n = n0, n0 + 2, ...; m = ((i - n) mod Mo) / 2 descends by one per tap
-    const int n0 = -hw + ((i + hw) & 1);
-    int m = imod(i - n0, Mo) >> 1;                 // Mo = 2 Mi
-    for (int n = n0; n <= hw; n += 2) {
-      acc = fma(J.c[n + hw], line[(size_t)m * p.stride], acc);
-      if (--m < 0) m += Mi;
-    }
-  } else {
-    const int v0 = i + lo_out;                     // 2 (m + lo_in) = v0 - n
-    const int n0 = -hw + ((v0 + hw) & 1);
-    for (int n = n0; n <= hw; n += 2) {
-      const int v = v0 - n;                        // even (possibly negative): exact halving
-      const int m = v / 2 - lo_in;
-      if (m < 0 || m >= Mi) continue;
-      acc = fma(J.c[n + hw], line[(size_t)m * p.stride], acc);
-    }
-  }
-  if (ADD) out[t] += acc; else out[t] = acc;
 }
 
 // S6: dense top-level operator e = T q, one warp per row; with VIRIAL also the six quadratic forms

@@ -4,6 +4,7 @@
 #include <cstring>
 
 #include "gridops.cuh"
+#include "gridops_fused.cuh"
 #include "pair.cuh"
 #include "particle_grid.cuh"
 #include "plan.hpp"
@@ -212,6 +213,12 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
 
   // ---------------- S4 restriction
   const AxisTaps<T> Jt = make_taps<T>(p->J), Wt = make_taps<T>(p->omega);
+  auto grid3 = [](const Level& lv) {
+    Grid3 g;
+    for (int ax = 0; ax < 3; ++ax) { g.M[ax] = lv.M[ax]; g.lo[ax] = lv.lo[ax]; }
+    return g;
+  };
+  const int per3[3] = {p->bg.periodic[0], p->bg.periodic[1], p->bg.periodic[2]};
   for (int l = 1; l < p->n_t; ++l) {
     const Level &f = H.lev[l], &c = H.lev[l + 1];
     const T* src = (const T*)p->lev[l].Q;
@@ -338,25 +345,12 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   // ---------------- S7 prolongation + accumulate, z then y then x
   for (int l = p->n_t - 1; l >= 1; --l) {
     const Level &f = H.lev[l], &c = H.lev[l + 1];
-    const T* src = (const T*)p->lev[l + 1].E;
-    int din[3] = {c.M[0], c.M[1], c.M[2]};
-    const int order[3] = {2, 1, 0};
-    for (int s3 = 0; s3 < 3; ++s3) {
-      const int ax = order[s3];
-      AxisDims d;
-      for (int k = 0; k < 3; ++k) { d.in[k] = din[k]; d.out[k] = din[k]; }
-      d.out[ax] = f.M[ax];
-      d.axis = ax; d.periodic = p->bg.periodic[ax];
-      if (s3 < 2) {
-        T* dst = (T*)(s3 == 0 ? p->tmpA : p->tmpB);
-        MSM_LAUNCH(p, (k_prolong_axis<T, false><<<axis_grid(d), axis_block(), 0, st>>>(d, c.lo[ax], f.lo[ax], Jt, src, dst)));
-        src = dst;
-      } else {
-        MSM_LAUNCH(p, (k_prolong_axis<T, true><<<axis_grid(d), axis_block(), 0, st>>>(d, c.lo[ax], f.lo[ax], Jt, src,
-                                                                                    (T*)p->lev[l].E)));
-      }
-      din[ax] = f.M[ax];
-    }
+    const size_t sm = prolong3_smem_elems(P) * sizeof(T);
+    auto kern = k_prolong3<T>;
+    if (sm > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    const dim3 grid((f.M[0] + kPTX - 1) / kPTX, (f.M[1] + kPTY - 1) / kPTY, (f.M[2] + kPTZ - 1) / kPTZ);
+    MSM_LAUNCH(p, (kern<<<grid, 256, sm, st>>>(grid3(f), grid3(c), per3[0], per3[1], per3[2], Jt,
+                                               (const T*)p->lev[l + 1].E, (T*)p->lev[l].E)));
   }
   mark();
 
