@@ -1,7 +1,7 @@
 // gridops.cuh -- S4 restriction (Eq. 19 line 1, separable, one axis at a time; the
-// prolongation is in gridops_fused.cuh), and the omega' pre-filter that writes the haloed (padded) copy of a level's grid
-// charge which the stencil convolution reads (Eq. 20's omega' factors moved from the stencil to the
-// grid charge: K * q = s * (omega' (x) omega' (x) omega' * q)).
+// prolongation is in gridops_fused.cuh), and the omega' pre-filter that writes the haloed (padded)
+// copy of a level's grid charge which the stencil convolution reads (Eq. 20's omega' factors moved
+// from the stencil to the grid charge: K * q = s * (omega' (x) omega' (x) omega' * q)).
 //
 // One thread per output element; x is the fastest index in every array, so each warp reads and
 // writes contiguous runs (the grids at config sizes are L2-resident).
