@@ -44,7 +44,7 @@ struct AxisPos {
   size_t base;     // offset of the input line's element 0 (working-axis coordinate 0)
   size_t stride;   // input stride along the working axis
 };
-__device__ __forceinline__ AxisPos axis_pos(const AxisDims& d) {
+template <int AXIS> __device__ __forceinline__ AxisPos axis_pos(const AxisDims& d) {
   AxisPos p;
   const unsigned t = blockIdx.x * kAxisThreads + threadIdx.x;
   const unsigned total = (unsigned)d.out[0] * (unsigned)d.out[1] * (unsigned)d.out[2];
@@ -54,22 +54,21 @@ __device__ __forceinline__ AxisPos axis_pos(const AxisDims& d) {
   p.c[0] = (int)(t - r * (unsigned)d.out[0]);
   p.c[2] = (int)(r / (unsigned)d.out[1]);
   p.c[1] = (int)(r - (unsigned)p.c[2] * (unsigned)d.out[1]);
-  int z[3] = {p.c[0], p.c[1], p.c[2]};
-  z[d.axis] = 0;
-  p.base = lin(d.in, z[0], z[1], z[2]);
-  p.stride = d.axis == 0 ? 1 : (d.axis == 1 ? (size_t)d.in[0] : (size_t)d.in[0] * d.in[1]);
+  // the working axis is a compile-time constant: no dynamically indexed local arrays
+  p.base = lin(d.in, AXIS == 0 ? 0 : p.c[0], AXIS == 1 ? 0 : p.c[1], AXIS == 2 ? 0 : p.c[2]);
+  p.stride = AXIS == 0 ? 1 : (AXIS == 1 ? (size_t)d.in[0] : (size_t)d.in[0] * d.in[1]);
   return p;
 }
 
 // out[o] = sum_k w[k] in_logical[o - H - k]: omega' filter that also lays down the halo.
 // Logical input index i: periodic -> in[i mod M]; open -> in[i] inside [0, M), else 0.
 // One thread per output; the wrapped index is carried along the taps (one modulo per thread).
-template <typename T>
+template <typename T, int AXIS>
 __global__ void k_pad_filter(AxisDims d, int H, AxisTaps<T> w, const T* __restrict__ in, T* __restrict__ out) {
-  const AxisPos p = axis_pos(d);
+  const AxisPos p = axis_pos<AXIS>(d);
   if (!p.valid) return;
   const size_t t = p.t;
-  const int g = p.c[d.axis] - H, M = d.in[d.axis], hw = w.n / 2;
+  const int g = p.c[AXIS] - H, M = d.in[AXIS], hw = w.n / 2;
   const T* line = in + p.base;
   T acc = 0;
   if (d.periodic) {
@@ -86,13 +85,13 @@ __global__ void k_pad_filter(AxisDims d, int H, AxisTaps<T> w, const T* __restri
 }
 
 // out[m] = sum_n J_n in[2(m + lo_out) + n - lo_in]   (restriction along one axis)
-template <typename T>
+template <typename T, int AXIS>
 __global__ void k_restrict_axis(AxisDims d, int lo_in, int lo_out, AxisTaps<T> J, const T* __restrict__ in,
                                 T* __restrict__ out) {
-  const AxisPos p = axis_pos(d);
+  const AxisPos p = axis_pos<AXIS>(d);
   if (!p.valid) return;
   const size_t t = p.t;
-  const int m = p.c[d.axis], M = d.in[d.axis], hw = J.n / 2;
+  const int m = p.c[AXIS], M = d.in[AXIS], hw = J.n / 2;
   const T* line = in + p.base;
   if (d.periodic && M == 1) { out[t] = line[0]; return; }
   T acc = 0;

@@ -229,7 +229,9 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
       d.out[ax] = c.M[ax];
       d.axis = ax; d.periodic = p->bg.periodic[ax];
       T* dst = ax == 2 ? (T*)p->lev[l + 1].Q : (T*)(ax == 0 ? p->tmpA : p->tmpB);
-      MSM_LAUNCH(p, (k_restrict_axis<T><<<axis_grid(d), axis_block(), 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
+      if (ax == 0) MSM_LAUNCH(p, (k_restrict_axis<T, 0><<<axis_grid(d), axis_block(), 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
+      else if (ax == 1) MSM_LAUNCH(p, (k_restrict_axis<T, 1><<<axis_grid(d), axis_block(), 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
+      else MSM_LAUNCH(p, (k_restrict_axis<T, 2><<<axis_grid(d), axis_block(), 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
       src = dst;
       din[ax] = c.M[ax];
     }
@@ -255,7 +257,9 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
       T* dst = ax == 2 ? (T*)d.pad : (T*)(ax == 0 ? p->tmpA : p->tmpB);
       // along the filtered axis the logical size is the grid's, not the (already padded) array's
       ad.in[ax] = lv.M[ax];
-      MSM_LAUNCH(p, (k_pad_filter<T><<<axis_grid(ad), axis_block(), 0, st>>>(ad, halo[ax], Wt, src, dst)));
+      if (ax == 0) MSM_LAUNCH(p, (k_pad_filter<T, 0><<<axis_grid(ad), axis_block(), 0, st>>>(ad, halo[ax], Wt, src, dst)));
+      else if (ax == 1) MSM_LAUNCH(p, (k_pad_filter<T, 1><<<axis_grid(ad), axis_block(), 0, st>>>(ad, halo[ax], Wt, src, dst)));
+      else MSM_LAUNCH(p, (k_pad_filter<T, 2><<<axis_grid(ad), axis_block(), 0, st>>>(ad, halo[ax], Wt, src, dst)));
       src = dst;
       din[ax] = g.P[ax];
     }
