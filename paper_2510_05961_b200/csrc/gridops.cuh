@@ -84,6 +84,59 @@ __global__ void k_pad_filter(AxisDims d, int H, AxisTaps<T> w, const T* __restri
   out[t] = acc;
 }
 
+// The same filter with the tap count NT known at compile time: one thread computes RUN consecutive
+// outputs along the working axis from NT + RUN - 1 loaded inputs (each input is read once per
+// thread instead of NT times by NT threads), taps as immediates/constant operands.
+constexpr int kFilterRun = 4;
+template <typename T, int AXIS, int NT>
+__global__ void __launch_bounds__(kAxisThreads)
+k_pad_filter_run(AxisDims d, int H, AxisTaps<T> w, const T* __restrict__ in, T* __restrict__ out) {
+  constexpr int RUN = kFilterRun, HW = NT / 2;
+  // thread grid: the output dims with the working axis divided by RUN
+  const unsigned na = ((unsigned)d.out[AXIS] + RUN - 1) / RUN;
+  const unsigned g0 = AXIS == 0 ? na : (unsigned)d.out[0], g1 = AXIS == 1 ? na : (unsigned)d.out[1],
+                 g2 = AXIS == 2 ? na : (unsigned)d.out[2];
+  const unsigned t = blockIdx.x * kAxisThreads + threadIdx.x;
+  if (t >= g0 * g1 * g2) return;
+  const unsigned r = t / g0;
+  int c[3] = {(int)(t - r * g0), 0, (int)(r / g1)};
+  c[1] = (int)(r - (unsigned)c[2] * g1);
+  const int o0 = c[AXIS] * RUN;                      // first output of this thread along the axis
+  const int M = d.in[AXIS];
+  const size_t istride = AXIS == 0 ? 1 : (AXIS == 1 ? (size_t)d.in[0] : (size_t)d.in[0] * d.in[1]);
+  const size_t ostride = AXIS == 0 ? 1 : (AXIS == 1 ? (size_t)d.out[0] : (size_t)d.out[0] * d.out[1]);
+  const T* line = in + lin(d.in, AXIS == 0 ? 0 : c[0], AXIS == 1 ? 0 : c[1], AXIS == 2 ? 0 : c[2]);
+  T* oline = out + lin(d.out, AXIS == 0 ? 0 : c[0], AXIS == 1 ? 0 : c[1], AXIS == 2 ? 0 : c[2]);
+  // inputs: logical indices g = o0 - H - HW ... o0 - H + HW + RUN - 1
+  T v[NT + RUN - 1];
+  int i = o0 - H - HW;
+  if (d.periodic) {
+    i = imod(i, M);
+#pragma unroll
+    for (int j = 0; j < NT + RUN - 1; ++j) {
+      v[j] = line[(size_t)i * istride];
+      if (++i >= M) i -= M;
+    }
+  } else {
+#pragma unroll
+    for (int j = 0; j < NT + RUN - 1; ++j, ++i) v[j] = (i >= 0 && i < M) ? line[(size_t)i * istride] : (T)0;
+  }
+  // output o0 + q reads logical o0 + q - H - k', k' = -HW..HW: v[q + HW - k'] with tap w.c[k' + HW]
+#pragma unroll
+  for (int q = 0; q < RUN; ++q) {
+    if (o0 + q >= d.out[AXIS]) break;
+    T acc = 0;
+#pragma unroll
+    for (int k = 0; k < NT; ++k) acc = fma(w.c[k], v[q + NT - 1 - k], acc);
+    oline[(size_t)(o0 + q) * ostride] = acc;
+  }
+}
+inline unsigned filter_run_grid(const AxisDims& d) {
+  size_t total = 1;
+  for (int k = 0; k < 3; ++k) total *= k == d.axis ? (size_t)(d.out[k] + kFilterRun - 1) / kFilterRun : (size_t)d.out[k];
+  return (unsigned)((total + kAxisThreads - 1) / kAxisThreads);
+}
+
 // out[m] = sum_n J_n in[2(m + lo_out) + n - lo_in]   (restriction along one axis)
 template <typename T, int AXIS>
 __global__ void k_restrict_axis(AxisDims d, int lo_in, int lo_out, AxisTaps<T> J, const T* __restrict__ in,

@@ -257,9 +257,18 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
       T* dst = ax == 2 ? (T*)d.pad : (T*)(ax == 0 ? p->tmpA : p->tmpB);
       // along the filtered axis the logical size is the grid's, not the (already padded) array's
       ad.in[ax] = lv.M[ax];
-      if (ax == 0) MSM_LAUNCH(p, (k_pad_filter<T, 0><<<axis_grid(ad), axis_block(), 0, st>>>(ad, halo[ax], Wt, src, dst)));
-      else if (ax == 1) MSM_LAUNCH(p, (k_pad_filter<T, 1><<<axis_grid(ad), axis_block(), 0, st>>>(ad, halo[ax], Wt, src, dst)));
-      else MSM_LAUNCH(p, (k_pad_filter<T, 2><<<axis_grid(ad), axis_block(), 0, st>>>(ad, halo[ax], Wt, src, dst)));
+#define MSM_FILTER_RUN(AX, NT) MSM_LAUNCH(p, (k_pad_filter_run<T, AX, NT><<<filter_run_grid(ad), axis_block(), 0, st>>>( \
+    ad, halo[ax], Wt, src, dst)))
+#define MSM_FILTER_AX(AX)                                                                                  \
+      switch (Wt.n) {                                                                                      \
+        case 11: MSM_FILTER_RUN(AX, 11); break;                                                            \
+        case 13: MSM_FILTER_RUN(AX, 13); break;                                                            \
+        case 15: MSM_FILTER_RUN(AX, 15); break;                                                            \
+        default: MSM_LAUNCH(p, (k_pad_filter<T, AX><<<axis_grid(ad), axis_block(), 0, st>>>(ad, halo[ax], Wt, src, dst))); \
+      }
+      if (ax == 0) { MSM_FILTER_AX(0) } else if (ax == 1) { MSM_FILTER_AX(1) } else { MSM_FILTER_AX(2) }
+#undef MSM_FILTER_AX
+#undef MSM_FILTER_RUN
       src = dst;
       din[ax] = g.P[ax];
     }
