@@ -162,6 +162,49 @@ __global__ void k_restrict_axis(AxisDims d, int lo_in, int lo_out, AxisTaps<T> J
   out[t] = acc;
 }
 
+// Restriction with the mask length NJ = p + 1 known at compile time: one thread computes RUN
+// consecutive coarse outputs along the working axis from 2 RUN + NJ - 2 loaded fine values.
+template <typename T, int AXIS, int NJ>
+__global__ void __launch_bounds__(kAxisThreads)
+k_restrict_axis_run(AxisDims d, int lo_in, int lo_out, AxisTaps<T> J, const T* __restrict__ in, T* __restrict__ out) {
+  constexpr int RUN = kFilterRun, HW = NJ / 2, NV = 2 * RUN + NJ - 2;
+  const unsigned na = ((unsigned)d.out[AXIS] + RUN - 1) / RUN;
+  const unsigned g0 = AXIS == 0 ? na : (unsigned)d.out[0], g1 = AXIS == 1 ? na : (unsigned)d.out[1],
+                 g2 = AXIS == 2 ? na : (unsigned)d.out[2];
+  const unsigned t = blockIdx.x * kAxisThreads + threadIdx.x;
+  if (t >= g0 * g1 * g2) return;
+  const unsigned r = t / g0;
+  int c[3] = {(int)(t - r * g0), 0, (int)(r / g1)};
+  c[1] = (int)(r - (unsigned)c[2] * g1);
+  const int m0 = c[AXIS] * RUN;
+  const int M = d.in[AXIS];
+  const size_t istride = AXIS == 0 ? 1 : (AXIS == 1 ? (size_t)d.in[0] : (size_t)d.in[0] * d.in[1]);
+  const size_t ostride = AXIS == 0 ? 1 : (AXIS == 1 ? (size_t)d.out[0] : (size_t)d.out[0] * d.out[1]);
+  const T* line = in + lin(d.in, AXIS == 0 ? 0 : c[0], AXIS == 1 ? 0 : c[1], AXIS == 2 ? 0 : c[2]);
+  T* oline = out + lin(d.out, AXIS == 0 ? 0 : c[0], AXIS == 1 ? 0 : c[1], AXIS == 2 ? 0 : c[2]);
+  T v[NV];
+  int i = 2 * (m0 + lo_out) - HW - lo_in;            // fine array index of tap -HW of output m0
+  if (d.periodic) {
+    i = imod(i, M);
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      v[j] = line[(size_t)i * istride];
+      if (++i >= M) i -= M;
+    }
+  } else {
+#pragma unroll
+    for (int j = 0; j < NV; ++j, ++i) v[j] = (i >= 0 && i < M) ? line[(size_t)i * istride] : (T)0;
+  }
+#pragma unroll
+  for (int q = 0; q < RUN; ++q) {
+    if (m0 + q >= d.out[AXIS]) break;
+    T acc = 0;
+#pragma unroll
+    for (int k = 0; k < NJ; ++k) acc = fma(J.c[k], v[2 * q + k], acc);
+    oline[(size_t)(m0 + q) * ostride] = acc;
+  }
+}
+
 // S6: dense top-level operator e = T q, one warp per row; with VIRIAL also the six quadratic forms
 // q_r (TD_k q)_r per row (summed later in fixed order).
 template <typename T, bool VIRIAL>

@@ -229,9 +229,17 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
       d.out[ax] = c.M[ax];
       d.axis = ax; d.periodic = p->bg.periodic[ax];
       T* dst = ax == 2 ? (T*)p->lev[l + 1].Q : (T*)(ax == 0 ? p->tmpA : p->tmpB);
-      if (ax == 0) MSM_LAUNCH(p, (k_restrict_axis<T, 0><<<axis_grid(d), axis_block(), 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
-      else if (ax == 1) MSM_LAUNCH(p, (k_restrict_axis<T, 1><<<axis_grid(d), axis_block(), 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
-      else MSM_LAUNCH(p, (k_restrict_axis<T, 2><<<axis_grid(d), axis_block(), 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
+      // (a periodic axis that is already down to one point is copied: only the generic kernel does that)
+      if (d.periodic && f.M[ax] == 1) {
+        if (ax == 0) MSM_LAUNCH(p, (k_restrict_axis<T, 0><<<axis_grid(d), axis_block(), 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
+        else if (ax == 1) MSM_LAUNCH(p, (k_restrict_axis<T, 1><<<axis_grid(d), axis_block(), 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
+        else MSM_LAUNCH(p, (k_restrict_axis<T, 2><<<axis_grid(d), axis_block(), 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
+      } else {
+        const unsigned rg = filter_run_grid(d);
+        if (ax == 0) MSM_LAUNCH(p, (k_restrict_axis_run<T, 0, P + 1><<<rg, axis_block(), 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
+        else if (ax == 1) MSM_LAUNCH(p, (k_restrict_axis_run<T, 1, P + 1><<<rg, axis_block(), 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
+        else MSM_LAUNCH(p, (k_restrict_axis_run<T, 2, P + 1><<<rg, axis_block(), 0, st>>>(d, f.lo[ax], c.lo[ax], Jt, src, dst)));
+      }
       src = dst;
       din[ax] = c.M[ax];
     }
