@@ -4,6 +4,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
 #include <new>
 
 #include "pair.cuh"
@@ -150,19 +151,27 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
     };
     std::vector<int4> r2((size_t)ny * (nz + 1));
     std::vector<double> t2(8, 0.0);                  // guard chunk in front of the table (index -1)
+    std::map<std::vector<double>, int> seen2, seenv2;
     for (int d = -Rz; d <= Rz + 1; ++d)
       for (int dy = -st.R[1]; dy <= st.R[1]; ++dy) {
         const int ra = row_rx(d, dy), rb = row_rx(d - 1, dy), Rx = std::max(ra, rb);
         int4& r = r2[(size_t)(d + Rz) * ny + (dy + st.R[1])];
         if (Rx < 0) { r = make_int4(0, 0, -1, 0); continue; }   // empty: clamps to chunk -1
         const int clo = (-Rx + g.X0) / 4, chi = (Rx + g.X0) / 4;
-        r = make_int4((int)(t2.size() / 8) - 1, clo, chi, 0);
+        std::vector<double> rowv;
         for (int c = clo; c <= chi; ++c)
           for (int t = 0; t < 4; ++t) {
             const int dx = 4 * c - g.X0 + t;
-            t2.push_back(ra >= 0 && dx >= -ra && dx <= ra ? st.at(st.s, dx, dy, d) : 0.0);
-            t2.push_back(rb >= 0 && dx >= -rb && dx <= rb ? st.at(st.s, dx, dy, d - 1) : 0.0);
+            rowv.push_back(ra >= 0 && dx >= -ra && dx <= ra ? st.at(st.s, dx, dy, d) : 0.0);
+            rowv.push_back(rb >= 0 && dx >= -rb && dx <= rb ? st.at(st.s, dx, dy, d - 1) : 0.0);
           }
+        // rows (d, dy) and (d, -dy) hold the same taps: stored once (half the table, better L1 reuse)
+        auto it = seen2.find(rowv);
+        if (it == seen2.end()) {
+          it = seen2.emplace(rowv, (int)(t2.size() / 8) - 1).first;
+          t2.insert(t2.end(), rowv.begin(), rowv.end());
+        }
+        r = make_int4(it->second, clo, chi, 0);
       }
     // virial, packed: half-space rows d and d - 1 merged, per chunk 24 floats (2g, 2g dx, 2g dx^2)
     // x 4 taps x (row d, row d - 1)
@@ -185,7 +194,7 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
         const int xlo = ha && hb ? std::min(alo, blo) : (ha ? alo : blo);
         const int xhi = ha && hb ? std::max(ahi, bhi) : (ha ? ahi : bhi);
         const int clo = (xlo + g.X0) / 4, chi = (xhi + g.X0) / 4;
-        r = make_int4((int)(tv2.size() / 24), clo, chi, 0);
+        std::vector<double> rowv;
         for (int c = clo; c <= chi; ++c)
           for (int m = 0; m < 3; ++m)
             for (int t = 0; t < 4; ++t) {
@@ -193,9 +202,15 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
               const double ga = ha && dx >= alo && dx <= ahi ? 2.0 * st.at(st.g, dx, dy, d) : 0.0;
               const double gb = hb && dx >= blo && dx <= bhi ? 2.0 * st.at(st.g, dx, dy, d - 1) : 0.0;
               const double f = m == 0 ? 1.0 : m == 1 ? (double)dx : (double)dx * dx;
-              tv2.push_back(ga * f);
-              tv2.push_back(gb * f);
+              rowv.push_back(ga * f);
+              rowv.push_back(gb * f);
             }
+        auto it = seenv2.find(rowv);
+        if (it == seenv2.end()) {
+          it = seenv2.emplace(rowv, (int)(tv2.size() / 24)).first;
+          tv2.insert(tv2.end(), rowv.begin(), rowv.end());
+        }
+        r = make_int4(it->second, clo, chi, 0);
       }
     g.vrows2 = up_rows(vr2);
     g.vtaps2 = upload(p, tv2);
