@@ -49,6 +49,8 @@ struct ConvLevel {
   const void* staps;          // s_l in 4-tap chunks
   const int4* rows2;          // fp32 packed path: per (d, dy), d = -R[2] .. R[2]+1, rows d and d-1 merged
   const void* taps2;          // per chunk 8 floats: (s_d[t], s_{d-1}[t]) for the chunk's 4 taps
+  int n_rows2, n_taps2q;      // entries of rows2; float4 quads of taps2 including the guard chunk in front
+  int sunit0;                 // first unit of this level in the shared-table launch (multiple of kConvSW)
   const void* vtaps;          // per chunk: 4 x 2g, 4 x 2g dx, 4 x 2g dx^2
   const int4* vrows2;         // fp32 packed virial: half-space rows d and d - 1 merged, d = 0 .. R[2]+1
   const void* vtaps2;         // per chunk 24 floats: for 2g, 2g dx, 2g dx^2: 4 taps x (row d, row d - 1)
@@ -58,9 +60,11 @@ struct ConvLevel {
   double* wpart;              // virial partials, 6 per unit
 };
 
+constexpr int kConvSW = 8;    // warps (units) per block of the shared-table convolution kernel
+
 struct ConvTable {
   int nlev;
-  int total_units, total_vunits;
+  int total_units, total_vunits, total_sunits;
   ConvLevel lev[kMaxConvLevels];
 };
 
@@ -253,23 +257,17 @@ __device__ __forceinline__ float4 ldg_pinned(const float4* p) {
   return v;
 }
 
-template <int XT>
-__global__ void __launch_bounds__(32, 16)
-k_conv_f2(const ConvTable* __restrict__ tabp) {
-  constexpr int ZT = 4, ZP = 2;                       // two pairs of output planes
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  float* plane = reinterpret_cast<float*>(smem_raw);
-  const ConvTable& tab = *tabp;
-  const int lane = threadIdx.x;
-  const ConvUnit cu = decode_unit<false, XT, ZT>(tab, blockIdx.x);
-  const ConvLevel& g = tab.lev[cu.lev];
+// One unit of the packed convolution. SM: the row and tap tables are in shared memory (plain loads)
+// instead of global memory (pinned read-only loads).
+template <int XT, bool SM>
+__device__ __forceinline__ void conv_f2_unit(const ConvLevel& g, const ConvUnit& cu, const int4* rows2,
+                                             const float4* taps2, float* plane, int lane) {
+  constexpr int ZP = 2;                               // two pairs of output planes
   const int X = cu.X, Y = cu.Y, Z = cu.Z;
   const int Ry = g.R[1], Rz = g.R[2];
   const int nrow = 32 + 2 * Ry;
   const int WX = XT + 2 * g.X0 + 4;
   const int ny = g.ny;
-  const int4* __restrict__ rows2 = g.rows2;
-  const float4* __restrict__ taps2 = reinterpret_cast<const float4*>(g.taps2);
   const float* __restrict__ qpad = reinterpret_cast<const float*>(g.pad);
 
   unsigned long long acc[ZP][XT];                     // (plane 2kp, plane 2kp + 1) of output x + i
@@ -288,7 +286,7 @@ k_conv_f2(const ConvTable* __restrict__ tabp) {
 #pragma unroll
       for (int k = 0; k < ZP; ++k) {
         const int d = zr - 2 * k;                     // planes (2k, 2k+1) take stencil rows (d, d - 1)
-        if (d >= -Rz && d <= Rz + 1) re[k] = __ldg(rows2 + (d + Rz) * ny + (dy + Ry));
+        if (d >= -Rz && d <= Rz + 1) re[k] = SM ? rows2[(d + Rz) * ny + (dy + Ry)] : __ldg(rows2 + (d + Rz) * ny + (dy + Ry));
         else re[k] = make_int4(0, 0, -1, 0);          // empty
         if (re[k].y <= re[k].z) { cl = min(cl, re[k].y); ch = max(ch, re[k].z); }
       }
@@ -308,8 +306,8 @@ k_conv_f2(const ConvTable* __restrict__ tabp) {
           // unconditional address (clamped into the row; an empty row reads the guard chunk in front
           // of the table), so the loads are not tied to the branch below
           const float4* tp = taps2 + (re[k].x + min(max(c, re[k].y), re[k].z) - re[k].y) * 2;
-          tq[k][0] = ldg_pinned(tp);
-          tq[k][1] = ldg_pinned(tp + 1);
+          tq[k][0] = SM ? tp[0] : ldg_pinned(tp);
+          tq[k][1] = SM ? tp[1] : ldg_pinned(tp + 1);
         }
 #pragma unroll
         for (int k = 0; k < ZP; ++k) {
@@ -348,6 +346,50 @@ k_conv_f2(const ConvTable* __restrict__ tabp) {
       }
     }
   }
+}
+
+
+template <int XT>
+__global__ void __launch_bounds__(32, 16)
+k_conv_f2(const ConvTable* __restrict__ tabp) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const ConvTable& tab = *tabp;
+  const ConvUnit cu = decode_unit<false, XT, 4>(tab, blockIdx.x);
+  const ConvLevel& g = tab.lev[cu.lev];
+  conv_f2_unit<XT, false>(g, cu, g.rows2, reinterpret_cast<const float4*>(g.taps2),
+                          reinterpret_cast<float*>(smem_raw), threadIdx.x);
+}
+
+// The same with the level's row and tap tables copied into shared memory once per block of kConvSW
+// warps (one unit each, all of one level): a tap quad then costs a fixed-latency shared load instead
+// of a global load that misses the L1 half of the time (30 % of the warp time of k_conv_f2).
+template <int XT>
+__global__ void __launch_bounds__(32 * kConvSW, 2)
+k_conv_f2s(const ConvTable* __restrict__ tabp, int plane_bytes) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const ConvTable& tab = *tabp;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int l = 0;
+#pragma unroll 1
+  for (int k = 1; k < tab.nlev; ++k)
+    if ((int)blockIdx.x * kConvSW >= tab.lev[k].sunit0) l = k;
+  const ConvLevel& g = tab.lev[l];
+  float4* staps = reinterpret_cast<float4*>(smem_raw);
+  int4* srows = reinterpret_cast<int4*>(staps + g.n_taps2q);
+  float* planes = reinterpret_cast<float*>(srows + g.n_rows2);
+  const float4* gt = reinterpret_cast<const float4*>(g.taps2) - 2;          // from the guard chunk on
+  for (int i = threadIdx.x; i < g.n_taps2q; i += 32 * kConvSW) staps[i] = __ldg(gt + i);
+  for (int i = threadIdx.x; i < g.n_rows2; i += 32 * kConvSW) srows[i] = __ldg(g.rows2 + i);
+  __syncthreads();
+  int r = (int)blockIdx.x * kConvSW + warp - g.sunit0;
+  if (r >= g.tiles[0] * g.tiles[1] * g.tiles[2] * g.nslices) return;         // padding unit
+  ConvUnit cu;
+  cu.lev = l; cu.local = r;
+  cu.slice = r % g.nslices; r /= g.nslices;
+  cu.X = (r % g.tiles[0]) * XT; r /= g.tiles[0];
+  cu.Y = (r % g.tiles[1]) * 32;
+  cu.Z = (r / g.tiles[1]) * 4;
+  conv_f2_unit<XT, true>(g, cu, srows, staps + 2, planes + (size_t)warp * (plane_bytes / 4), lane);
 }
 
 // E[i] = sum_s part[s][i], s ascending (fixed order)

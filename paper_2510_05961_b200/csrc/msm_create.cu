@@ -216,6 +216,8 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
     g.vtaps2 = upload(p, tv2);
     g.rows2 = up_rows(r2);
     g.taps2 = (const char*)upload(p, t2) + 8 * p->esz;   // chunk 0 of the table follows the guard chunk
+    g.n_rows2 = (int)r2.size();
+    g.n_taps2q = (int)(t2.size() / 4);
   }
   d.pad = dev_alloc(p, (size_t)g.P[0] * g.P[1] * g.P[2] * p->esz);
   g.pad = d.pad;
@@ -243,6 +245,10 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   balanced_bounds(wv, g.vslices, g.vb);
   g.unit0 = p->conv.total_units;
   g.vunit0 = p->conv.total_vunits;
+  g.sunit0 = p->conv.total_sunits;                       // blocks of kConvSW units never straddle two levels
+  p->conv.total_sunits += (tiles * g.nslices + kConvSW - 1) / kConvSW * kConvSW;
+  if (p->fp32)
+    p->conv_tables_smem = std::max(p->conv_tables_smem, (size_t)g.n_taps2q * 16 + (size_t)g.n_rows2 * 16);
   p->conv.total_units += tiles * g.nslices;
   p->conv.total_vunits += tiles * g.vslices;
   if (g.nslices > 1) {

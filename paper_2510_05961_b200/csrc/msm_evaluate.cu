@@ -308,10 +308,21 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     }
     {
       if constexpr (sizeof(T) == 4) {
-        auto kern = k_conv_f2<XT>;                    // packed FMAs (FFMA2)
-        if (p->conv_smem > 48 * 1024)
-          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
-        MSM_LAUNCH(p, (kern<<<p->conv.total_units, 32, p->conv_smem, st>>>(p->d_conv)));
+        // packed FMAs (FFMA2); the stencil tables go to shared memory when two blocks of kConvSW
+        // warps with their planes and tables fit on an SM
+        const size_t plane_b = (p->conv_smem + 15) / 16 * 16;
+        const size_t sm_s = p->conv_tables_smem + kConvSW * plane_b;
+        static const bool no_s = std::getenv("MSM_CONV_GLOBAL_TAPS") != nullptr;
+        if (!no_s && sm_s <= 110 * 1024 && p->conv.total_units >= 4096) {   // small jobs: the table copy does not pay
+          auto kern = k_conv_f2s<XT>;
+          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_s);
+          MSM_LAUNCH(p, (kern<<<p->conv.total_sunits / kConvSW, 32 * kConvSW, sm_s, st>>>(p->d_conv, (int)plane_b)));
+        } else {
+          auto kern = k_conv_f2<XT>;
+          if (p->conv_smem > 48 * 1024)
+            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
+          MSM_LAUNCH(p, (kern<<<p->conv.total_units, 32, p->conv_smem, st>>>(p->d_conv)));
+        }
       } else {
         auto kern = k_conv<T, XT, ZT>;
         if (p->conv_smem > 48 * 1024)
