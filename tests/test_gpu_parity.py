@@ -358,3 +358,60 @@ def test_tiny_periodic_box_minimum_image():
         gpu = run_gpu(w, precision=prec)
         ref = run_oracle(w)
         _log(w.name, compare(w, gpu, ref, prec))
+
+
+def test_non_default_stream_and_null_outputs():
+    """The call works on a caller-owned stream (fork/join to the plan's streams, graph replay) and
+    with any subset of the optional outputs; results are bit-identical."""
+    import torch
+    from paper_2510_05961_b200 import msm
+    w = small_workload("slab", 1203, seed=1303, p=4)
+    dev = torch.device("cuda", 0)
+    plan = msm.Plan.for_workload(w)
+    pos = torch.tensor(w.positions, device=dev); q = torch.tensor(w.charges, device=dev)
+    F = torch.zeros((w.n, 3), dtype=torch.float64, device=dev); V = torch.zeros(w.n, dtype=torch.float64, device=dev)
+    U0, W0 = plan.evaluate(pos, q, F, V)
+    F0, V0 = F.clone(), V.clone()
+    s = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(s):
+        for _ in range(3):
+            F.zero_(); V.zero_()
+            U, W = plan.evaluate(pos, q, F, V, stream=s)
+            assert U == U0 and np.array_equal(W, W0) and torch.equal(F, F0) and torch.equal(V, V0)
+    torch.cuda.synchronize()
+    # forces only, potentials only, energy only, no virial
+    F.zero_()
+    U, W = plan.evaluate(pos, q, F, None, want_energy=True, want_virial=False)
+    assert U == U0 and W is None and torch.equal(F, F0)
+    V.zero_()
+    U, W = plan.evaluate(pos, q, None, V, want_energy=False, want_virial=True)
+    assert U is None and np.array_equal(W, W0) and torch.equal(V, V0)
+
+
+def test_one_million_fp64_properties():
+    """Config 4's largest box in fp64 (capacity and indexing at 10^6 particles in the other
+    precision): U = 1/2 sum q V, grid charge = total charge, net force ~ 0 (MSM error), agreement with the
+    fp32 run of the same inputs within the fp32 tolerances."""
+    import torch
+    from paper_2510_05961_b200 import msm
+    from paper_2510_05961_b200.workloads import make_workload
+    w = make_workload("cfg4_water1m")
+    dev = torch.device("cuda", 0)
+    res = {}
+    for prec, dt in (("fp64", torch.float64), ("fp32", torch.float32)):
+        plan = msm.Plan.for_workload(w, prec)
+        pos = torch.tensor(w.positions, dtype=dt, device=dev); q = torch.tensor(w.charges, dtype=dt, device=dev)
+        F = torch.zeros((w.n, 3), dtype=dt, device=dev); V = torch.zeros(w.n, dtype=dt, device=dev)
+        U, W = plan.evaluate(pos, q, F, V)
+        res[prec] = (U, W, F.cpu().numpy().astype(np.float64), V.cpu().numpy().astype(np.float64))
+        if prec == "fp64":
+            assert abs(U - 0.5 * np.dot(w.charges, res[prec][3])) <= 1e-12 * abs(U)
+            assert abs(plan.debug_grid(1, "Q").sum() - w.charges.sum()) < 1e-8
+            # the grid breaks exact translation invariance, so the net force only vanishes to MSM error
+            assert np.abs(res[prec][2].sum(axis=0)).max() < 1e-5 * np.abs(res[prec][2]).sum(axis=0).max()
+        plan.close()
+    U64, W64, F64, V64 = res["fp64"]
+    U32, W32, F32, V32 = res["fp32"]
+    assert abs(U32 - U64) <= 1e-5 * abs(U64)
+    assert np.sqrt(np.mean((F32 - F64) ** 2)) <= 1e-4 * np.sqrt(np.mean(F64 ** 2))
+    assert np.abs(W32 - W64).max() <= 1e-3 * max(np.abs(W64).max(), abs(U64))
