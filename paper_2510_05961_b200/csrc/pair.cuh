@@ -71,7 +71,16 @@ __device__ __forceinline__ float rsqrt_fast(float x) {
   asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-__device__ __forceinline__ double rsqrt_fast(double x) { return 1.0 / sqrt(x); }
+// fp64: fp32 hardware seed (relative error 2^-22.9) + two Newton steps y <- y (3/2 - x/2 y^2), each of
+// which squares the error: ~1e-13, then below the fp64 rounding unit. x is a squared distance inside
+// the cutoff (far from the fp32 range limits).
+__device__ __forceinline__ double rsqrt_fast(double x) {
+  double y = (double)rsqrt_fast((float)x);
+  const double hx = 0.5 * x;
+  y = y * fma(-hx, y * y, 1.5);
+  y = y * fma(-hx, y * y, 1.5);
+  return y;
+}
 
 template <typename T, int P, bool VIRIAL, bool MI>
 __global__ void __launch_bounds__(kPairWarps * 32)
