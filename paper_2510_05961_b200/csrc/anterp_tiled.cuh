@@ -6,11 +6,12 @@
 // each particle's p^3 contributions q_i phi_m(r_i) to its private (T+p-1)^3 node grid in shared
 // memory: lane t handles nodes t, t+32, ... of the p^3 block, so one particle's targets are all
 // distinct, and particles are processed one after the other, so every node sees its additions in a
-// fixed order. When p divides 32 every lane's nodes keep the same (jx, jy) and a fixed set of jz, so
-// the lane holds the spline pieces of its own rows in registers and evaluates its weights itself
-// (no shuffles: the shared-memory/shuffle pipe is the bottleneck of this kernel); otherwise the 3p
-// one-dimensional weights are evaluated once per particle (lane k < 3p evaluates weight k) and
-// handed round by shuffles. The batch of particle records is broadcast from shared memory. The tile grids go to a scratch array; a second
+// fixed order. Every lane evaluates the weights of its own nodes from spline pieces it holds in
+// registers or takes as constant operands (no shuffles: the shared-memory/shuffle pipe is the
+// bottleneck of this kernel): for p = 4 a lane owns nodes t and t + 32 of the 64, for p >= 6 it owns
+// (jx, jy) pairs and walks jz. The batch of particle records is broadcast from shared memory. Grids
+// with few tiles give every tile several warps (each takes every split-th row of cells and writes
+// its own scratch grid). The tile grids go to a scratch array; a second
 // kernel sums, for every node, the (at most 8) tiles that cover it in a fixed order. Used when
 // every periodic axis has at least T + p - 1 nodes (each node then appears at
 // most once in a tile's grid); smaller grids use the gather kernel of particle_grid.cuh.
@@ -25,9 +26,10 @@ struct AnterpTiles {
   int T[3];        // tile edge in grid cells per axis (each >= p - 1)
   int nt[3];       // tiles per axis
   int D[3];        // T + p - 1: tile grid edge in nodes
+  int split;       // warps per tile: warp s takes the cell rows r = s (mod split), own scratch grid
 };
 
-// dynamic shared memory of k_anterp_tiles: node grid, spline pieces (padded so that the int arrays
+// dynamic shared memory of k_anterp_tiles: node grid (padded so that the int arrays
 // and the 32-byte records that follow stay aligned), row tables, batch staging
 template <typename T, int P> inline size_t anterp_smem_bytes(int D3) {
   const size_t grid_elems = ((size_t)D3 + P * P + 7) / 8 * 8;
@@ -43,25 +45,36 @@ k_anterp_tiles(GridGeom g, AnterpTiles at, SplineTab<T, P> tab, const int* __res
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* tg = reinterpret_cast<T*>(smem_raw);          // D^3 node grid
   const int D3 = at.D[0] * at.D[1] * at.D[2], Dx = at.D[0], Dy = at.D[1];
-  T* coef = tg + D3;                               // P x P spline piece coefficients
   constexpr int NT = (P * P * P + 31) / 32;        // nodes per lane
   const int lane = threadIdx.x;
-  int tl = blockIdx.x;
+  const int sub = blockIdx.x % at.split;
+  int tl = blockIdx.x / at.split;
   const int tx = tl % at.nt[0]; tl /= at.nt[0];
   const int ty = tl % at.nt[1], tz = tl / at.nt[1];
   const int C0[3] = {tx * at.T[0], ty * at.T[1], tz * at.T[2]};
   for (int i = lane; i < D3; i += 32) tg[i] = 0;
-  for (int i = lane; i < P * P; i += 32) coef[i] = tab.c[i / P][i % P];
   // static node offsets of this lane inside a particle's p^3 block, and the lanes that hold its weights
-  int noff[NT], lx[NT], ly[NT], lz[NT];
+  int noff[NT];
 #pragma unroll
   for (int s = 0; s < NT; ++s) {
     const int t = min(lane + 32 * s, P * P * P - 1);
     const int jx = t % P, jy = (t / P) % P, jz = t / (P * P);
     noff[s] = (jz * Dy + jy) * Dx + jx;
-    lx[s] = jx; ly[s] = P + jy; lz[s] = 2 * P + jz;
   }
-  constexpr bool kRegRows = (32 % P) == 0;
+  constexpr bool kRegRows = (32 % P) == 0 && P * P <= 32;
+  constexpr int NP = (P * P + 31) / 32;              // (jx, jy) pairs per lane in the other path
+  T pxr[kRegRows ? 1 : NP][P], pyr[kRegRows ? 1 : NP][P];
+  int poff[NP];
+  if (!kRegRows) {
+#pragma unroll
+    for (int s2 = 0; s2 < NP; ++s2) {
+      const int t = min(lane + 32 * s2, P * P - 1);
+      const int jx = t % P, jy = t / P;
+      poff[s2] = jy * Dx + jx;
+#pragma unroll
+      for (int k = 0; k < P; ++k) { pxr[s2][k] = tab.c[jx][k]; pyr[s2][k] = tab.c[jy][k]; }
+    }
+  }
   T cxr[P], cyr[P], czr[kRegRows ? NT : 1][P];       // spline pieces of this lane's rows
   if (kRegRows) {
     const int jx = lane % P, jy = (lane / P) % P;
@@ -79,13 +92,15 @@ k_anterp_tiles(GridGeom g, AnterpTiles at, SplineTab<T, P> tab, const int* __res
             cxn = min(at.T[0], g.ng[0] - C0[0]);
   // the tile's particles are one contiguous run per (cz, cy) row of cells: fetch all row bounds at
   // once and walk the concatenation of the runs (row-major, so the canonical order is kept)
-  const int nrows = czn * cyn;
+  const int nrows_all = czn * cyn;
+  const int nrows = (nrows_all - sub + at.split - 1) / at.split;      // rows sub, sub + split, ...
   int* rks = reinterpret_cast<int*>(tg + (D3 + P * P + 7) / 8 * 8);   // first particle of row r
   int* roff = rks + kMaxAnterpRows;                  // particles before row r; roff[nrows] = total
   int* sbase = roff + kMaxAnterpRows + 2;            // node offset of each particle of the batch
   V4* srec = reinterpret_cast<V4*>(sbase + 32 + 6);  // the batch's records (offset is a multiple of 32 B)
   for (int r = lane; r < nrows; r += 32) {
-    const int cz = r / cyn, cy = r - cz * cyn;
+    const int ra = sub + r * at.split;
+    const int cz = ra / cyn, cy = ra - cz * cyn;
     const int rowbase = ((C0[2] + cz) * g.ng[1] + (C0[1] + cy)) * g.ng[0];
     const int ks = gstart[rowbase + C0[0]], ke = gstart[rowbase + C0[0] + cxn];
     rks[r] = ks;
@@ -109,7 +124,8 @@ k_anterp_tiles(GridGeom g, AnterpTiles at, SplineTab<T, P> tab, const int* __res
         const int mid = (lo + hi + 1) >> 1;
         if (roff[mid] <= flat) lo = mid; else hi = mid - 1;
       }
-      const int cz = lo / cyn, cy = lo - cz * cyn;
+      const int ra = sub + lo * at.split;
+      const int cz = ra / cyn, cy = ra - cz * cyn;
       const int rowbase = ((C0[2] + cz) * g.ng[1] + (C0[1] + cy)) * g.ng[0];
       const int k = rks[lo] + (flat - roff[lo]);
       r = ldg4(grec + k);
@@ -138,25 +154,27 @@ k_anterp_tiles(GridGeom g, AnterpTiles at, SplineTab<T, P> tab, const int* __res
           }
         }
       } else {
-        // lane k < 3P evaluates weight (axis k / P, node offset k % P)
-        const int a = lane / P, j = lane - a * P;
-        const T f = a == 0 ? pr.x : (a == 1 ? pr.y : pr.z);
-        T w = 0;
-        if (lane < 3 * P) {
-          const T* c = coef + j * P;
-          w = c[P - 1];
+        // lanes own (jx, jy) pairs (pair t = lane + 32 s) and walk jz; the z weights use the spline
+        // pieces straight from the kernel parameters (compile-time rows: constant operands), the x
+        // and y weights the pieces of the lane's own rows in registers -- no shuffles
+        T wz[P];
 #pragma unroll
-          for (int k = P - 2; k >= 0; --k) w = fma(w, f, c[k]);
-          if (a == 2) w *= pr.w;
+        for (int j = 0; j < P; ++j) {
+          T w = tab.c[j][P - 1];
+#pragma unroll
+          for (int k = P - 2; k >= 0; --k) w = fma(w, pr.z, tab.c[j][k]);
+          wz[j] = w * pr.w;
         }
 #pragma unroll
-        for (int s2 = 0; s2 < NT; ++s2) {
-          const T wx = __shfl_sync(0xffffffffu, w, lx[s2]);
-          const T wy = __shfl_sync(0xffffffffu, w, ly[s2]);
-          const T wz = __shfl_sync(0xffffffffu, w, lz[s2]);
-          if (lane + 32 * s2 < P * P * P) {
-            T* dst = tg + base + noff[s2];
-            *dst = fma(wz * wy, wx, *dst);
+        for (int s2 = 0; s2 < NP; ++s2) {
+          T wx = pxr[s2][P - 1], wy = pyr[s2][P - 1];
+#pragma unroll
+          for (int k = P - 2; k >= 0; --k) { wx = fma(wx, pr.x, pxr[s2][k]); wy = fma(wy, pr.y, pyr[s2][k]); }
+          const T wxy = wx * wy;
+          if (lane + 32 * s2 < P * P) {
+            T* dst = tg + base + poff[s2];
+#pragma unroll
+            for (int j = 0; j < P; ++j) dst[j * Dx * Dy] = fma(wz[j], wxy, dst[j * Dx * Dy]);
           }
         }
       }
@@ -168,7 +186,7 @@ k_anterp_tiles(GridGeom g, AnterpTiles at, SplineTab<T, P> tab, const int* __res
 }
 
 // Q[m] = sum over the tiles whose grid covers node m (at most two per axis), in a fixed order
-template <typename T, int P>
+template <typename T, int P, bool SPLIT>
 __global__ void __launch_bounds__(128)
 k_anterp_combine(GridGeom g, AnterpTiles at, const T* __restrict__ scratch, T* __restrict__ Q) {
   constexpr int HP = P / 2;
@@ -204,7 +222,12 @@ k_anterp_combine(GridGeom g, AnterpTiles at, const T* __restrict__ scratch, T* _
     for (int b = 0; b < cnt[1]; ++b)
       for (int c = 0; c < cnt[0]; ++c) {
         const size_t tile = ((size_t)tix[2][a] * at.nt[1] + tix[1][b]) * at.nt[0] + tix[0][c];
-        acc += scratch[tile * D3 + ((size_t)lix[2][a] * at.D[1] + lix[1][b]) * at.D[0] + lix[0][c]];
+        const size_t off = ((size_t)lix[2][a] * at.D[1] + lix[1][b]) * at.D[0] + lix[0][c];
+        if (SPLIT) {
+          for (int sb = 0; sb < at.split; ++sb) acc += scratch[(tile * at.split + sb) * D3 + off];
+        } else {
+          acc += scratch[tile * D3 + off];
+        }
       }
   Q[m] = acc;
 }

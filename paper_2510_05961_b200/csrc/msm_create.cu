@@ -366,8 +366,10 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
       if (ntiles < (e ? std::atoi(e) : 128)) p->anterp_tiled = false;
     }
     if (const char* e = std::getenv("MSM_ANTERP_TILED")) p->anterp_tiled = p->anterp_tiled && std::atoi(e) != 0;
+    // few tiles: several warps per tile (each its own scratch grid) so that ~2000 warps run
+    p->at.split = (int)std::max<long long>(1, std::min<long long>(8, 2048 / std::max<long long>(ntiles, 1)));
     if (p->anterp_tiled)
-      p->anterp_scratch = dev_alloc(p, (size_t)ntiles * p->at.D[0] * p->at.D[1] * p->at.D[2] * p->esz);
+      p->anterp_scratch = dev_alloc(p, (size_t)ntiles * p->at.split * p->at.D[0] * p->at.D[1] * p->at.D[2] * p->esz);
   }
   const long long npc = (long long)bg.nc[0] * bg.nc[1] * bg.nc[2];
   const long long ngc = (long long)bg.ng[0] * bg.ng[1] * bg.ng[2];

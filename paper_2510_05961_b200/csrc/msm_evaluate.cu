@@ -200,11 +200,15 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   if (p->anterp_tiled) {
     const int D3 = p->at.D[0] * p->at.D[1] * p->at.D[2];
     const size_t sm = anterp_smem_bytes<T, P>(D3);
-    const int ntiles = p->at.nt[0] * p->at.nt[1] * p->at.nt[2];
+    const int ntiles = p->at.nt[0] * p->at.nt[1] * p->at.nt[2] * p->at.split;
     MSM_LAUNCH(p, (k_anterp_tiles<T, P><<<ntiles, 32, sm, st>>>(gg, p->at, tab, p->gstart, (const V4*)p->grec,
                                                                  p->gcell_sorted, (T*)p->anterp_scratch)));
-    MSM_LAUNCH(p, (k_anterp_combine<T, P><<<blocks_for(H.lev[1].points(), 128), 128, 0, st>>>(
-                      gg, p->at, (const T*)p->anterp_scratch, (T*)p->lev[1].Q)));
+    if (p->at.split > 1)
+      MSM_LAUNCH(p, (k_anterp_combine<T, P, true><<<blocks_for(H.lev[1].points(), 128), 128, 0, st>>>(
+                        gg, p->at, (const T*)p->anterp_scratch, (T*)p->lev[1].Q)));
+    else
+      MSM_LAUNCH(p, (k_anterp_combine<T, P, false><<<blocks_for(H.lev[1].points(), 128), 128, 0, st>>>(
+                        gg, p->at, (const T*)p->anterp_scratch, (T*)p->lev[1].Q)));
   } else {
     MSM_LAUNCH(p, (k_anterpolate<T, P><<<blocks_for(H.lev[1].points(), 128), 128, 0, st>>>(
                       gg, tab, p->gstart, (const V4*)p->grec, (T*)p->lev[1].Q)));
