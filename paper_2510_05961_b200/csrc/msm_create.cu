@@ -351,7 +351,7 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   // tiled anterpolation when each tile grid fits once into every periodic axis and there are enough
   // tiles (one warp each) to fill the GPU; otherwise the gather kernel
   {
-    const int tdim[3] = {8, 4, 4};
+    const int tdim[3] = {8, 8, 4};
     p->anterp_tiled = true;
     long long ntiles = 1;
     for (int ax = 0; ax < 3; ++ax) {

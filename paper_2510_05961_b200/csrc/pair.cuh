@@ -10,8 +10,9 @@
 // Only 17-27 % of the candidates are inside the cutoff, and a warp that branches per candidate
 // pays the full interaction whenever ANY lane hits. So the candidates of consecutive neighbour
 // rows are gathered into batches and each batch is processed in two phases:
-//   scan  -- every lane tests every candidate (one broadcast 16-byte shared load, 3 subtractions,
-//            3 multiply-adds, one compare, in fp32 on both precisions) and appends the index of
+//   scan  -- every lane tests every candidate (broadcast shared loads, 3 subtractions, 3 multiply-
+//            adds, one compare, in fp32 on both precisions, two candidates per packed f32x2
+//            instruction) and appends the index of
 //            each hit to its private list in shared memory; in fp64 mode the fp32 test uses a
 //            widened cutoff and the exact test is repeated in the drain;
 //   drain -- round r evaluates, on every lane that has one, the r-th hit of its list in full
@@ -46,22 +47,33 @@ template <typename T> struct PairParams {
 constexpr int kPairWarps = 1;
 constexpr int kPairMaxSplit = 5;
 
-template <typename T> struct PairStage;       // shared-memory staging of one warp
+// Shared-memory staging of one warp. The fp32 records are interleaved in pairs of candidates,
+// (x0 x1 | y0 y1 | z0 z1 | q0 q1), so that the scan tests two candidates per packed instruction:
+// candidate k sits at float offset pair_slot(k) + {0, 2, 4, 6}.
+__device__ __forceinline__ int pair_slot(int k) { return (k >> 1) * 8 + (k & 1); }
+template <typename T> struct PairStage;
 template <> struct PairStage<float> {
   static constexpr int kBatch = 160;          // candidates per batch (multiple of 32)
-  float4 f[kBatch];                           // scan and drain read the same record
+  __align__(16) float f[kBatch * 4];          // scan and drain read the same records
   unsigned char list[kBatch * 32];            // hit r of lane l at [r * 32 + l]
-  __device__ __forceinline__ void put(int k, float4 r) { f[k] = r; }
-  __device__ __forceinline__ float4 full(int k) const { return f[k]; }
+  __device__ __forceinline__ void put(int k, float4 r) {
+    float* q = f + pair_slot(k);
+    q[0] = r.x; q[2] = r.y; q[4] = r.z; q[6] = r.w;
+  }
+  __device__ __forceinline__ float4 full(int k) const {
+    const float* q = f + pair_slot(k);
+    return make_float4(q[0], q[2], q[4], q[6]);
+  }
 };
 template <> struct PairStage<double> {
   static constexpr int kBatch = 96;
-  float4 f[kBatch];                           // fp32 copy for the scan
+  __align__(16) float f[kBatch * 4];          // fp32 copy for the scan
   double4 d[kBatch];                          // full precision for the drain
   unsigned char list[kBatch * 32];
   __device__ __forceinline__ void put(int k, double4 r) {
     d[k] = r;
-    f[k] = make_float4((float)r.x, (float)r.y, (float)r.z, 0.f);
+    float* q = f + pair_slot(k);
+    q[0] = (float)r.x; q[2] = (float)r.y; q[4] = (float)r.z;
   }
   __device__ __forceinline__ double4 full(int k) const { return d[k]; }
 };
@@ -148,20 +160,26 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
       unsigned char* const lp = sj.list + lane;
       unsigned char* le = lp;                                 // end of this lane's hit list (stride 32)
       for (int w = 0; w < nw; ++w) {
-        const float4* fp = sj.f + w * 32;
+        const float* fw = sj.f + w * 128;                     // 16 candidate pairs of 8 floats
         const int ib = w * 32;
         if (!anymi) {
+          // two candidates per packed instruction (FADD2 / FMUL2 / FFMA2); same roundings as scalar
 #pragma unroll
-          for (int kk = 0; kk < 32; ++kk) {
-            const float4 pj = fp[kk];
-            const float dx = xs - pj.x, dy_ = ys - pj.y, dz_ = zs - pj.z;
-            const float r2 = fmaf(dx, dx, fmaf(dy_, dy_, dz_ * dz_));
-            if (r2 < a2_scan) { *le = (unsigned char)(ib + kk); le += 32; }
+          for (int m = 0; m < 16; ++m) {
+            const float4 xy = *reinterpret_cast<const float4*>(fw + m * 8);        // x0 x1 y0 y1
+            const float2 zz = *reinterpret_cast<const float2*>(fw + m * 8 + 4);    // z0 z1
+            const float2 dx = __fadd2_rn(make_float2(xs, xs), make_float2(-xy.x, -xy.y));
+            const float2 dy_ = __fadd2_rn(make_float2(ys, ys), make_float2(-xy.z, -xy.w));
+            const float2 dz_ = __fadd2_rn(make_float2(zs, zs), make_float2(-zz.x, -zz.y));
+            const float2 r2 = __ffma2_rn(dx, dx, __ffma2_rn(dy_, dy_, __fmul2_rn(dz_, dz_)));
+            if (r2.x < a2_scan) { *le = (unsigned char)(ib + 2 * m); le += 32; }
+            if (r2.y < a2_scan) { *le = (unsigned char)(ib + 2 * m + 1); le += 32; }
           }
         } else {
 #pragma unroll 4
           for (int kk = 0; kk < 32; ++kk) {
-            const float4 pj = fp[kk];
+            const float* pq = fw + pair_slot(kk);
+            const float4 pj = make_float4(pq[0], pq[2], pq[4], 0.f);
             float dx = xs - pj.x, dy_ = ys - pj.y, dz_ = zs - pj.z;
             if (mix) dx -= (float)prm.box[0] * rintf(dx * (float)prm.inv_box[0]);
             if (miy) dy_ -= (float)prm.box[1] * rintf(dy_ * (float)prm.inv_box[1]);
@@ -184,10 +202,10 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
             // the particle itself gets charge 0 and a harmless distance
             const bool two = r + 1 < n;
             const int ia = lp[r * 32], ib = two ? lp[(r + 1) * 32] : ia;
-            const float* pa = sf + ia * 4;
-            const float* pb = sf + ib * 4;
-            const float2 xj = make_float2(pa[0], pb[0]), yj = make_float2(pa[1], pb[1]), zj = make_float2(pa[2], pb[2]);
-            const float2 qj = make_float2(ia != selfpos ? pa[3] : 0.f, (two && ib != selfpos) ? pb[3] : 0.f);
+            const float* pa = sf + pair_slot(ia);
+            const float* pb = sf + pair_slot(ib);
+            const float2 xj = make_float2(pa[0], pb[0]), yj = make_float2(pa[2], pb[2]), zj = make_float2(pa[4], pb[4]);
+            const float2 qj = make_float2(ia != selfpos ? pa[6] : 0.f, (two && ib != selfpos) ? pb[6] : 0.f);
             const float2 dx = __fadd2_rn(make_float2(xf, xf), make_float2(-xj.x, -xj.y));
             const float2 dy_ = __fadd2_rn(make_float2(yf, yf), make_float2(-yj.x, -yj.y));
             const float2 dz_ = __fadd2_rn(make_float2(zf, zf), make_float2(-zj.x, -zj.y));
