@@ -5,6 +5,7 @@
 
 #include "gridops.cuh"
 #include "gridops_fused.cuh"
+#include "gridops_stream.cuh"
 #include "pair.cuh"
 #include "particle_grid.cuh"
 #include "plan.hpp"
@@ -223,9 +224,39 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     return g;
   };
   const int per3[3] = {p->bg.periodic[0], p->bg.periodic[1], p->bg.periodic[2]};
+  // one-sweep kernels: x periodic (lo = 0, whole 16-byte chunks), grid too large for the L2
+  auto stream_ok = [&](const Level& f, const Level& c) {
+    constexpr int VE = VecT<T>::VE;
+    return per3[0] && f.lo[0] == 0 && c.lo[0] == 0 && f.M[0] % (2 * VE) == 0 && c.M[0] * 2 == f.M[0] &&
+           (long long)f.points() >= p->stream_min_points;
+  };
+  auto stream_geom = [&](const Level& f, const Level& c) {
+    StreamGeom sg;
+    sg.f = grid3(f); sg.c = grid3(c);
+    sg.per_y = per3[1]; sg.per_z = per3[2];
+    sg.ntx = 1; sg.zseg = 1;
+    return sg;
+  };
+  // planes per block along the marching axis: enough blocks for ~8 per SM, at least 8 planes each
+  auto stream_zseg = [](int columns, int nplanes) {
+    const int want = std::max(1, (148 * 8 + columns - 1) / columns);
+    return std::max(std::min(8, nplanes), (nplanes + want - 1) / want);
+  };
   for (int l = 1; l < p->n_t; ++l) {
     const Level &f = H.lev[l], &c = H.lev[l + 1];
     const T* src = (const T*)p->lev[l].Q;
+    if (stream_ok(f, c)) {
+      // large grid: one sweep over the fine grid (gridops_stream.cuh)
+      constexpr int CY = 8;
+      StreamGeom sg = stream_geom(f, c);
+      const int cx = restrict_stream_cx<T, P + 1>();
+      sg.ntx = (c.M[0] + cx - 1) / cx;
+      const int nty = (c.M[1] + CY - 1) / CY;
+      sg.zseg = stream_zseg(sg.ntx * nty, c.M[2]);
+      const dim3 grid(sg.ntx * nty, (c.M[2] + sg.zseg - 1) / sg.zseg);
+      MSM_LAUNCH(p, (k_restrict_stream<T, P + 1, CY><<<grid, kStreamThreads, 0, st>>>(sg, Jt, src, (T*)p->lev[l + 1].Q)));
+      continue;
+    }
     int din[3] = {f.M[0], f.M[1], f.M[2]};
     for (int ax = 0; ax < 3; ++ax) {
       AxisDims d;
@@ -381,6 +412,18 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   // ---------------- S7 prolongation + accumulate, z then y then x
   for (int l = p->n_t - 1; l >= 1; --l) {
     const Level &f = H.lev[l], &c = H.lev[l + 1];
+    if (stream_ok(f, c)) {
+      StreamGeom sg = stream_geom(f, c);
+      constexpr int FXP = 64 * VecT<T>::VE, BY = 4;
+      sg.ntx = (f.M[0] + FXP - 1) / FXP;
+      auto pairs = [](int lo, int M) { return ((lo + M - 1) >> 1) - (lo >> 1) + 1; };   // node pairs (2b, 2b + 1) covering the axis
+      const int nty = (pairs(f.lo[1], f.M[1]) + BY - 1) / BY, npz = pairs(f.lo[2], f.M[2]);
+      sg.zseg = stream_zseg(sg.ntx * nty, npz);
+      const dim3 grid(sg.ntx * nty, (npz + sg.zseg - 1) / sg.zseg);
+      MSM_LAUNCH(p, (k_prolong_stream<T, P + 1><<<grid, kStreamThreads, 0, st>>>(sg, Jt, (const T*)p->lev[l + 1].E,
+                                                                                  (T*)p->lev[l].E)));
+      continue;
+    }
     const size_t sm = prolong3_smem_elems(P) * sizeof(T);
     auto kern = k_prolong3<T>;
     if (sm > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);

@@ -93,6 +93,10 @@ struct msm_plan {
   cudaGraphExec_t gexec = nullptr;
   cudaEvent_t gev = nullptr;
 
+  // fine grids with at least this many points take the one-sweep restriction / prolongation
+  // kernels of gridops_stream.cuh (they only pay when the grid does not fit the L2)
+  long long stream_min_points = 1ll << 24;
+
   // second stream for the pair kernel (runs beside the grid pipeline)
   bool overlap = true;
   cudaStream_t pstream = nullptr, vstream = nullptr;
