@@ -330,8 +330,53 @@ def run_ours(args, rank: int, world: int):
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "stages": stages,
         "energy": energy,
     }
+    if world == 1 and args.grid_microbench > 0:
+        plan.close()
+        out["grid_microbench"] = grid_microbench(args.grid_microbench, local, peaks["hbm_gbs"])
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.workload, 1, 0)[0]
+    return out
+
+
+def grid_microbench(M: int, local: int, hbm_gbs: float):
+    """S4/S7 (and the omega' filter of S5) on a grid that does not fit the L2: the same library
+    call on a periodic M^3 finest grid (fp32, p = 4, h = 2, a = 9, top grid 8^3) with a few
+    particles, per-stage CUDA-event times, against the algorithmic bytes of SURVEY.md 8(d):
+    restriction reads G_l and writes G_l / 8, prolongation reads G_l / 8 + G_l and writes G_l, the
+    filter reads and writes G_l, summed over the levels."""
+    import numpy as np
+    import torch
+    from paper_2510_05961_b200 import msm
+    dev = torch.device("cuda", local)
+    L = 2.0 * M
+    rng = np.random.default_rng(1)
+    n = 20000
+    pos = rng.random((n, 3)) * L
+    q = rng.uniform(-1, 1, n)
+    q -= q.mean()
+    levels = int(np.log2(M)) - 2
+    plan = msm.Plan((L,) * 3, (1, 1, 1), 2.0, 9.0, 4, levels, "fp32", max_particles=n, device=local)
+    tp = torch.tensor(pos, dtype=torch.float32, device=dev)
+    tq = torch.tensor(q, dtype=torch.float32, device=dev)
+    F = torch.zeros((n, 3), dtype=torch.float32, device=dev)
+    V = torch.zeros(n, dtype=torch.float32, device=dev)
+    plan.set_profiling(True)
+    acc = {}
+    reps = 3
+    for i in range(2 + reps):
+        plan.evaluate(tp, tq, F, V, True, False)
+        if i >= 2:
+            for k, v in plan.stage_times().items():
+                acc[k] = acc.get(k, 0.0) + v / reps
+    sum_g = float(sum((M >> l) ** 3 for l in range(levels - 1)))      # points of the levels that have a coarser one
+    byts = {"restrict": 4 * sum_g * (1 + 1 / 8), "prolongate": 4 * sum_g * (2 + 1 / 8), "filter": 4 * sum_g * 2}
+    out = {"grid": [M, M, M], "dtype": "f32", "p": 4, "levels": levels, "device_mb": round(plan.info.device_bytes / 1e6, 1),
+           "peak_gbs": hbm_gbs}
+    for k, b in byts.items():
+        gbs = b / (acc[k] * 1e-3) / 1e9
+        out[k] = {"ms": round(acc[k], 4), "algorithmic_mb": round(b / 1e6, 1), "achieved_gbs": round(gbs, 1),
+                  "frac": round(gbs / hbm_gbs, 4)}
+    plan.close()
     return out
 
 
@@ -384,9 +429,15 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4_water1m")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--grid-microbench", type=int, default=512,
+                    help="finest grid size M (power of two) of the HBM-bound grid-stage measurement; 0 skips it")
+    ap.add_argument("--only-grid-microbench", action="store_true", help="print the grid_microbench object alone")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.only_grid_microbench:
+        print(json.dumps({"grid_microbench": grid_microbench(args.grid_microbench, 0, load_peaks()[0]["hbm_gbs"])}), flush=True)
+        return
     if args.impl == "reference":
         args.steps = args.steps if args.steps is not None else 2
         args.warmup = args.warmup if args.warmup is not None else 1

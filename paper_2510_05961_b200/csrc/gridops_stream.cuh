@@ -196,18 +196,17 @@ template <typename T, int NJ> constexpr int restrict_stream_cx() {
 // Tile: 64 VE fine x (a warp row of 32 coarse chunks; the coarse neighbours of a chunk are loaded
 // directly -- the coarse array is 1/8 of the traffic), 8 fine y (4 node pairs); the block marches
 // over the coarse planes, keeps the x-y-prolonged planes of the window in registers and emits one
-// pair of fine planes (nodes 2a, 2a + 1) per step.
+// pair of fine planes (nodes 2a, 2a + 1) per step. In the y/z phase a thread owns one 16-byte
+// vector of fine x and one node pair in y: four vector loads and stores of E per step.
 template <typename T, int NJ>
-__global__ void __launch_bounds__(kStreamThreads)
+__global__ void __launch_bounds__(kStreamThreads, sizeof(T) == 4 ? 3 : 2)
 k_prolong_stream(StreamGeom g, AxisTaps<T> J, const T* __restrict__ ec, T* __restrict__ E) {
   using V = typename VecT<T>::type;
   using W = PairWindow<NJ / 2>;
   constexpr int VE = VecT<T>::VE;
   constexpr int KA = W::KA, OFFMIN = W::OFFMIN, OFFMAX = W::OFFMAX;
   constexpr int FXP = 64 * VE;                   // fine x per tile
-  constexpr int NG = kStreamThreads / FXP;       // thread groups along y (1 or 2)
-  constexpr int BY = 4;                          // y node pairs per tile
-  constexpr int FYT = 2 * BY / NG;               // fine y per thread
+  constexpr int BY = kStreamThreads / 64;        // y node pairs per tile (one per thread group)
   constexpr int NRC = BY + KA - 1;               // coarse rows per plane
   static_assert(NRC <= 8, "one row per warp");
   __shared__ __align__(16) T XP[NRC][FXP];
@@ -218,13 +217,11 @@ k_prolong_stream(StreamGeom g, AxisTaps<T> J, const T* __restrict__ ec, T* __res
   const int mcx = g.c.M[0];
   const int c0 = tx * 32 * VE + lane * VE;
   const bool xact = c0 < mcx;
-  // y: node pairs b0 .. b0 + BY - 1 (fine nodes 2b, 2b + 1); first pair covers the array's first node
-  const int bfirst = g.f.lo[1] >> 1;             // floor(lo / 2)
-  const int b0 = bfirst + ty * BY;
+  // y: node pairs b0 .. b0 + BY - 1 (fine nodes 2b, 2b + 1); the first pair holds the array's first node
+  const int b0 = (g.f.lo[1] >> 1) + ty * BY;
   // z: node pairs a0 .. a0 + na - 1
-  const int afirst = g.f.lo[2] >> 1;
   const int alast = (g.f.lo[2] + g.f.M[2] - 1) >> 1;
-  const int a0 = afirst + blockIdx.y * g.zseg, na = min(g.zseg, alast - a0 + 1);
+  const int a0 = (g.f.lo[2] >> 1) + blockIdx.y * g.zseg, na = min(g.zseg, alast - a0 + 1);
   const size_t cplane = (size_t)g.c.M[0] * g.c.M[1], fplane = (size_t)g.f.M[0] * g.f.M[1];
 
   // coarse row of this warp: node b0 + OFFMIN + warp
@@ -234,22 +231,24 @@ k_prolong_stream(StreamGeom g, AxisTaps<T> J, const T* __restrict__ ec, T* __res
 #pragma unroll
   for (int j = 0; j < VE + KA - 1; ++j) cxi[j] = imod(c0 + OFFMIN + j, mcx);
 
-  // the thread's fine points in the y/z phase
-  const int fxl = tid % FXP, grp = tid / FXP;
-  const int fx = tx * FXP + fxl;
+  // the thread's fine points in the y/z phase: x vector xg, node pair yg
+  const int xg = tid & 63, yg = tid >> 6;
+  const int fx = tx * FXP + xg * VE;
   const bool pact = fx < g.f.M[0];
-  int fyi[FYT];                                  // array row of fine y, or -1
+  int rowoff[2];                                 // offset of (fine y, fx) inside a plane, or -1
 #pragma unroll
-  for (int q = 0; q < FYT; ++q) {
-    const int i = 2 * b0 + grp * FYT + q - g.f.lo[1];
-    fyi[q] = (i >= 0 && i < g.f.M[1]) ? i : -1;
+  for (int s = 0; s < 2; ++s) {
+    const int i = 2 * (b0 + yg) + s - g.f.lo[1];
+    rowoff[s] = (pact && i >= 0 && i < g.f.M[1]) ? i * g.f.M[0] + fx : -1;
   }
 
-  T Pw[KA][FYT];
+  T Pw[KA][2][VE];
 #pragma unroll
   for (int d = 0; d < KA; ++d)
 #pragma unroll
-    for (int q = 0; q < FYT; ++q) Pw[d][q] = 0;
+    for (int s = 0; s < 2; ++s)
+#pragma unroll
+      for (int e = 0; e < VE; ++e) Pw[d][s][e] = 0;
 
   auto load_row = [&](int m, T (&buf)[VE + KA - 1]) {     // coarse plane node m, this warp's row
     const int cz = axis_index(m, g.c.lo[2], g.c.M[2], g.per_z);
@@ -267,15 +266,17 @@ k_prolong_stream(StreamGeom g, AxisTaps<T> J, const T* __restrict__ ec, T* __res
     if (m < mlast) load_row(m + 1, nxt);
     const int a = m - OFFMAX;                            // pair emitted in this step (if >= a0)
     // prefetch the fine values of that pair
-    T eold[2][FYT];
-    int fz[2];
+    V eold[2][2];
+    T* eptr[2][2];
 #pragma unroll
-    for (int s = 0; s < 2; ++s) {
-      const int i = 2 * a + s - g.f.lo[2];
-      fz[s] = (a >= a0 && i >= 0 && i < g.f.M[2]) ? i : -1;
+    for (int sz = 0; sz < 2; ++sz) {
+      const int i = 2 * a + sz - g.f.lo[2];
+      const bool zok = a >= a0 && i >= 0 && i < g.f.M[2];
 #pragma unroll
-      for (int q = 0; q < FYT; ++q)
-        eold[s][q] = (fz[s] >= 0 && fyi[q] >= 0 && pact) ? E[(size_t)fz[s] * fplane + (size_t)fyi[q] * g.f.M[0] + fx] : (T)0;
+      for (int sy = 0; sy < 2; ++sy) {
+        eptr[sz][sy] = (zok && rowoff[sy] >= 0) ? E + (size_t)i * fplane + rowoff[sy] : nullptr;
+        eold[sz][sy] = eptr[sz][sy] ? *reinterpret_cast<const V*>(eptr[sz][sy]) : zero_vec((V*)nullptr);
+      }
     }
     // x: fine 2 c + s <- sum over window slots of the coarse values around c
     if (warp < NRC) {
@@ -295,44 +296,51 @@ k_prolong_stream(StreamGeom g, AxisTaps<T> J, const T* __restrict__ ec, T* __res
       dst[1] = pack_vec((V*)nullptr, &fine[VE]);
     }
     __syncthreads();
-    // y: fine y (pair bl, parity s) <- rows bl + d; store as the newest plane of the window
+    // y: fine y (pair yg, parity s) <- rows yg + d; the result is the newest plane of the window
     {
-      constexpr int NRT = FYT / 2 + KA - 1;              // coarse rows this thread needs
-      T rows[NRT];
+      T rows[KA][VE];
 #pragma unroll
-      for (int j = 0; j < NRT; ++j) rows[j] = XP[grp * (FYT / 2) + j][fxl];
+      for (int d = 0; d < KA; ++d) unpack(*reinterpret_cast<const V*>(&XP[yg + d][xg * VE]), rows[d]);
 #pragma unroll
-      for (int q = 0; q < FYT; ++q) {
-        const int bl = q >> 1, s = q & 1;
-        T v = 0;
+      for (int s = 0; s < 2; ++s)
 #pragma unroll
-        for (int d = 0; d < KA; ++d) {
-          const int tap = s ? W::odd_tap(d) : W::even_tap(d);
-          if (tap >= 0) v = fma(J.c[tap >= 0 ? tap : 0], rows[bl + d], v);
-        }
-        Pw[KA - 1][q] = v;
-      }
-    }
-    // z: emit the pair a
-#pragma unroll
-    for (int s = 0; s < 2; ++s) {
-      if (fz[s] >= 0 && pact) {
-#pragma unroll
-        for (int q = 0; q < FYT; ++q) {
+        for (int e = 0; e < VE; ++e) {
           T v = 0;
 #pragma unroll
           for (int d = 0; d < KA; ++d) {
             const int tap = s ? W::odd_tap(d) : W::even_tap(d);
-            if (tap >= 0) v = fma(J.c[tap >= 0 ? tap : 0], Pw[d][q], v);
+            if (tap >= 0) v = fma(J.c[tap >= 0 ? tap : 0], rows[d][e], v);
           }
-          if (fyi[q] >= 0) E[(size_t)fz[s] * fplane + (size_t)fyi[q] * g.f.M[0] + fx] = eold[s][q] + v;
+          Pw[KA - 1][s][e] = v;
+        }
+    }
+    // z: emit the pair a
+#pragma unroll
+    for (int sz = 0; sz < 2; ++sz)
+#pragma unroll
+      for (int sy = 0; sy < 2; ++sy) {
+        if (eptr[sz][sy]) {
+          T o[VE];
+          unpack(eold[sz][sy], o);
+#pragma unroll
+          for (int e = 0; e < VE; ++e) {
+            T v = 0;
+#pragma unroll
+            for (int d = 0; d < KA; ++d) {
+              const int tap = sz ? W::odd_tap(d) : W::even_tap(d);
+              if (tap >= 0) v = fma(J.c[tap >= 0 ? tap : 0], Pw[d][sy][e], v);
+            }
+            o[e] += v;
+          }
+          *reinterpret_cast<V*>(eptr[sz][sy]) = pack_vec((V*)nullptr, o);
         }
       }
-    }
 #pragma unroll
     for (int d = 0; d + 1 < KA; ++d)
 #pragma unroll
-      for (int q = 0; q < FYT; ++q) Pw[d][q] = Pw[d + 1][q];
+      for (int s = 0; s < 2; ++s)
+#pragma unroll
+        for (int e = 0; e < VE; ++e) Pw[d][s][e] = Pw[d + 1][s][e];
     __syncthreads();
 #pragma unroll
     for (int j = 0; j < VE + KA - 1; ++j) cur[j] = nxt[j];

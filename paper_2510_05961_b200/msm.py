@@ -106,7 +106,7 @@ class Plan:
                    max_particles or w.n, device)
 
     def close(self):
-        if getattr(self, "_h", None):
+        if getattr(self, "_h", None) and lib is not None:     # (module globals are gone at interpreter exit)
             lib().msm_plan_destroy(self._h)
             self._h = None
 
