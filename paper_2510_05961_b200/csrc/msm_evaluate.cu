@@ -225,10 +225,10 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   };
   const int per3[3] = {p->bg.periodic[0], p->bg.periodic[1], p->bg.periodic[2]};
   // one-sweep kernels: x periodic (lo = 0, whole 16-byte chunks), grid too large for the L2
-  auto stream_ok = [&](const Level& f, const Level& c) {
+  auto stream_ok = [&](const Level& f, const Level& c, long long min_points) {
     constexpr int VE = VecT<T>::VE;
     return per3[0] && f.lo[0] == 0 && c.lo[0] == 0 && f.M[0] % (2 * VE) == 0 && c.M[0] * 2 == f.M[0] &&
-           (long long)f.points() >= p->stream_min_points;
+           (long long)f.points() >= min_points;
   };
   auto stream_geom = [&](const Level& f, const Level& c) {
     StreamGeom sg;
@@ -245,7 +245,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   for (int l = 1; l < p->n_t; ++l) {
     const Level &f = H.lev[l], &c = H.lev[l + 1];
     const T* src = (const T*)p->lev[l].Q;
-    if (stream_ok(f, c)) {
+    if (stream_ok(f, c, p->stream_min_points)) {
       // large grid: one sweep over the fine grid (gridops_stream.cuh)
       constexpr int CY = 8;
       StreamGeom sg = stream_geom(f, c);
@@ -412,7 +412,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   // ---------------- S7 prolongation + accumulate, z then y then x
   for (int l = p->n_t - 1; l >= 1; --l) {
     const Level &f = H.lev[l], &c = H.lev[l + 1];
-    if (stream_ok(f, c)) {
+    if (stream_ok(f, c, p->prolong_stream_min_points)) {
       StreamGeom sg = stream_geom(f, c);
       constexpr int FXP = 64 * VecT<T>::VE, BY = 4;
       sg.ntx = (f.M[0] + FXP - 1) / FXP;
