@@ -237,10 +237,10 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     sg.ntx = 1; sg.zseg = 1;
     return sg;
   };
-  // planes per block along the marching axis: enough blocks for ~8 per SM, at least 8 planes each
-  auto stream_zseg = [](int columns, int nplanes) {
+  // planes per block along the marching axis: enough blocks for ~8 per SM, at least min_planes each
+  auto stream_zseg = [](int columns, int nplanes, int min_planes) {
     const int want = std::max(1, (148 * 8 + columns - 1) / columns);
-    return std::max(std::min(8, nplanes), (nplanes + want - 1) / want);
+    return std::max(std::min(min_planes, nplanes), (nplanes + want - 1) / want);
   };
   for (int l = 1; l < p->n_t; ++l) {
     const Level &f = H.lev[l], &c = H.lev[l + 1];
@@ -252,7 +252,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
       const int cx = restrict_stream_cx<T, P + 1>();
       sg.ntx = (c.M[0] + cx - 1) / cx;
       const int nty = (c.M[1] + CY - 1) / CY;
-      sg.zseg = stream_zseg(sg.ntx * nty, c.M[2]);
+      sg.zseg = stream_zseg(sg.ntx * nty, c.M[2], 8);
       const dim3 grid(sg.ntx * nty, (c.M[2] + sg.zseg - 1) / sg.zseg);
       MSM_LAUNCH(p, (k_restrict_stream<T, P + 1, CY><<<grid, kStreamThreads, 0, st>>>(sg, Jt, src, (T*)p->lev[l + 1].Q)));
       continue;
@@ -418,7 +418,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
       sg.ntx = (f.M[0] + FXP - 1) / FXP;
       auto pairs = [](int lo, int M) { return ((lo + M - 1) >> 1) - (lo >> 1) + 1; };   // node pairs (2b, 2b + 1) covering the axis
       const int nty = (pairs(f.lo[1], f.M[1]) + BY - 1) / BY, npz = pairs(f.lo[2], f.M[2]);
-      sg.zseg = stream_zseg(sg.ntx * nty, npz);
+      sg.zseg = stream_zseg(sg.ntx * nty, npz, 2);     // small grids: short marches, more blocks
       const dim3 grid(sg.ntx * nty, (npz + sg.zseg - 1) / sg.zseg);
       MSM_LAUNCH(p, (k_prolong_stream<T, P + 1><<<grid, kStreamThreads, 0, st>>>(sg, Jt, (const T*)p->lev[l + 1].E,
                                                                                   (T*)p->lev[l].E)));
