@@ -428,7 +428,8 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
       cudaEventCreateWithFlags(&p->join2_ev, cudaEventDisableTiming) != cudaSuccess)
     return MSM_ERR_CUDA;
   if (const char* e = std::getenv("MSM_NO_OVERLAP")) p->overlap = std::atoi(e) == 0;
-  if (const char* e = std::getenv("MSM_GRID_STREAM_MIN")) p->stream_min_points = p->prolong_stream_min_points = std::atoll(e);
+  if (const char* e = std::getenv("MSM_GRID_STREAM_MIN")) p->stream_min_points = p->prolong_stream_min_points = p->filter_stream_min_points = std::atoll(e);
+  if (const char* e = std::getenv("MSM_FILTER_STREAM_MIN")) p->filter_stream_min_points = std::atoll(e);
   // stage list of msm_evaluate, in launch order
   for (const char* s : {"sort", "pair", "anterpolate", "restrict"}) p->stage_name_store.push_back(s);
   for (const char* s : {"filter", "conv", "conv_virial"}) p->stage_name_store.push_back(s);

@@ -6,6 +6,7 @@
 #include "gridops.cuh"
 #include "gridops_fused.cuh"
 #include "gridops_stream.cuh"
+#include "gridops_filter_stream.cuh"
 #include "pair.cuh"
 #include "particle_grid.cuh"
 #include "plan.hpp"
@@ -292,6 +293,42 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     const T* src = (const T*)d.Q;
     int din[3] = {lv.M[0], lv.M[1], lv.M[2]};
     const int halo[3] = {g.X0, g.R[1], g.R[2]};
+    {
+      // large grid: one sweep (gridops_filter_stream.cuh)
+      constexpr int VE = VecT<T>::VE;
+      const bool shape_ok = lv.M[0] % VE == 0 && g.P[0] % VE == 0 && g.X0 % VE == 0 &&
+                            (Wt.n == 11 || Wt.n == 13 || Wt.n == 15);
+      if (shape_ok && (long long)lv.points() >= p->filter_stream_min_points) {
+        FilterGeom fg;
+        for (int k = 0; k < 3; ++k) { fg.M[k] = lv.M[k]; fg.P[k] = g.P[k]; fg.H[k] = halo[k]; fg.per[k] = p->bg.periodic[k]; }
+        fg.ntx = (g.P[0] / VE + kFilterTXC - 1) / kFilterTXC;
+        const int ncols = fg.ntx * ((g.P[1] + kFilterTY - 1) / kFilterTY);
+        FilterTaps2 w2;
+        for (int k = 0; k < 15; ++k) w2.c[k] = k < Wt.n ? make_float2((float)Wt.c[k], (float)Wt.c[k]) : make_float2(0.f, 0.f);
+        // segments of planes: full waves of resident blocks against the 2 HW extra planes per segment
+        auto launch = [&](auto kern, int minb, size_t sm) {
+          const int resident = 148 * minb, extra = Wt.n - 1;
+          int best = 1; double best_eff = 0.0;
+          for (int ns = 1; ns <= std::max(1, g.P[2] / 16); ++ns) {
+            const long long nb = (long long)ncols * ns;
+            const int zs = (g.P[2] + ns - 1) / ns;
+            const double eff = (double)nb / (double)((nb + resident - 1) / resident * resident) * zs / (zs + extra);
+            if (eff > best_eff + 1e-9) { best_eff = eff; best = ns; }
+          }
+          fg.zseg = (g.P[2] + best - 1) / best;
+          const dim3 grid(ncols, (g.P[2] + fg.zseg - 1) / fg.zseg);
+          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+          MSM_LAUNCH(p, (kern<<<grid, kStreamThreads, sm, st>>>(fg, Wt, w2, src, (T*)d.pad)));
+        };
+        constexpr int MINB = sizeof(T) == 4 ? 2 : 1;
+        switch (Wt.n) {
+          case 11: launch(k_pad_filter_stream<T, 11, MINB>, MINB, filter_stream_smem<T, 11>()); break;
+          case 13: launch(k_pad_filter_stream<T, 13, 1>, 1, filter_stream_smem<T, 13>()); break;
+          default: launch(k_pad_filter_stream<T, 15, 1>, 1, filter_stream_smem<T, 15>()); break;
+        }
+        continue;
+      }
+    }
     for (int ax = 0; ax < 3; ++ax) {
       AxisDims ad;
       for (int k = 0; k < 3; ++k) { ad.in[k] = din[k]; ad.out[k] = din[k]; }

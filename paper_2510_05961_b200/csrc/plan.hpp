@@ -96,7 +96,7 @@ struct msm_plan {
   // fine grids with at least this many points take the one-sweep restriction / prolongation
   // kernels of gridops_stream.cuh (the restriction only pays when the grid does not fit the L2;
   // the prolongation measured faster at every size); MSM_GRID_STREAM_MIN sets both
-  long long stream_min_points = 1ll << 22, prolong_stream_min_points = 0;
+  long long stream_min_points = 1ll << 22, prolong_stream_min_points = 0, filter_stream_min_points = 1ll << 22;
 
   // second stream for the pair kernel (runs beside the grid pipeline)
   bool overlap = true;
