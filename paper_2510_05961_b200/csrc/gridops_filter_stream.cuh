@@ -34,7 +34,10 @@ struct FilterGeom {
   int ntx;           // columns along x (gridDim.x = columns in all)
   int zseg;          // output planes per block (gridDim.y segments)
 };
-struct FilterTaps2 { float2 c[15]; };   // (w[n], w[n]) for the packed fp32 passes
+struct FilterTaps2 {      // tap pairs of the packed fp32 passes
+  float2 c[15];           // (w[n], w[n])
+  float2 x[16];           // (w[k - 1], w[k]), zero outside the mask
+};
 
 constexpr int kFilterTXC = 16;     // output chunks per tile row
 constexpr int kFilterTY = 32;      // output rows per tile
@@ -45,9 +48,8 @@ template <typename T, int NT> constexpr size_t filter_stream_smem() {
   return (size_t)(2 * (kFilterTY + 2 * HW) + 2 * kFilterTY) * (kFilterTXC + 2 * HC) * VE * sizeof(T);
 }
 
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, bool valid) {
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int n) {   // n = 16, or 0: zero fill
   const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  const int n = valid ? 16 : 0;    // src-size 0: the 16 bytes are zero-filled
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gmem), "r"(n) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
@@ -78,7 +80,11 @@ template <> struct ChunkAcc<double> {
   }
   __device__ __forceinline__ void load(const double* p) { const double2 t = *reinterpret_cast<const double2*>(p); v[0] = t.x; v[1] = t.y; }
   __device__ __forceinline__ void store(double* p) const { *reinterpret_cast<double2*>(p) = make_double2(v[0], v[1]); }
-  __device__ __forceinline__ void set(const double (&a)[2]) { v[0] = a[0]; v[1] = a[1]; }
+  // x pass: outputs (2 H, 2 H + 1) of the chunk += (w[n], w[n + 1]) r
+  template <int H, int NT> __device__ __forceinline__ void fma_x(const AxisTaps<double>& w, const FilterTaps2&, int n, double r) {
+    if (n >= 0 && n < NT) v[0] = fma(w.c[n], r, v[0]);
+    if (n + 1 >= 0 && n + 1 < NT) v[1] = fma(w.c[n + 1], r, v[1]);
+  }
 };
 template <> struct ChunkAcc<float> {
   unsigned long long v[2];
@@ -95,18 +101,21 @@ template <> struct ChunkAcc<float> {
     const float2 a = f2_unpack(v[0]), b = f2_unpack(v[1]);
     *reinterpret_cast<float4*>(p) = make_float4(a.x, a.y, b.x, b.y);
   }
-  __device__ __forceinline__ void set(const float (&a)[4]) { v[0] = f2_pack(a[0], a[1]); v[1] = f2_pack(a[2], a[3]); }
+  // x pass: outputs (2 H, 2 H + 1) of the chunk += (w[n], w[n + 1]) r (r as broadcast operand)
+  template <int H, int NT> __device__ __forceinline__ void fma_x(const AxisTaps<float>&, const FilterTaps2& w2, int n, float r) {
+    if (n >= -1 && n < NT) f2_fma(v[H], f2_pack(w2.x[n + 1]), f2_pack(r, r));
+  }
 };
 
 // z pass of one plane whose index is SS mod NT: add to the ring, store and clear the finished slot
 template <int SS, typename T, int NT, int RY>
 __device__ __forceinline__ void filter_zstep(ChunkAcc<T> (&acc)[NT][RY], const ChunkAcc<T> (&v)[RY], const AxisTaps<T>& w,
-                                             const FilterTaps2& w2, T* const (&optr)[RY]) {
+                                             const FilterTaps2& w2, T* const (&optr)[RY], const bool (&emit)[RY]) {
 #pragma unroll
   for (int q = 0; q < RY; ++q) {
 #pragma unroll
     for (int n = 0; n < NT; ++n) acc[(SS + n) % NT][q].fma_tap(w, w2, n, v[q]);
-    if (optr[q]) acc[SS % NT][q].store(optr[q]);
+    if (emit[q]) acc[SS % NT][q].store(optr[q]);
     acc[SS % NT][q].zero();
   }
 }
@@ -137,8 +146,9 @@ k_pad_filter_stream(FilterGeom g, AxisTaps<T> w, FilterTaps2 w2, const T* __rest
   const int oz0 = blockIdx.y * g.zseg, nz = min(g.zseg, g.P[2] - oz0);
   const int S = nz + 2 * HW;                     // steps: raw planes oz0 - Hz - HW + s
 
-  // this thread's raw chunks: source inside a plane (nullptr: zeros)
-  const T* src[NLD];
+  // this thread's raw chunks: element offset inside a plane and copy size (0: zero fill)
+  unsigned roff[NLD];
+  int rsz[NLD];
 #pragma unroll
   for (int n = 0; n < NLD; ++n) {
     const int i = tid + kStreamThreads * n;
@@ -147,22 +157,19 @@ k_pad_filter_stream(FilterGeom g, AxisTaps<T> w, FilterTaps2 w2, const T* __rest
     bool ok = i < RC * NR;
     if (g.per[0]) gx = imod(gx, g.M[0]); else ok = ok && gx >= 0 && gx < g.M[0];
     if (g.per[1]) gy = imod(gy, g.M[1]); else ok = ok && gy >= 0 && gy < g.M[1];
-    src[n] = ok ? in + (size_t)gy * g.M[0] + gx : nullptr;
+    roff[n] = ok ? (unsigned)(gy * g.M[0] + gx) : 0u;
+    rsz[n] = ok ? 16 : 0;
   }
   int gz_next = oz0 - g.H[2] - HW;               // logical plane of the next fetch
   if (g.per[2]) gz_next = imod(gz_next, g.M[2]);
   auto fetch = [&](int s) {                      // raw plane of step s into RAW[s & 1]; always commits a group
     if (s < S) {
       const bool zok = gz_next >= 0 && gz_next < g.M[2];
-      const size_t zoff = zok ? (size_t)gz_next * iplane : 0;
+      const T* base = zok ? in + (size_t)gz_next * iplane : in;
       T* dst = RAW + (s & 1) * NR * RW + tid * VE;
 #pragma unroll
-      for (int n = 0; n < NLD; ++n) {
-        if (tid + kStreamThreads * n < RC * NR) {
-          const bool ok = zok && src[n] != nullptr;
-          cp_async16(dst + kStreamThreads * n * VE, ok ? src[n] + zoff : in, ok);
-        }
-      }
+      for (int n = 0; n < NLD; ++n)
+        if (tid + kStreamThreads * n < RC * NR) cp_async16(dst + kStreamThreads * n * VE, base + roff[n], zok ? rsz[n] : 0);
       if (++gz_next == g.M[2] && g.per[2]) gz_next = 0;
     }
     cp_async_commit();
@@ -195,12 +202,15 @@ k_pad_filter_stream(FilterGeom g, AxisTaps<T> w, FilterTaps2 w2, const T* __rest
   // x/z pass item: output chunk xc, rows RY * xr, RY * xr + 1
   const int xc = tid % TXC, xr = tid / TXC;
   const bool xact = VE * (xc0 + xc) < g.P[0];
-  T* optr[RY];                                   // where the next finished plane goes (nullptr: nowhere)
+  unsigned ooff[RY];                             // offset of the thread's chunks inside an output plane
+  bool oval[RY];
 #pragma unroll
   for (int q = 0; q < RY; ++q) {
     const int oy = oy0 + RY * xr + q;
-    optr[q] = (xact && oy < g.P[1]) ? out + (size_t)oz0 * oplane + (size_t)oy * g.P[0] + VE * (xc0 + xc) : nullptr;
+    oval[q] = xact && oy < g.P[1];
+    ooff[q] = oval[q] ? (unsigned)(oy * g.P[0] + VE * (xc0 + xc)) : 0u;
   }
+  T* obase = out + (size_t)oz0 * oplane;         // the plane that completes next
   CA acc[NT][RY];
 #pragma unroll
   for (int d = 0; d < NT; ++d)
@@ -223,40 +233,35 @@ k_pad_filter_stream(FilterGeom g, AxisTaps<T> w, FilterTaps2 w2, const T* __rest
 #pragma unroll
     for (int q = 0; q < RY; ++q) {
       const T* row = YF + (s & 1) * TY * RW + (RY * xr + q) * RW + xc * VE;
-      T vs[VE];
-#pragma unroll
-      for (int e = 0; e < VE; ++e) vs[e] = 0;
+      v[q].zero();
 #pragma unroll
       for (int c = 0; c < 2 * HC + 1; ++c) {
         if (VE * (c + 1) - 1 >= VE * HC - HW && VE * c <= VE - 1 + VE * HC + HW) {   // chunk holds needed values
           T r[VE];
           unpack(*reinterpret_cast<const V*>(row + c * VE), r);
 #pragma unroll
-          for (int i = 0; i < VE; ++i)
-#pragma unroll
-            for (int e = 0; e < VE; ++e) {
-              const int n = e + VE * HC + HW - (VE * c + i);
-              if (n >= 0 && n < NT) vs[e] = fma(w.c[n], r[i], vs[e]);
-            }
+          for (int i = 0; i < VE; ++i) {
+            // output e takes tap n = e + VE HC + HW - (VE c + i)
+            v[q].template fma_x<0, NT>(w, w2, VE * HC + HW - (VE * c + i), r[i]);
+            if constexpr (VE == 4) v[q].template fma_x<1, NT>(w, w2, 2 + VE * HC + HW - (VE * c + i), r[i]);
+          }
         }
       }
-      v[q].set(vs);
     }
     // z: into the ring; from step 2 HW on a plane is complete
+    const bool zdone = s >= 2 * HW;
     T* st[RY];
+    bool emit[RY];
 #pragma unroll
-    for (int q = 0; q < RY; ++q) st[q] = s >= 2 * HW ? optr[q] : nullptr;
+    for (int q = 0; q < RY; ++q) { st[q] = obase + ooff[q]; emit[q] = zdone && oval[q]; }
     switch (ss) {
-#define MSM_ZCASE(K) case K: if constexpr (K < NT) filter_zstep<K, T, NT, RY>(acc, v, w, w2, st); break;
+#define MSM_ZCASE(K) case K: if constexpr (K < NT) filter_zstep<K, T, NT, RY>(acc, v, w, w2, st, emit); break;
       MSM_ZCASE(0) MSM_ZCASE(1) MSM_ZCASE(2) MSM_ZCASE(3) MSM_ZCASE(4) MSM_ZCASE(5) MSM_ZCASE(6) MSM_ZCASE(7)
       MSM_ZCASE(8) MSM_ZCASE(9) MSM_ZCASE(10) MSM_ZCASE(11) MSM_ZCASE(12) MSM_ZCASE(13) MSM_ZCASE(14)
 #undef MSM_ZCASE
     }
     if (++ss == NT) ss = 0;
-    if (s >= 2 * HW) {
-#pragma unroll
-      for (int q = 0; q < RY; ++q) if (optr[q]) optr[q] += oplane;
-    }
+    if (zdone) obase += oplane;
   }
 }
 

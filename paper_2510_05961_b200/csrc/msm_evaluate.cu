@@ -304,7 +304,9 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
         fg.ntx = (g.P[0] / VE + kFilterTXC - 1) / kFilterTXC;
         const int ncols = fg.ntx * ((g.P[1] + kFilterTY - 1) / kFilterTY);
         FilterTaps2 w2;
-        for (int k = 0; k < 15; ++k) w2.c[k] = k < Wt.n ? make_float2((float)Wt.c[k], (float)Wt.c[k]) : make_float2(0.f, 0.f);
+        auto tap = [&](int k) { return k >= 0 && k < Wt.n ? (float)Wt.c[k] : 0.f; };
+        for (int k = 0; k < 15; ++k) w2.c[k] = make_float2(tap(k), tap(k));
+        for (int k = 0; k < 16; ++k) w2.x[k] = make_float2(tap(k - 1), tap(k));
         // segments of planes: full waves of resident blocks against the 2 HW extra planes per segment
         auto launch = [&](auto kern, int minb, size_t sm) {
           const int resident = 148 * minb, extra = Wt.n - 1;
