@@ -40,12 +40,11 @@ struct FilterTaps2 {      // tap pairs of the packed fp32 passes
 };
 
 constexpr int kFilterTXC = 16;     // output chunks per tile row
-constexpr int kFilterTY = 32;      // output rows per tile
 constexpr int kFilterCYY = 4;      // rows per thread in the y pass
 
-template <typename T, int NT> constexpr size_t filter_stream_smem() {
+template <typename T, int NT, int TY> constexpr size_t filter_stream_smem() {   // TY = output rows per tile
   constexpr int VE = VecT<T>::VE, HW = NT / 2, HC = (HW + VE - 1) / VE;
-  return (size_t)(2 * (kFilterTY + 2 * HW) + 2 * kFilterTY) * (kFilterTXC + 2 * HC) * VE * sizeof(T);
+  return (size_t)(2 * (TY + 2 * HW) + 2 * TY) * (kFilterTXC + 2 * HC) * VE * sizeof(T);
 }
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int n) {   // n = 16, or 0: zero fill
@@ -120,19 +119,19 @@ __device__ __forceinline__ void filter_zstep(ChunkAcc<T> (&acc)[NT][RY], const C
   }
 }
 
-template <typename T, int NT, int MINB>
+template <typename T, int NT, int MINB, int TY>
 __global__ void __launch_bounds__(kStreamThreads, MINB)
 k_pad_filter_stream(FilterGeom g, AxisTaps<T> w, FilterTaps2 w2, const T* __restrict__ in, T* __restrict__ out) {
   using V = typename VecT<T>::type;
   using CA = ChunkAcc<T>;
   constexpr int VE = VecT<T>::VE, HW = NT / 2, HC = (HW + VE - 1) / VE;
-  constexpr int TXC = kFilterTXC, TY = kFilterTY, CYY = kFilterCYY;
+  constexpr int TXC = kFilterTXC, CYY = kFilterCYY;
   constexpr int RC = TXC + 2 * HC;               // raw chunks per row
   constexpr int RW = RC * VE;                    // raw row length
   constexpr int NR = TY + 2 * HW;                // raw rows
   constexpr int NLD = (RC * NR + kStreamThreads - 1) / kStreamThreads;
-  constexpr int RY = 2;                          // output rows per thread in the x/z pass
-  static_assert(TXC * TY == kStreamThreads * RY, "tile shape");
+  constexpr int RY = TXC * TY / kStreamThreads;   // output rows per thread in the x/z pass
+  static_assert(TXC * TY == kStreamThreads * RY && RY >= 1, "tile shape");
   static_assert(RC * (TY / CYY) <= kStreamThreads, "one y-pass item per thread");
   static_assert(NT <= 15, "switch over the ring slots");
   extern __shared__ __align__(16) unsigned char filter_smem[];

@@ -302,13 +302,13 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
         FilterGeom fg;
         for (int k = 0; k < 3; ++k) { fg.M[k] = lv.M[k]; fg.P[k] = g.P[k]; fg.H[k] = halo[k]; fg.per[k] = p->bg.periodic[k]; }
         fg.ntx = (g.P[0] / VE + kFilterTXC - 1) / kFilterTXC;
-        const int ncols = fg.ntx * ((g.P[1] + kFilterTY - 1) / kFilterTY);
         FilterTaps2 w2;
         auto tap = [&](int k) { return k >= 0 && k < Wt.n ? (float)Wt.c[k] : 0.f; };
         for (int k = 0; k < 15; ++k) w2.c[k] = make_float2(tap(k), tap(k));
         for (int k = 0; k < 16; ++k) w2.x[k] = make_float2(tap(k - 1), tap(k));
         // segments of planes: full waves of resident blocks against the 2 HW extra planes per segment
-        auto launch = [&](auto kern, int minb, size_t sm) {
+        auto launch = [&](auto kern, int minb, int ty, size_t sm) {
+          const int ncols = fg.ntx * ((g.P[1] + ty - 1) / ty);
           const int resident = 148 * minb, extra = Wt.n - 1;
           int best = 1; double best_eff = 0.0;
           for (int ns = 1; ns <= std::max(1, g.P[2] / 16); ++ns) {
@@ -324,9 +324,9 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
         };
         constexpr int MINB = sizeof(T) == 4 ? 2 : 1;
         switch (Wt.n) {
-          case 11: launch(k_pad_filter_stream<T, 11, MINB>, MINB, filter_stream_smem<T, 11>()); break;
-          case 13: launch(k_pad_filter_stream<T, 13, 1>, 1, filter_stream_smem<T, 13>()); break;
-          default: launch(k_pad_filter_stream<T, 15, 1>, 1, filter_stream_smem<T, 15>()); break;
+          case 11: launch(k_pad_filter_stream<T, 11, MINB, 32>, MINB, 32, filter_stream_smem<T, 11, 32>()); break;
+          case 13: launch(k_pad_filter_stream<T, 13, 1, 32>, 1, 32, filter_stream_smem<T, 13, 32>()); break;
+          default: launch(k_pad_filter_stream<T, 15, 1, 32>, 1, 32, filter_stream_smem<T, 15, 32>()); break;
         }
         continue;
       }
