@@ -109,13 +109,17 @@ __device__ __forceinline__ void stage_plane(const ConvLevel& g, const T* __restr
   const T* src = qpad + ((size_t)pz * g.P[1] + Y) * g.P[0] + X;
   const int vper = WX / 4, nvec = nrow * vper;
   __syncwarp();
+  // asynchronous 16-byte copies: every load of the plane is in flight at once, no registers
   for (int v = lane; v < nvec; v += 32) {
     const int r = v / vper, cx = (v - r * vper) * 4;
-    T t[4];
-    SmemVec<T>::ldcg(src + (size_t)r * g.P[0] + cx, t);
+    const T* s = src + (size_t)r * g.P[0] + cx;
     T* dst = plane + r * g.pitch + cx;
-    dst[0] = t[0]; dst[1] = t[1]; dst[2] = t[2]; dst[3] = t[3];
+#pragma unroll
+    for (int h = 0; h < (int)(4 * sizeof(T) / 16); ++h)
+      cp_async16(reinterpret_cast<unsigned char*>(dst) + 16 * h, reinterpret_cast<const unsigned char*>(s) + 16 * h, 16);
   }
+  cp_async_commit();
+  cp_async_wait<0>();
   __syncwarp();
 }
 

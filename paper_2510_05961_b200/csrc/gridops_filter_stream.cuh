@@ -47,13 +47,6 @@ template <typename T, int NT, int TY> constexpr size_t filter_stream_smem() {   
   return (size_t)(2 * (TY + 2 * HW) + 2 * TY) * (kFilterTXC + 2 * HC) * VE * sizeof(T);
 }
 
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int n) {   // n = 16, or 0: zero fill
-  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gmem), "r"(n) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
 __device__ __forceinline__ unsigned long long f2_pack(float a, float b) {
   unsigned long long r;
   asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
