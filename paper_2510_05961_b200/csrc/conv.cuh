@@ -146,12 +146,53 @@ __device__ __forceinline__ ConvUnit decode_unit(const ConvTable& tab, int u) {
   return cu;
 }
 
+// Layout of a one-warp unit's shared memory in the generic (fp64) kernels: the input plane, then
+// the row entries of the ZT stencil layers the plane feeds, then two buffers for the taps of one
+// stencil row (all ZT layers). The table entries are copied with cp.async -- the next row's taps
+// while the current row is computed -- so that no FMA waits for a global load and no registers
+// are held for the prefetch.
+struct ConvSmemLayout {
+  int rows_off;      // byte offset of int4 srows[ZT][ny_max]
+  int taps_off;      // byte offset of the two tap buffers
+  int tapbuf;        // elements per tap buffer = ZT * tapk
+  int tapk;          // elements per layer and buffer
+};
+
+// row entries of layers dz(k), k < ZT, of one plane; invalid layers are marked empty
+template <int ZT, typename F>
+__device__ __forceinline__ void stage_rows(int4* srows, const int4* __restrict__ rows, int ny, int lane, F layer_row0) {
+  for (int i = lane; i < ZT * ny; i += 32) {
+    const int k = i / ny, j = i - k * ny;
+    const int r0 = layer_row0(k);                      // first entry of the layer in `rows`, or -1
+    if (r0 >= 0) cp_async16(srows + i, rows + r0 + j, 16);
+    else srows[i] = make_int4(0, 1, 0, 0);
+  }
+}
+
+// taps of stencil row j (all layers) into buffer `buf`: EPC elements per chunk
+template <typename T, int ZT, int EPC>
+__device__ __forceinline__ void issue_row_taps(const int4* srows, int ny, int j, const T* __restrict__ taps, T* buf,
+                                               int tapk, int lane) {
+  constexpr int PPC = EPC * (int)sizeof(T) / 16;       // 16-byte pieces per chunk
+#pragma unroll
+  for (int k = 0; k < ZT; ++k) {
+    const int4 e = srows[k * ny + j];
+    const int np = (e.z - e.y + 1) * PPC;
+    const unsigned char* src = reinterpret_cast<const unsigned char*>(taps + (size_t)e.x * EPC);
+    unsigned char* dst = reinterpret_cast<unsigned char*>(buf + k * tapk);
+    for (int q = lane; q < np; q += 32) cp_async16(dst + 16 * q, src + 16 * q, 16);
+  }
+  cp_async_commit();
+}
+
 // ---------------------------------------------------------------------------------- potential
 template <typename T, int XT, int ZT>
 __global__ void __launch_bounds__(32, sizeof(T) == 4 ? 16 : 12)
-k_conv(const ConvTable* __restrict__ tabp) {
+k_conv(const ConvTable* __restrict__ tabp, ConvSmemLayout sl) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* plane = reinterpret_cast<T*>(smem_raw);
+  int4* srows = reinterpret_cast<int4*>(smem_raw + sl.rows_off);
+  T* stap = reinterpret_cast<T*>(smem_raw + sl.taps_off);
   const ConvTable& tab = *tabp;
   const int lane = threadIdx.x;
   const ConvUnit cu = decode_unit<false, XT, ZT>(tab, blockIdx.x);
@@ -174,34 +215,42 @@ k_conv(const ConvTable* __restrict__ tabp) {
   const int p0 = g.pb[cu.slice], p1 = g.pb[cu.slice + 1];
   for (int pz = p0; pz < p1; ++pz) {
     const int zr = pz - Rz;              // input plane z = Z + zr
-    stage_plane<T>(g, qpad, plane, Z + pz, X, Y, nrow, WX, lane);
+    stage_rows<ZT>(srows, rows, ny, lane, [&](int k) {
+      const int dz = zr - k;
+      return dz >= -Rz && dz <= Rz ? (dz + Rz) * ny : -1;
+    });
+    stage_plane<T>(g, qpad, plane, Z + pz, X, Y, nrow, WX, lane);     // commits and waits (the row entries too)
+    issue_row_taps<T, ZT, 4>(srows, ny, 0, staps, stap, sl.tapk, lane);
     for (int dy = -Ry; dy <= Ry; ++dy) {
+      const int j = dy + Ry;
+      cp_async_wait<0>();                                  // this row's taps have landed
+      __syncwarp();
+      if (dy < Ry) issue_row_taps<T, ZT, 4>(srows, ny, j + 1, staps, stap + ((j + 1) & 1) * sl.tapbuf, sl.tapk, lane);
+      const T* tapb = stap + (j & 1) * sl.tapbuf;
       int4 re[ZT];
       int cl = 1 << 30, ch = -1;
 #pragma unroll
       for (int k = 0; k < ZT; ++k) {
-        const int dz = zr - k;
-        if (dz >= -Rz && dz <= Rz) re[k] = __ldg(rows + (dz + Rz) * ny + (dy + Ry));
-        else re[k] = make_int4(0, 1, 0, 0);   // empty
+        re[k] = srows[k * ny + j];
         if (re[k].y <= re[k].z) { cl = min(cl, re[k].y); ch = max(ch, re[k].z); }
       }
       const T* srow = plane + (lane + dy + Ry) * g.pitch;
       for (int c = cl; c <= ch; ++c) {
         T win[XT + 4];
 #pragma unroll
-        for (int j = 0; j < XT + 4; j += 4) {
+        for (int jj = 0; jj < XT + 4; jj += 4) {
           T t[4];
-          SmemVec<T>::load4(srow + 4 * c + j, t);
-          win[j] = t[0]; win[j + 1] = t[1]; win[j + 2] = t[2]; win[j + 3] = t[3];
+          SmemVec<T>::load4(srow + 4 * c + jj, t);
+          win[jj] = t[0]; win[jj + 1] = t[1]; win[jj + 2] = t[2]; win[jj + 3] = t[3];
         }
-        // all tap quads of this chunk are requested before the first FMA (loads of inactive rows
-        // read the table's first quad and are not used)
+        // all tap quads of this chunk are read before the first FMA (inactive rows read their
+        // layer's first quad and do not use it)
         T tp[ZT][4];
         bool on[ZT];
 #pragma unroll
         for (int k = 0; k < ZT; ++k) {
           on[k] = c >= re[k].y && c <= re[k].z;
-          SmemVec<T>::ldg(staps + (on[k] ? (re[k].x + c - re[k].y) * 4 : 0), tp[k]);
+          SmemVec<T>::load4(tapb + k * sl.tapk + (on[k] ? (c - re[k].y) * 4 : 0), tp[k]);
         }
 #pragma unroll
         for (int k = 0; k < ZT; ++k) {
@@ -213,6 +262,7 @@ k_conv(const ConvTable* __restrict__ tabp) {
           }
         }
       }
+      __syncwarp();                                        // the buffer is free for row dy + 2
     }
   }
   // outputs (slice partial or the final value)
@@ -409,9 +459,11 @@ __global__ void k_sum_slices(size_t n, int nslices, const T* __restrict__ part, 
 // ------------------------------------------------------------------------------------- virial
 template <typename T, int XT, int ZT>
 __global__ void __launch_bounds__(32, sizeof(T) == 4 ? 16 : 9)
-k_conv_virial(const ConvTable* __restrict__ tabp) {
+k_conv_virial(const ConvTable* __restrict__ tabp, ConvSmemLayout sl) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* plane = reinterpret_cast<T*>(smem_raw);
+  int4* srows = reinterpret_cast<int4*>(smem_raw + sl.rows_off);
+  T* stap = reinterpret_cast<T*>(smem_raw + sl.taps_off);
   const ConvTable& tab = *tabp;
   const int lane = threadIdx.x;
   const ConvUnit cu = decode_unit<true, XT, ZT>(tab, blockIdx.x);
@@ -440,18 +492,25 @@ k_conv_virial(const ConvTable* __restrict__ tabp) {
   const int p0 = g.vb[cu.slice], p1 = g.vb[cu.slice + 1];
   for (int pp = p0; pp < p1; ++pp) {
     const int zr = pp;
-    stage_plane<T>(g, qpad, plane, Z + zr + Rz, X, Y, nrow, WX, lane);
+    stage_rows<ZT>(srows, rows, ny, lane, [&](int k) {
+      const int dz = zr - k;
+      return dz >= 0 && dz <= Rz ? dz * ny : -1;
+    });
+    stage_plane<T>(g, qpad, plane, Z + zr + Rz, X, Y, nrow, WX, lane);   // commits and waits (the row entries too)
+    issue_row_taps<T, ZT, 12>(srows, ny, 0, vtaps, stap, sl.tapk, lane);
     for (int dy = -Ry; dy <= Ry; ++dy) {
+      const int j = dy + Ry;
+      cp_async_wait<0>();                                  // this row's taps have landed
+      __syncwarp();
+      if (dy < Ry) issue_row_taps<T, ZT, 12>(srows, ny, j + 1, vtaps, stap + ((j + 1) & 1) * sl.tapbuf, sl.tapk, lane);
+      const T* tapb = stap + (j & 1) * sl.tapbuf;
       int4 re[ZT];
       int cl = 1 << 30, ch = -1;
 #pragma unroll
       for (int k = 0; k < ZT; ++k) {
-        const int dz = zr - k;
-        if (dz >= 0 && dz <= Rz) re[k] = __ldg(rows + dz * ny + (dy + Ry));
-        else re[k] = make_int4(0, 1, 0, 0);
+        re[k] = srows[k * ny + j];
         if (re[k].y <= re[k].z) { cl = min(cl, re[k].y); ch = max(ch, re[k].z); }
       }
-      if (ch < cl) continue;
       T e0[ZT], e1[ZT], e2[ZT];
 #pragma unroll
       for (int k = 0; k < ZT; ++k) { e0[k] = 0; e1[k] = 0; e2[k] = 0; }
@@ -459,19 +518,19 @@ k_conv_virial(const ConvTable* __restrict__ tabp) {
       for (int c = cl; c <= ch; ++c) {
         T win[XT + 4];
 #pragma unroll
-        for (int j = 0; j < XT + 4; j += 4) {
+        for (int jj = 0; jj < XT + 4; jj += 4) {
           T t[4];
-          SmemVec<T>::load4(srow + 4 * c + j, t);
-          win[j] = t[0]; win[j + 1] = t[1]; win[j + 2] = t[2]; win[j + 3] = t[3];
+          SmemVec<T>::load4(srow + 4 * c + jj, t);
+          win[jj] = t[0]; win[jj + 1] = t[1]; win[jj + 2] = t[2]; win[jj + 3] = t[3];
         }
 #pragma unroll
         for (int k = 0; k < ZT; ++k) {
           if (c >= re[k].y && c <= re[k].z) {
-            const T* tp = vtaps + (size_t)(re[k].x + c - re[k].y) * 12;
+            const T* tp = tapb + k * sl.tapk + (c - re[k].y) * 12;
             T g0[4], g1[4], g2[4];
-            SmemVec<T>::ldg(tp, g0);
-            SmemVec<T>::ldg(tp + 4, g1);
-            SmemVec<T>::ldg(tp + 8, g2);
+            SmemVec<T>::load4(tp, g0);
+            SmemVec<T>::load4(tp + 4, g1);
+            SmemVec<T>::load4(tp + 8, g2);
 #pragma unroll
             for (int t = 0; t < 4; ++t) {
               T c0 = 0, c1 = 0;
@@ -488,6 +547,8 @@ k_conv_virial(const ConvTable* __restrict__ tabp) {
           }
         }
       }
+      __syncwarp();                                        // the buffer is free for row dy + 2
+      if (ch < cl) continue;
 #pragma unroll
       for (int k = 0; k < ZT; ++k) {
         const double fy = (double)dy, fz = (double)(zr - k);

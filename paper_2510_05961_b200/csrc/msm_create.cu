@@ -79,6 +79,7 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   else { pitch = round_up(pitch, 2); if (((pitch / 2) & 1) == 0) pitch += 2; }
   g.pitch = pitch;
   g.ny = 2 * st.R[1] + 1;
+  p->conv_ny_max = std::max(p->conv_ny_max, g.ny);
   p->conv_smem = std::max(p->conv_smem, (size_t)(32 + 2 * st.R[1]) * pitch * p->esz);
 
   const double A = std::ldexp(p->mp.a, l);
@@ -100,6 +101,7 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
       else {
         const int clo = (-Rx + g.X0) / 4, chi = (Rx + g.X0) / 4;
         r = make_int4((int)(ts.size() / 4), clo, chi, 0);
+        p->conv_maxc = std::max(p->conv_maxc, chi - clo + 1);
         wz[dz + Rz] += chi - clo + 1 + 0.5;
         for (int c = clo; c <= chi; ++c)
           for (int t = 0; t < 4; ++t) {

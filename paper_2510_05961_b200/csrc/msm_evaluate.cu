@@ -358,6 +358,16 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   mark();
   if (p->conv.nlev > 0) {
     constexpr int XT = sizeof(T) == 4 ? 16 : 8, ZT = 4;
+    // shared memory of a generic (fp64) unit: plane | row entries of ZT layers | two row-tap buffers
+    auto conv_layout = [&](int elems_per_chunk, size_t& total) {
+      ConvSmemLayout sl;
+      sl.rows_off = (int)((p->conv_smem + 15) / 16 * 16);
+      sl.taps_off = sl.rows_off + ZT * p->conv_ny_max * 16;
+      sl.tapk = p->conv_maxc * elems_per_chunk;
+      sl.tapbuf = ZT * sl.tapk;
+      total = (size_t)sl.taps_off + 2 * (size_t)sl.tapbuf * sizeof(T);
+      return sl;
+    };
     auto launch_virial = [&](cudaStream_t vs) {
       if constexpr (sizeof(T) == 4) {
         auto kern = k_conv_virial_f2<XT>;             // packed FMAs (FFMA2)
@@ -366,9 +376,10 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
         MSM_LAUNCH(p, (kern<<<p->conv.total_vunits, 32, p->conv_smem, vs>>>(p->d_conv)));
       } else {
         auto kern = k_conv_virial<T, XT, ZT>;
-        if (p->conv_smem > 48 * 1024)
-          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
-        MSM_LAUNCH(p, (kern<<<p->conv.total_vunits, 32, p->conv_smem, vs>>>(p->d_conv)));
+        size_t sm;
+        const ConvSmemLayout sl = conv_layout(12, sm);
+        if (sm > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        MSM_LAUNCH(p, (kern<<<p->conv.total_vunits, 32, sm, vs>>>(p->d_conv, sl)));
       }
     };
     // the virial correlation only needs the filtered grid charge: it runs on a third stream beside
@@ -399,9 +410,10 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
         }
       } else {
         auto kern = k_conv<T, XT, ZT>;
-        if (p->conv_smem > 48 * 1024)
-          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
-        MSM_LAUNCH(p, (kern<<<p->conv.total_units, 32, p->conv_smem, st>>>(p->d_conv)));
+        size_t sm;
+        const ConvSmemLayout sl = conv_layout(4, sm);
+        if (sm > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        MSM_LAUNCH(p, (kern<<<p->conv.total_units, 32, sm, st>>>(p->d_conv, sl)));
       }
       for (int l = 1; l < p->n_t; ++l) {
         const ConvLevel& g = p->conv.lev[l - 1];

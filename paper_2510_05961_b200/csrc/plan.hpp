@@ -52,6 +52,7 @@ struct msm_plan {
   msm::ConvTable conv{};                             // host copy; conv.lev[l - 1] is level l
   msm::ConvTable* d_conv = nullptr;
   size_t conv_smem = 0;
+  int conv_ny_max = 0, conv_maxc = 0;   // largest row count 2 R_y + 1 and chunks per stencil row over the levels
   size_t conv_tables_smem = 0;                       // fp32: largest row + tap table of a level (bytes)
   int conv_slices = 1;                               // input-plane slices per output tile
   double* conv_wpart = nullptr;                      // total_vunits x 6
