@@ -587,10 +587,12 @@ __device__ __forceinline__ unsigned long long fadd2_pp(unsigned long long a, uns
 
 template <int XT>
 __global__ void __launch_bounds__(32, 16)
-k_conv_virial_f2(const ConvTable* __restrict__ tabp) {
+k_conv_virial_f2(const ConvTable* __restrict__ tabp, ConvSmemLayout sl) {
   constexpr int ZT = 4, ZP = 2;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float* plane = reinterpret_cast<float*>(smem_raw);
+  int4* srows = reinterpret_cast<int4*>(smem_raw + sl.rows_off);      // [ZP][ny]
+  float* stap = reinterpret_cast<float*>(smem_raw + sl.taps_off);     // two buffers of ZP * tapk floats
   const ConvTable& tab = *tabp;
   const int lane = threadIdx.x;
   const ConvUnit cu = decode_unit<true, XT, ZT>(tab, blockIdx.x);
@@ -601,7 +603,7 @@ k_conv_virial_f2(const ConvTable* __restrict__ tabp) {
   const int WX = XT + 2 * g.X0 + 4;
   const int ny = g.ny;
   const int4* __restrict__ rows = g.vrows2;
-  const float4* __restrict__ vtaps = reinterpret_cast<const float4*>(g.vtaps2);
+  const float* __restrict__ vtaps = reinterpret_cast<const float*>(g.vtaps2);   // 24 floats per chunk
   const float* __restrict__ qpad = reinterpret_cast<const float*>(g.pad);
   const float* __restrict__ Q = reinterpret_cast<const float*>(g.Q);
 
@@ -620,15 +622,25 @@ k_conv_virial_f2(const ConvTable* __restrict__ tabp) {
 
   const int p0 = g.vb[cu.slice], p1 = g.vb[cu.slice + 1];
   for (int zr = p0; zr < p1; ++zr) {                  // input plane z = Z + zr, only dz >= 0
-    stage_plane<float>(g, qpad, plane, Z + zr + Rz, X, Y, nrow, WX, lane);
+    // row entries of the merged layers to shared memory with the plane; the taps of stencil row
+    // dy + 1 are copied (cp.async) while row dy is computed: no FMA waits for a table load
+    stage_rows<ZP>(srows, rows, ny, lane, [&](int k) {
+      const int d = zr - 2 * k;                       // planes (2k, 2k+1) take rows (d, d - 1)
+      return d >= 0 && d <= Rz + 1 ? d * ny : -1;
+    });
+    stage_plane<float>(g, qpad, plane, Z + zr + Rz, X, Y, nrow, WX, lane);   // commits and waits
+    issue_row_taps<float, ZP, 24>(srows, ny, 0, vtaps, stap, sl.tapk, lane);
     for (int dy = -Ry; dy <= Ry; ++dy) {
+      const int jr = dy + Ry;
+      cp_async_wait<0>();                             // this row's taps have landed
+      __syncwarp();
+      if (dy < Ry) issue_row_taps<float, ZP, 24>(srows, ny, jr + 1, vtaps, stap + ((jr + 1) & 1) * sl.tapbuf, sl.tapk, lane);
+      const float* tapb = stap + (jr & 1) * sl.tapbuf;
       int4 re[ZP];
       int cl = 1 << 30, ch = -1;
 #pragma unroll
       for (int k = 0; k < ZP; ++k) {
-        const int d = zr - 2 * k;                     // planes (2k, 2k+1) take rows (d, d - 1)
-        if (d >= 0 && d <= Rz + 1) re[k] = __ldg(rows + d * ny + (dy + Ry));
-        else re[k] = make_int4(0, 1, 0, 0);
+        re[k] = srows[k * ny + jr];
         if (re[k].y <= re[k].z) { cl = min(cl, re[k].y); ch = max(ch, re[k].z); }
       }
       if (ch < cl) continue;
@@ -646,10 +658,10 @@ k_conv_virial_f2(const ConvTable* __restrict__ tabp) {
 #pragma unroll
         for (int k = 0; k < ZP; ++k) {
           if (c >= re[k].y && c <= re[k].z) {
-            const float4* tp = vtaps + (size_t)(re[k].x + c - re[k].y) * 6;
+            const float4* tp = reinterpret_cast<const float4*>(tapb + k * sl.tapk + (c - re[k].y) * 24);
             float4 gq[6];
 #pragma unroll
-            for (int m = 0; m < 6; ++m) gq[m] = __ldg(tp + m);
+            for (int m = 0; m < 6; ++m) gq[m] = tp[m];
 #pragma unroll
             for (int t = 0; t < 4; ++t) {
               unsigned long long c0 = 0ull, c1 = 0ull;

@@ -196,6 +196,7 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
         const int xlo = ha && hb ? std::min(alo, blo) : (ha ? alo : blo);
         const int xhi = ha && hb ? std::max(ahi, bhi) : (ha ? ahi : bhi);
         const int clo = (xlo + g.X0) / 4, chi = (xhi + g.X0) / 4;
+        p->conv_maxc = std::max(p->conv_maxc, chi - clo + 1);
         std::vector<double> rowv;
         for (int c = clo; c <= chi; ++c)
           for (int m = 0; m < 3; ++m)

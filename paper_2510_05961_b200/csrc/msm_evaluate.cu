@@ -359,25 +359,26 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   if (p->conv.nlev > 0) {
     constexpr int XT = sizeof(T) == 4 ? 16 : 8, ZT = 4;
     // shared memory of a generic (fp64) unit: plane | row entries of ZT layers | two row-tap buffers
-    auto conv_layout = [&](int elems_per_chunk, size_t& total) {
+    auto conv_layout = [&](int elems_per_chunk, int layers, size_t& total) {
       ConvSmemLayout sl;
       sl.rows_off = (int)((p->conv_smem + 15) / 16 * 16);
-      sl.taps_off = sl.rows_off + ZT * p->conv_ny_max * 16;
+      sl.taps_off = sl.rows_off + layers * p->conv_ny_max * 16;
       sl.tapk = p->conv_maxc * elems_per_chunk;
-      sl.tapbuf = ZT * sl.tapk;
+      sl.tapbuf = layers * sl.tapk;
       total = (size_t)sl.taps_off + 2 * (size_t)sl.tapbuf * sizeof(T);
       return sl;
     };
     auto launch_virial = [&](cudaStream_t vs) {
       if constexpr (sizeof(T) == 4) {
         auto kern = k_conv_virial_f2<XT>;             // packed FMAs (FFMA2)
-        if (p->conv_smem > 48 * 1024)
-          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
-        MSM_LAUNCH(p, (kern<<<p->conv.total_vunits, 32, p->conv_smem, vs>>>(p->d_conv)));
+        size_t sm;
+        const ConvSmemLayout sl = conv_layout(24, 2, sm);
+        if (sm > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        MSM_LAUNCH(p, (kern<<<p->conv.total_vunits, 32, sm, vs>>>(p->d_conv, sl)));
       } else {
         auto kern = k_conv_virial<T, XT, ZT>;
         size_t sm;
-        const ConvSmemLayout sl = conv_layout(12, sm);
+        const ConvSmemLayout sl = conv_layout(12, ZT, sm);
         if (sm > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
         MSM_LAUNCH(p, (kern<<<p->conv.total_vunits, 32, sm, vs>>>(p->d_conv, sl)));
       }
@@ -411,7 +412,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
       } else {
         auto kern = k_conv<T, XT, ZT>;
         size_t sm;
-        const ConvSmemLayout sl = conv_layout(4, sm);
+        const ConvSmemLayout sl = conv_layout(4, ZT, sm);
         if (sm > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
         MSM_LAUNCH(p, (kern<<<p->conv.total_units, 32, sm, st>>>(p->d_conv, sl)));
       }
