@@ -302,20 +302,17 @@ __device__ __forceinline__ void ffma2_bcast(unsigned long long& acc, float s, un
   asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(pack2(s, s)), "l"(pair));
 }
 
-// read-only 16-byte load that the compiler may not move (it would otherwise sink the tap loads into
-// the branch that uses them, right in front of the first dependent FMA)
-__device__ __forceinline__ float4 ldg_pinned(const float4* p) {
-  float4 v;
-  asm volatile("ld.global.nc.L1::evict_last.v4.f32 {%0, %1, %2, %3}, [%4];"
-               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
-  return v;
-}
-
-// One unit of the packed convolution. SM: the row and tap tables are in shared memory (plain loads)
-// instead of global memory (pinned read-only loads).
+// One unit of the packed convolution. SM: the level's whole row and tap tables are in the block's
+// shared memory; otherwise the warp stages the entries it needs row by row (see below).
 template <int XT, bool SM>
 __device__ __forceinline__ void conv_f2_unit(const ConvLevel& g, const ConvUnit& cu, const int4* rows2,
-                                             const float4* taps2, float* plane, int lane) {
+                                             const float4* taps2, float* plane, int lane,
+                                             int4* wrows = nullptr, float* stap = nullptr,
+                                             ConvSmemLayout sl = ConvSmemLayout()) {
+  // SM: rows2 / taps2 are the block's shared-memory copies of the level's whole tables. Otherwise
+  // (one-warp blocks, small jobs) they are the global tables: the warp copies the row entries of its
+  // two merged layers to `wrows` with the plane and the taps of stencil row dy + 1 into one of the
+  // two buffers of `stap` (cp.async) while row dy is computed.
   constexpr int ZP = 2;                               // two pairs of output planes
   const int X = cu.X, Y = cu.Y, Z = cu.Z;
   const int Ry = g.R[1], Rz = g.R[2];
@@ -333,14 +330,31 @@ __device__ __forceinline__ void conv_f2_unit(const ConvLevel& g, const ConvUnit&
   const int p0 = g.pb[cu.slice], p1 = g.pb[cu.slice + 1];
   for (int pz = p0; pz < p1; ++pz) {
     const int zr = pz - Rz;                           // input plane z = Z + zr
-    stage_plane<float>(g, qpad, plane, Z + pz, X, Y, nrow, WX, lane);
+    if (!SM)
+      stage_rows<ZP>(wrows, rows2, ny, lane, [&](int k) {
+        const int d = zr - 2 * k;
+        return d >= -Rz && d <= Rz + 1 ? (d + Rz) * ny : -1;
+      });
+    stage_plane<float>(g, qpad, plane, Z + pz, X, Y, nrow, WX, lane);     // commits and waits
+    if (!SM) issue_row_taps<float, ZP, 8>(wrows, ny, 0, reinterpret_cast<const float*>(taps2), stap, sl.tapk, lane);
     for (int dy = -Ry; dy <= Ry; ++dy) {
+      const int jr = dy + Ry;
+      const float* tapb = nullptr;
+      if (!SM) {
+        cp_async_wait<0>();                           // this row's taps have landed
+        __syncwarp();
+        if (dy < Ry)
+          issue_row_taps<float, ZP, 8>(wrows, ny, jr + 1, reinterpret_cast<const float*>(taps2),
+                                       stap + ((jr + 1) & 1) * sl.tapbuf, sl.tapk, lane);
+        tapb = stap + (jr & 1) * sl.tapbuf;
+      }
       int4 re[ZP];
       int cl = 1 << 30, ch = -1;
 #pragma unroll
       for (int k = 0; k < ZP; ++k) {
         const int d = zr - 2 * k;                     // planes (2k, 2k+1) take stencil rows (d, d - 1)
-        if (d >= -Rz && d <= Rz + 1) re[k] = SM ? rows2[(d + Rz) * ny + (dy + Ry)] : __ldg(rows2 + (d + Rz) * ny + (dy + Ry));
+        if (!SM) re[k] = wrows[k * ny + jr];
+        else if (d >= -Rz && d <= Rz + 1) re[k] = rows2[(d + Rz) * ny + (dy + Ry)];
         else re[k] = make_int4(0, 0, -1, 0);          // empty
         if (re[k].y <= re[k].z) { cl = min(cl, re[k].y); ch = max(ch, re[k].z); }
       }
@@ -359,9 +373,10 @@ __device__ __forceinline__ void conv_f2_unit(const ConvLevel& g, const ConvUnit&
           on[k] = c >= re[k].y && c <= re[k].z;
           // unconditional address (clamped into the row; an empty row reads the guard chunk in front
           // of the table), so the loads are not tied to the branch below
-          const float4* tp = taps2 + (re[k].x + min(max(c, re[k].y), re[k].z) - re[k].y) * 2;
-          tq[k][0] = SM ? tp[0] : ldg_pinned(tp);
-          tq[k][1] = SM ? tp[1] : ldg_pinned(tp + 1);
+          const float4* tp = SM ? taps2 + (re[k].x + min(max(c, re[k].y), re[k].z) - re[k].y) * 2
+                                : reinterpret_cast<const float4*>(tapb + k * sl.tapk + (on[k] ? (c - re[k].y) * 8 : 0));
+          tq[k][0] = tp[0];
+          tq[k][1] = tp[1];
         }
 #pragma unroll
         for (int k = 0; k < ZP; ++k) {
@@ -405,13 +420,14 @@ __device__ __forceinline__ void conv_f2_unit(const ConvLevel& g, const ConvUnit&
 
 template <int XT>
 __global__ void __launch_bounds__(32, 16)
-k_conv_f2(const ConvTable* __restrict__ tabp) {
+k_conv_f2(const ConvTable* __restrict__ tabp, ConvSmemLayout sl) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const ConvTable& tab = *tabp;
   const ConvUnit cu = decode_unit<false, XT, 4>(tab, blockIdx.x);
   const ConvLevel& g = tab.lev[cu.lev];
   conv_f2_unit<XT, false>(g, cu, g.rows2, reinterpret_cast<const float4*>(g.taps2),
-                          reinterpret_cast<float*>(smem_raw), threadIdx.x);
+                          reinterpret_cast<float*>(smem_raw), threadIdx.x,
+                          reinterpret_cast<int4*>(smem_raw + sl.rows_off), reinterpret_cast<float*>(smem_raw + sl.taps_off), sl);
 }
 
 // The same with the level's row and tap tables copied into shared memory once per block of kConvSW

@@ -405,9 +405,10 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
           MSM_LAUNCH(p, (kern<<<p->conv.total_sunits / kConvSW, 32 * kConvSW, sm_s, st>>>(p->d_conv, (int)plane_b)));
         } else {
           auto kern = k_conv_f2<XT>;
-          if (p->conv_smem > 48 * 1024)
-            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->conv_smem);
-          MSM_LAUNCH(p, (kern<<<p->conv.total_units, 32, p->conv_smem, st>>>(p->d_conv)));
+          size_t sm;
+          const ConvSmemLayout sl = conv_layout(8, 2, sm);
+          if (sm > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+          MSM_LAUNCH(p, (kern<<<p->conv.total_units, 32, sm, st>>>(p->d_conv, sl)));
         }
       } else {
         auto kern = k_conv<T, XT, ZT>;
