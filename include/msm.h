@@ -32,8 +32,8 @@ typedef struct msm_plan msm_plan_t; /* opaque; owns all device and host scratch 
 typedef enum {
   MSM_OK = 0,
   MSM_ERR_INVALID_ARG = 1,        /* non-positive box/h/a, odd or unsupported p, levels < 1, NULL */
-  MSM_ERR_UNSUPPORTED = 2,        /* exactly one periodic axis (reading T4); unequal periodic grid
-                                     counts (reading B3); top grid larger than MSM_MAX_TOP_POINTS */
+  MSM_ERR_UNSUPPORTED = 2,        /* exactly one periodic axis (reading T4); top grid larger than
+                                     MSM_MAX_TOP_POINTS; stencil too wide for the shared memory */
   MSM_ERR_CUTOFF_TOO_LARGE = 3,   /* periodic axis with a > box/2: minimum image invalid */
   MSM_ERR_TOO_MANY_PARTICLES = 4, /* n > max_particles */
   MSM_ERR_OUT_OF_BOX = 5,         /* open-axis coordinate outside [0, box], or non-finite input */

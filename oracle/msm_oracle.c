@@ -36,6 +36,9 @@ typedef struct {
   int p;         /* B-spline order (even) */
   int levels;    /* used only when no axis is periodic (reading G4) */
   int mu;        /* extra quasi-interpolation terms (reading Q) */
+  int pad;       /* test knob for reading G3's pin: extra nodes added on both sides of every open
+                    axis at every level (0 = the minimal extents of G2/G3); no output may depend
+                    on it beyond round-off */
 } msmo_params;
 
 typedef struct {
@@ -189,8 +192,8 @@ static int setup_geometry(msmo_ctx *c) {
       c->hl[1][ax] = P->box[ax] / (double)m;
       if (m > maxM) maxM = m;
     } else {
-      c->lo[1][ax] = -(hp - 1);                             /* reading G2 */
-      c->hi[1][ax] = (int)floor(P->box[ax] / P->h) + hp;
+      c->lo[1][ax] = -(hp - 1) - P->pad;                    /* reading G2 (+ the G3 pin's padding) */
+      c->hi[1][ax] = (int)floor(P->box[ax] / P->h) + hp + P->pad;
       c->M[1][ax] = c->hi[1][ax] - c->lo[1][ax] + 1;
       c->hl[1][ax] = P->h;
     }
@@ -205,8 +208,8 @@ static int setup_geometry(msmo_ctx *c) {
         c->M[l + 1][ax] = m; c->lo[l + 1][ax] = 0; c->hi[l + 1][ax] = m - 1;
         c->hl[l + 1][ax] = P->box[ax] / (double)m;          /* reading B3 */
       } else {
-        c->lo[l + 1][ax] = iceil_div2(c->lo[l][ax] - hp);   /* reading G3 */
-        c->hi[l + 1][ax] = ifloor_div2(c->hi[l][ax] + hp);
+        c->lo[l + 1][ax] = iceil_div2(c->lo[l][ax] - hp) - P->pad;   /* reading G3 */
+        c->hi[l + 1][ax] = ifloor_div2(c->hi[l][ax] + hp) + P->pad;
         c->M[l + 1][ax] = c->hi[l + 1][ax] - c->lo[l + 1][ax] + 1;
         c->hl[l + 1][ax] = 2.0 * c->hl[l][ax];
       }
@@ -323,7 +326,7 @@ msmo_ctx *msmo_create(const msmo_params *prm, int *status) {
   msmo_ctx *c = (msmo_ctx *)calloc(1, sizeof(msmo_ctx));
   c->prm = *prm;
   int st = 0;
-  if (prm->p < 2 || prm->p > MSMO_MAXP || (prm->p & 1) || prm->h <= 0 || prm->a <= 0 || prm->mu < 0) st = 3;
+  if (prm->p < 2 || prm->p > MSMO_MAXP || (prm->p & 1) || prm->h <= 0 || prm->a <= 0 || prm->mu < 0 || prm->pad < 0) st = 3;
   for (int ax = 0; ax < 3 && !st; ++ax) {
     if (prm->box[ax] <= 0) st = 3;
     if (prm->periodic[ax] && prm->a > 0.5 * prm->box[ax]) st = 4;   /* minimum image */

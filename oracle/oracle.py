@@ -18,7 +18,7 @@ _lib = None
 
 class _Params(C.Structure):
     _fields_ = [("box", C.c_double * 3), ("periodic", C.c_int * 3), ("h", C.c_double),
-                ("a", C.c_double), ("p", C.c_int), ("levels", C.c_int), ("mu", C.c_int)]
+                ("a", C.c_double), ("p", C.c_int), ("levels", C.c_int), ("mu", C.c_int), ("pad", C.c_int)]
 
 
 def build(force: bool = False) -> str:
@@ -104,8 +104,11 @@ def direct_sum(pos, q, box=(1.0, 1.0, 1.0), periodic=(0, 0, 0), nimg=0, want_fv=
 class Oracle:
     """One MSM setup (the analogue of msm_plan_create on the CUDA side)."""
 
-    def __init__(self, box, periodic, h, a, p, levels, mu=4):
+    def __init__(self, box, periodic, h, a, p, levels, mu=4, pad=0):
+        """pad: extra grid nodes on both sides of every open axis at every level (the pin of
+        reading G3: no output may depend on it beyond round-off)."""
         prm = _Params()
+        prm.pad = int(pad)
         prm.box[:] = [float(b) for b in box]
         prm.periodic[:] = [int(b) for b in periodic]
         prm.h, prm.a, prm.p, prm.levels, prm.mu = float(h), float(a), int(p), int(levels), int(mu)

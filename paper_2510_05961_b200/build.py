@@ -10,13 +10,15 @@ CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libmsm_b200.so")
 SOURCES = ["msm_create.cu", "msm_evaluate.cu", "microbench.cu", "plan_math.cpp", "plan_top.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "--use_fast_math=false" if False else "-Xcompiler", "-fPIC", "-shared"]
+              "-Xcompiler", "-fPIC", "-shared"]
 
 
 def _stale() -> bool:
     if not os.path.exists(SO):
         return True
     t = os.path.getmtime(SO)
+    if os.path.getmtime(os.path.abspath(__file__)) > t:
+        return True
     for root in (CSRC, os.path.join(os.path.dirname(HERE), "include")):
         for f in os.listdir(root):
             if os.path.getmtime(os.path.join(root, f)) > t:
@@ -28,8 +30,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return SO
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-           "-Xcompiler", "-fPIC", "-shared", "-o", SO] + [os.path.join(CSRC, s) for s in SOURCES]
+    cmd = [nvcc] + NVCC_FLAGS + ["-o", SO] + [os.path.join(CSRC, s) for s in SOURCES]
     if verbose:
         cmd.insert(1, "-Xptxas"); cmd.insert(2, "-v")
     subprocess.check_call(cmd)

@@ -152,7 +152,7 @@ Hierarchy::Hierarchy(const Params& P) : prm(P), hp(P.p / 2), L(0), n_per(0), w(0
   if (n_per == 1) { status = 2; return; }  // reading T4
   top = n_per == 0 ? kTopOpen : (n_per == 3 ? kTopPeriodic : kTopSlab);
   Level l1;
-  int maxM = 1, minM = 1 << 30;
+  int maxM = 1;
   for (int ax = 0; ax < 3; ++ax) {
     if (P.periodic[ax]) {
       int e = (int)std::lround(std::log2(P.box[ax] / P.h));  // reading G1
@@ -161,7 +161,6 @@ Hierarchy::Hierarchy(const Params& P) : prm(P), hp(P.p / 2), L(0), n_per(0), w(0
       l1.lo[ax] = 0;
       l1.h[ax] = P.box[ax] / l1.M[ax];
       maxM = std::max(maxM, l1.M[ax]);
-      minM = std::min(minM, l1.M[ax]);
     } else {
       open_axis = ax;
       l1.lo[ax] = -(hp - 1);  // reading G2
@@ -170,7 +169,8 @@ Hierarchy::Hierarchy(const Params& P) : prm(P), hp(P.p / 2), L(0), n_per(0), w(0
       l1.h[ax] = P.h;
     }
   }
-  if (n_per > 0 && minM != maxM) { status = 2; return; }  // reading B3: rejected by this build
+  // reading B3: periodic axes may start from different grid counts; an axis that has reached one
+  // point keeps it (spacing = box edge) while the others go on halving
   if (n_per == 0) L = P.levels;
   else { L = 1; while ((1 << (L - 1)) < maxM) ++L; }  // until one point per periodic axis
   if (L > kMaxLevels) { status = 3; return; }

@@ -2,11 +2,13 @@
 CPU oracle on the same seeded inputs and compare element by element.
 
 Tolerances (BASELINE.json north_star): fp64 1e-10 relative; fp32 mode 1e-5 on the energy and 1e-4
-RMS on the forces. "Relative" is taken against the natural scale of each output (DESIGN.md
-"Tolerances"): |U| for the energy, max|V| for potentials, reading F1's scale for forces (max of
-the largest force and the largest single pair force, so that a perfect crystal with F = 0 is not
-divided by zero), max|Q| / max|E| for grids (not below one particle's charge, resp. its potential
-at the cutoff), max(|W|, |U|) for the virial.
+RMS on the forces. The fp32 outputs the north star does not bound are held to the bounds DESIGN.md
+section 3 derives from the arithmetic (FP32_BOUNDS, each within 5x of the worst value measured on
+the B200 over all fp32 cases). "Relative" is taken against the natural scale of each output
+(DESIGN.md "Tolerances"): |U| for the energy, max|V| for potentials, reading F1's scale for forces
+(max of the largest force and the largest single pair force, so that a perfect crystal with F = 0
+is not divided by zero), max|Q| / max|E| for grids (not below one particle's charge, resp. its
+potential at the cutoff), max(|W|, |U|) for the virial.
 """
 from __future__ import annotations
 
@@ -15,6 +17,9 @@ import numpy as np
 FP64_RTOL = 1e-10
 FP32_ENERGY_RTOL = 1e-5
 FP32_FORCE_RMS_RTOL = 1e-4
+# fp32 mode, outputs without a north-star bound (DESIGN.md section 3 "Tolerances"): key -> bound;
+# "Q" / "E" apply to the grids of every tiled level
+FP32_BOUNDS = {"force_rms": 2e-5, "force_max": 4e-5, "potential_max": 2e-5, "virial": 1e-5, "Q": 6e-6, "E": 3e-4}
 
 
 def run_oracle(w, mu=4, want_virial=True):
@@ -80,10 +85,11 @@ def compare(w, gpu, ref, precision="fp64", check_grids=True):
     else:
         assert out["energy"] <= FP32_ENERGY_RTOL, f"{w.name}: fp32 energy {out}"
         assert out["force_rms"] <= FP32_FORCE_RMS_RTOL, f"{w.name}: fp32 force rms {out}"
-        # the other outputs have no stated fp32 bound; DESIGN.md "Tolerances" derives 1e-3 of scale
         for k, v in out.items():
-            if k not in ("energy", "force_rms"):
-                assert v <= 1e-3, f"{w.name}: fp32 {k} {v:.3e} ({out})"
+            if k == "energy":
+                continue
+            bound = FP32_BOUNDS[k[0] if k[0] in "QE" and k[1:].isdigit() else k]
+            assert v <= bound, f"{w.name}: fp32 {k} {v:.3e} > {bound:g} ({out})"
     return out
 
 

@@ -201,6 +201,60 @@ def test_omega_converges_to_exact_interpolation(p):
 
 
 def test_omega_known_shortest_sequences():
-    # mu = 0: the shortest order-preserving sequences; p=4 is the classical [-1/3, 5/3, -1/3] hmm
-    # derived independently: (1 + t/6)^-2 = 1 - t/3 + O(t^2), t = delta^2 -> [ -1/3, 1 + 2/3, -1/3 ]
+    # mu = 0, p = 4: (1 + t/6)^-2 = 1 - t/3 + O(t^2) with t = delta^2 = [1, -2, 1]
+    #   -> [-1/3, 1 + 2/3, -1/3]
     assert oracle.omega(4, 0) == pytest.approx([-1 / 3, 5 / 3, -1 / 3], abs=1e-15)
+
+
+@pytest.mark.parametrize("key,p,mu", [("p4_mu0", 4, 0), ("p6_mu0", 6, 0), ("p4_mu4", 4, 4), ("p6_mu4", 6, 4)])
+def test_omega_exact_rationals(golden, key, p, mu):
+    """Reading Q with mu > 0: polynomial reproduction only constrains the first p/2 series terms, so
+    the extra mu terms are pinned by the exact rationals of SURVEY.md Appendix A (computed
+    symbolically, independent of the oracle)."""
+    from fractions import Fraction
+    ref = [float(Fraction(a, b)) for a, b in golden["omega_prime"][key]]
+    w = oracle.omega(p, mu)
+    hw = len(w) // 2
+    assert hw == p // 2 - 1 + mu == len(ref) - 1
+    assert w[hw:] == pytest.approx(ref, rel=1e-13, abs=1e-16)
+    assert w[:hw + 1][::-1] == pytest.approx(ref, rel=1e-13, abs=1e-16)
+
+
+@pytest.mark.parametrize("p", [4, 6])
+def test_omega_is_the_truncated_series_of_the_inverse_squared_symbol(golden, p):
+    """The stored series coefficients c_k satisfy (sum_k c_k t^k) * Phi_hat(t)^2 = 1 + O(t^(w+1)) in exact
+    rational arithmetic, with Phi_hat the symbol of the sampled spline in t = delta^2 built here from
+    the textbook integer values of the B-spline; and omega'(mu) - omega'(mu-1) is exactly
+    c_w (z - 2 + 1/z)^w, i.e. the alternating binomial row scaled by c_w."""
+    from fractions import Fraction
+    from math import comb
+    cs = [Fraction(a, b) for a, b in golden["omega_prime"][f"series_p{p}"]]
+    phi = [Fraction(a, b) for a, b in golden["bspline_at_integers"][str(p)]]      # Phi(-hp+1 .. hp-1)
+    hp = p // 2
+    # symbol in powers of t: Phi_hat(z) = sum_n Phi(n) z^n with z + 1/z = t + 2; Chebyshev-like recursion
+    # z^n + z^-n = T_n(t): T_0 = 2, T_1 = t + 2, T_n = (t + 2) T_{n-1} - T_{n-2}
+    def polymul(a, b):
+        out = [Fraction(0)] * (len(a) + len(b) - 1)
+        for i, x in enumerate(a):
+            for j, y in enumerate(b):
+                out[i + j] += x * y
+        return out
+    T = [[Fraction(2)], [Fraction(2), Fraction(1)]]
+    for n in range(2, hp):
+        nxt = polymul([Fraction(2), Fraction(1)], T[-1])
+        prev = T[-2] + [Fraction(0)] * (len(nxt) - len(T[-2]))
+        T.append([x - y for x, y in zip(nxt, prev)])
+    sym = [Fraction(0)] * hp
+    sym[0] += phi[hp - 1]
+    for n in range(1, hp):
+        for k, c in enumerate(T[n]):
+            sym[k] += phi[hp - 1 + n] * c
+    sq = polymul(sym, sym)
+    prod = polymul(cs, sq)
+    assert prod[0] == 1 and all(v == 0 for v in prod[1:len(cs)])
+    for mu in range(1, len(cs) - hp + 1):
+        w = hp - 1 + mu
+        full = oracle.omega(p, mu).copy()
+        full[1:-1] -= oracle.omega(p, mu - 1)
+        row = np.array([float(cs[w]) * (-1) ** (w - abs(n)) * comb(2 * w, w + n) for n in range(-w, w + 1)])
+        assert full == pytest.approx(row, rel=1e-12, abs=1e-15)

@@ -412,3 +412,96 @@ def test_open_levels_change_only_msm_error_and_periodic_ignores_levels():
     e1 = Oracle(box, (1, 1, 1), 1.5, 4.0, 4, 1).evaluate(pos, q, False)["energy"]
     e3 = Oracle(box, (1, 1, 1), 1.5, 4.0, 4, 3).evaluate(pos, q, False)["energy"]
     assert e1 == e3                                           # reading G4
+
+
+# ---------------------------------------------------------------- virial: all six components
+
+PERM_XY = [1, 0, 2, 3, 5, 4]      # components xx yy zz xy xz yz after swapping x and y
+PERM_YZ = [0, 2, 1, 4, 3, 5]      # after swapping y and z
+
+
+@pytest.mark.parametrize("periodic,box", [((1, 1, 1), (12.0, 12.0, 12.0)), ((1, 1, 1), (12.0, 13.0, 14.0)),
+                                          ((1, 1, 0), (12.0, 12.0, 7.0)), ((1, 1, 0), (12.0, 13.0, 7.0))])
+def test_virial_axis_swap_equivariance(periodic, box):
+    """Relabelling two axes (positions, box edges and periodicity flags together) permutes the six
+    virial components and leaves the energy unchanged, to round-off: no component of reading V
+    (pair term, D^l_ab stencils, T3 top level) is attached to the wrong axis, under full and mixed
+    periodicity."""
+    pos, q, _ = small_system(periodic, n=50, seed=23, box=box)
+    h, a, p = 1.5, 4.0, 4
+    r = Oracle(box, periodic, h, a, p, 2).evaluate(pos, q)
+    for cols, perm in (([1, 0, 2], PERM_XY), ([0, 2, 1], PERM_YZ)):
+        b2 = tuple(box[c] for c in cols)
+        per2 = tuple(periodic[c] for c in cols)
+        r2 = Oracle(b2, per2, h, a, p, 2).evaluate(np.ascontiguousarray(pos[:, cols]), q)
+        assert r2["energy"] == pytest.approx(r["energy"], rel=1e-11)
+        assert r2["virial"][perm] == pytest.approx(r["virial"], rel=1e-9, abs=1e-9 * np.abs(r["virial"]).max())
+        assert r2["forces"][:, cols] == pytest.approx(r["forces"], rel=1e-9, abs=1e-10)
+
+
+def _rotated_supercell(pos, q, L, Lz):
+    """The same infinite x-y-periodic system described in the cell spanned by (L, L, 0) and
+    (-L, L, 0): edges sqrt(2) L, twice the particles, axes rotated by +45 degrees about z."""
+    s = 1.0 / np.sqrt(2.0)
+    both = np.concatenate([pos, pos + np.array([L, 0.0, 0.0])])
+    xr = s * (both[:, 0] + both[:, 1])
+    yr = s * (-both[:, 0] + both[:, 1])
+    e = np.sqrt(2.0) * L
+    out = np.stack([xr - e * np.floor(xr / e), yr - e * np.floor(yr / e), both[:, 2]], axis=1)
+    return out, np.concatenate([q, q]), (e, e, Lz)
+
+
+@pytest.mark.parametrize("periodic,Lz", [((1, 1, 1), 10.0), ((1, 1, 0), 6.0)])
+def test_virial_offdiagonal_magnitude_from_rotated_cell(periodic, Lz):
+    """Magnitude (not only sign and index order) of the off-diagonal virial under periodicity: the
+    same infinite system in a cell rotated by 45 degrees about z has, for the exact energy,
+    W'_xx - W'_yy = 2 W_xy, W'_xy = (W_yy - W_xx)/2, W'_xx + W'_yy = W_xx + W_yy per original cell.
+    The diagonal components are pinned by finite differences of the energy
+    (test_virial_is_strain_derivative_per_axis), so this pins W_xy against them, within MSM error
+    (the two grids differ). x<->y, y<->z equivariance (above) carries it to xz and yz."""
+    L = 10.0
+    rng = np.random.default_rng(31)
+    n = 36
+    pos = rng.random((n, 3)) * np.array([L, L, Lz])
+    q = rng.uniform(-1, 1, n); q -= q.mean()
+    h, a, p = 0.7, 5.0, 6                                    # grids 16 x 16 (h = 0.625) and 16 x 16 (h = 0.884)
+    r = Oracle((L, L, Lz), periodic, h, a, p, 1).evaluate(pos, q)
+    pos2, q2, box2 = _rotated_supercell(pos, q, L, Lz)
+    r2 = Oracle(box2, periodic, h, a, p, 1).evaluate(pos2, q2)
+    W, W2 = r["virial"], 0.5 * r2["virial"]                  # per original cell
+    assert 0.5 * r2["energy"] == pytest.approx(r["energy"], rel=4e-4)
+    scale = np.abs(W).max()
+    assert abs(W[3]) > 0.02 * scale                          # the pinned component is not accidentally tiny
+    tol = 1.5e-3 * scale                                     # measured <= 4.4e-4; W_xy itself is 0.05 - 0.13 of scale
+    assert 0.5 * (W2[0] - W2[1]) == pytest.approx(W[3], abs=tol)
+    assert W2[3] == pytest.approx(0.5 * (W[1] - W[0]), abs=tol)
+    assert W2[0] + W2[1] == pytest.approx(W[0] + W[1], abs=tol)
+    assert W2[2] == pytest.approx(W[2], abs=tol)
+    s = 1.0 / np.sqrt(2.0)
+    assert s * (W2[4] - W2[5]) == pytest.approx(W[4], abs=tol)      # (xz, yz) rotate as a vector
+    assert s * (W2[4] + W2[5]) == pytest.approx(W[5], abs=tol)
+
+
+# ---------------------------------------------------------------- reading G3's own pin
+
+@pytest.mark.parametrize("periodic,box,levels", [((0, 0, 0), (11.0, 9.5, 10.2), 3), ((1, 1, 0), (12.0, 12.0, 7.3), 1)])
+def test_extra_padding_nodes_change_nothing(periodic, box, levels):
+    """Reading G3 (open-axis extents lo' = ceil((lo - p/2)/2), hi' = floor((hi + p/2)/2)) claims to be
+    the smallest ranges for which restriction loses no charge and prolongation reaches every fine
+    node. Its pin: extra nodes on both sides of every open axis at every level leave every output
+    unchanged to round-off."""
+    pos, q, _ = small_system(periodic, n=45, seed=5, box=box)
+    pos[0] = 0.0                                              # particles on the open faces
+    pos[1] = np.array(box)
+    if periodic[0]:
+        pos[1, :2] = 0.3
+    base = Oracle(box, periodic, 1.3, 3.5, 4, levels).evaluate(pos, q)
+    for pad in (1, 3):
+        o = Oracle(box, periodic, 1.3, 3.5, 4, levels, pad=pad)
+        r = o.evaluate(pos, q)
+        ax = periodic.index(0)
+        assert o.level_info(1)["M"][ax] == Oracle(box, periodic, 1.3, 3.5, 4, levels).level_info(1)["M"][ax] + 2 * pad
+        assert r["energy"] == pytest.approx(base["energy"], rel=1e-12)
+        assert r["forces"] == pytest.approx(base["forces"], rel=1e-10, abs=1e-12)
+        assert r["potentials"] == pytest.approx(base["potentials"], rel=1e-10, abs=1e-12)
+        assert r["virial"] == pytest.approx(base["virial"], rel=1e-10, abs=1e-11)
