@@ -79,12 +79,18 @@ class ClockSampler:
 
     def stop(self):
         if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+            return
         self.proc.terminate()
         try:
             self.proc.wait(timeout=5)
         except Exception:
             self.proc.kill()
+
+    def snapshot(self):
+        """Clocks and throttle reasons of the samples since the last mark()."""
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
         sm, mx, reasons = [], [], set()
         for r in self.rows[min(self.first, max(len(self.rows) - 1, 0)):]:
             try:
@@ -174,20 +180,31 @@ def whole_job_value(world: int, particles: int, steps: int, ms_total: float) -> 
     return world * particles * steps / (ms_total * 1e-3)
 
 
-def run_ours(args, rank: int, world: int):
-    import numpy as np
+def stored_traffic(kernel: str, workload: str, dtype: str):
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full`
+    capture) of the stage's kernel on this workload, from profiles/r2_dram_traffic.csv; None if
+    that kernel / workload pair was not captured."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")) as f:
+            for line in f:
+                c = [x.strip() for x in line.split(",")]
+                if len(c) >= 4 and c[0] == kernel and c[1] == workload and c[2] == dtype:
+                    return float(c[3])
+    except Exception:
+        pass
+    return None
+
+
+def measure(w, prec, local, dev, steps, warmup, world, flush, sampler=None, full=True):
+    """One workload in one precision -> dict(value, ms_per_step, stages, roofline, e2e, ...).
+
+    Three timed regions of `steps` evaluations each, all bracketed the same way (L2 flush outside
+    the per-step CUDA-event pair, synchronize on both sides): (1) per-stage event records on (one
+    stream, serial) -> `stages` / `roofline`; (2) records off: the library replays its CUDA graph
+    with the pair and virial kernels beside the grid pipeline -> `value`; (3) host buffers through
+    msm_evaluate_host -> `e2e`. full=False runs (2) only (the sweep points)."""
     import torch
     from paper_2510_05961_b200 import msm
-    from paper_2510_05961_b200.workloads import make_workload
-
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
-    w = make_workload(args.workload)
-    prec = w.precision
     esz = 4 if prec == "fp32" else 8
     plan = msm.Plan.for_workload(w, prec, device=local)
     dt = plan.torch_dtype
@@ -195,7 +212,6 @@ def run_ours(args, rank: int, world: int):
     q = torch.tensor(w.charges, dtype=dt, device=dev).contiguous()
     F = torch.zeros((w.n, 3), dtype=dt, device=dev)
     V = torch.zeros(w.n, dtype=dt, device=dev)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
     def barrier():
         if world > 1:
@@ -203,92 +219,78 @@ def run_ours(args, rank: int, world: int):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident arm, profiled pass (stage times for the roofline)
-    plan.set_profiling(True)          # one cudaEventRecord between stages: per-stage times, live
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    for _ in range(args.warmup):
-        plan.evaluate(pos, q, F, V)
-    if rank == 0:
-        sampler.mark()                # only samples taken from here on (the timed region) count
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    stage_sum, launches, energy = {}, 0, 0.0
-    barrier()
-    for s in range(args.steps):
-        flush.fill_(s & 0xFF)                               # L2 flush, outside the event pair
-        ev[s][0].record()
-        energy, _ = plan.evaluate(pos, q, F, V)             # energy + forces + potentials + virial
-        ev[s][1].record()
-        torch.cuda.synchronize()
-        for k, v in plan.stage_times().items():
-            stage_sum[k] = stage_sum.get(k, 0.0) + v
-        launches += plan.launch_count()
-    barrier()
-    ms_total = sum(a.elapsed_time(b) for a, b in ev)
+    def timed(fn, per_step=None):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        barrier()
+        for s in range(steps):
+            flush.fill_(s & 0xFF)                               # L2 flush, outside the event pair
+            ev[s][0].record()
+            fn()
+            ev[s][1].record()
+            torch.cuda.synchronize()
+            if per_step:
+                per_step()
+        barrier()
+        return sum(a.elapsed_time(b) for a, b in ev)
 
-    # ---- the timed steps of `value`: per-stage event records off, so the library replays its CUDA
-    # graph with the pair and virial kernels on their own streams beside the grid pipeline (the
-    # per-stage times above need one stream). Same K steps, same flush, same event bracketing.
+    res = {"particles": w.n, "dtype": "f32" if prec == "fp32" else "f64"}
+    stage_sum, launches, energy = {}, [0], [0.0]
+    if full:
+        plan.set_profiling(True)          # one cudaEventRecord between stages: per-stage times, live
+        for _ in range(warmup):
+            plan.evaluate(pos, q, F, V)
+        if sampler:
+            sampler.mark()                # only samples taken from here on (the timed regions) count
+
+        def collect():
+            for k, v in plan.stage_times().items():
+                stage_sum[k] = stage_sum.get(k, 0.0) + v
+            launches[0] += plan.launch_count()
+
+        def step():
+            energy[0], _ = plan.evaluate(pos, q, F, V)          # energy + forces + potentials + virial
+        ms_prof = timed(step, collect)
     plan.set_profiling(False)
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         plan.evaluate(pos, q, F, V)
-    barrier()
-    ev4 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    for s in range(args.steps):
-        flush.fill_(s & 0xFF)
-        ev4[s][0].record()
-        plan.evaluate(pos, q, F, V)
-        ev4[s][1].record()
-        torch.cuda.synchronize()
-    barrier()
-    ms_fast = sum(a.elapsed_time(b) for a, b in ev4)
-    clocks = sampler.stop() if rank == 0 else None      # sampled over the profiled and the timed steps
+    if sampler and not full:
+        sampler.mark()
+    ms_fast = timed(lambda: plan.evaluate(pos, q, F, V))
+    if not full:
+        ms_fast, _ = max_over_ranks(ms_fast, 0.0, world, dev)
+        res.update({"value": whole_job_value(world, w.n, steps, ms_fast), "ms_per_step": ms_fast / steps,
+                    "grids": [list(plan.info.grid_dims[i]) for i in range(plan.info.n_tiled)],
+                    "h": float(plan.info.grid_h[0][0]),
+                    "grid_points_per_particle": float(np_prod(plan.info.grid_dims[0])) / w.n})
+        plan.close()
+        return res
+    clocks = sampler.snapshot() if sampler else None
 
     # ---- end-to-end arm: host buffers through msm_evaluate_host, copies inside the timed region
     hpos = torch.tensor(w.positions, dtype=dt).pin_memory()
     hq = torch.tensor(w.charges, dtype=dt).pin_memory()
     hF = torch.zeros((w.n, 3), dtype=dt).pin_memory()
     hV = torch.zeros(w.n, dtype=dt).pin_memory()
-    for _ in range(max(1, args.warmup)):
+    for _ in range(max(1, min(warmup, 3))):
         plan.evaluate_host(hpos, hq, hF, hV)
-    ev2 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    barrier()
-    for s in range(args.steps):
-        flush.fill_(s & 0xFF)
-        ev2[s][0].record()
-        plan.evaluate_host(hpos, hq, hF, hV)
-        ev2[s][1].record()
-        torch.cuda.synchronize()
-    barrier()
-    ms_e2e = sum(a.elapsed_time(b) for a, b in ev2)
+    ms_e2e = timed(lambda: plan.evaluate_host(hpos, hq, hF, hV))
 
     # ---- context: the same step without the virial (energy + forces + potentials only)
-    plan.set_profiling(False)
     for _ in range(3):
         plan.evaluate(pos, q, F, V, True, False)
-    ev3 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    for s in range(args.steps):
-        flush.fill_(s & 0xFF)
-        ev3[s][0].record()
-        plan.evaluate(pos, q, F, V, True, False)
-        ev3[s][1].record()
-        torch.cuda.synchronize()
-    ms_nov = sum(a.elapsed_time(b) for a, b in ev3)
+    ms_nov = timed(lambda: plan.evaluate(pos, q, F, V, True, False))
 
-    ms_total, ms_e2e = max_over_ranks(ms_total, ms_e2e, world, dev)
+    ms_prof, ms_e2e = max_over_ranks(ms_prof, ms_e2e, world, dev)
     ms_fast, _ = max_over_ranks(ms_fast, 0.0, world, dev)
-    if rank != 0:
-        return None
 
     peaks, peak_src = load_peaks()
-    dtype = "f32" if prec == "fp32" else "f64"
+    dtype = res["dtype"]
     alu_peak = derived_alu_peak_tflops(dtype)
     fma_meas = msm.measure_fma_peak(prec, local)
     pairs = count_pairs(w)
     stages = {}
     for k, v in stage_sum.items():
-        ms = v / args.steps
+        ms = v / steps
         kind, amount = stage_work(k, w, plan, esz, pairs)
         if kind == "flop":
             ach = amount / (ms * 1e-3) * 1e-12 if ms > 0 else 0.0
@@ -300,38 +302,102 @@ def run_ours(args, rank: int, world: int):
                          "frac": round(ach / peaks["hbm_gbs"], 5)}
     dom = max(stages, key=lambda k: stages[k]["ms"])
     d = stages[dom]
-    roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"],
-                "peak": round(alu_peak, 2) if d["bound"] == "alu" else peaks["hbm_gbs"], "unit": d["unit"],
-                "frac": d["frac"], "traffic": None,
-                "peak_source": ("derived: 148 SM x %d lanes x 2 x 1.965 GHz" % (128 if dtype == "f32" else 64))
-                if d["bound"] == "alu" else f"{peak_src} MEASURED_PEAKS.json hbm_gbs",
-                "measured_fma_tflops": round(fma_meas, 2),
-                "share_of_step": round(d["ms"] / (ms_total / args.steps), 4),
-                "timed_in": "the profiled K steps (serial, one stream); see `profiled`"}
-    out = {
-        "metric": METRIC, "value": whole_job_value(world, w.n, args.steps, ms_fast), "unit": UNIT,
-        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_fast / args.steps,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
-        "config": {"workload": args.workload, "particles": w.n, "box": list(w.box), "periodic": list(w.periodic),
-                   "p": w.p, "h_target": w.h, "a": w.a, "levels": w.levels, "mu": int(plan.info.mu),
-                   "grids": [list(plan.info.grid_dims[i]) for i in range(plan.info.n_tiled)],
-                   "outputs": "energy+forces+potentials+virial", "parallelism": "replicas" if world > 1 else "1gpu",
-                   "l2": "256 MiB fill between steps (outside the per-step event pairs)"},
-        "e2e": {"value": whole_job_value(world, w.n, args.steps, ms_e2e), "unit": UNIT,
+    res.update({
+        "value": whole_job_value(world, w.n, steps, ms_fast), "ms_per_step": ms_fast / steps,
+        "e2e": {"value": whole_job_value(world, w.n, steps, ms_e2e), "unit": UNIT,
                 "h2d_bytes_per_step": w.n * 4 * esz, "d2h_bytes_per_step": w.n * 4 * esz + 64,
-                "ms_per_step": ms_e2e / args.steps},
-        "profiled": {"value": whole_job_value(world, w.n, args.steps, ms_total), "unit": UNIT,
-                     "ms_per_step": ms_total / args.steps,
+                "ms_per_step": ms_e2e / steps},
+        "profiled": {"value": whole_job_value(world, w.n, steps, ms_prof), "unit": UNIT,
+                     "ms_per_step": ms_prof / steps,
                      "note": "the same K steps with per-stage CUDA-event records, timed the same way just before the "
                              "`value` steps; the library then keeps every kernel on one stream (no pair/virial "
                              "overlap); `stages` and `roofline` come from these steps"},
-        "without_virial": {"value": w.n * args.steps / (ms_nov * 1e-3), "unit": UNIT, "ms_per_step": ms_nov / args.steps,
+        "without_virial": {"value": w.n * steps / (ms_nov * 1e-3), "unit": UNIT, "ms_per_step": ms_nov / steps,
                            "note": "rank 0, energy+forces+potentials only; context, not the metric"},
-        "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "stages": stages,
-        "energy": energy,
+        "roofline": {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"],
+                     "peak": round(alu_peak, 2) if d["bound"] == "alu" else peaks["hbm_gbs"], "unit": d["unit"],
+                     "frac": d["frac"], "traffic": stored_traffic(dom, w.name, dtype),
+                     "traffic_unit": "DRAM bytes per launch, ncu --set full (profiles/r2_dram_traffic.csv)",
+                     "algorithmic": stage_work(dom, w, plan, esz, pairs)[1],
+                     "algorithmic_unit": "flop per launch" if d["bound"] == "alu" else "bytes per launch",
+                     "peak_source": ("derived: 148 SM x %d lanes x 2 x 1.965 GHz" % (128 if dtype == "f32" else 64))
+                     if d["bound"] == "alu" else f"{peak_src} MEASURED_PEAKS.json hbm_gbs",
+                     "measured_fma_tflops": round(fma_meas, 2),
+                     "share_of_step": round(d["ms"] / (ms_prof / steps), 4),
+                     "timed_in": "the profiled K steps (serial, one stream); see `profiled`"},
+        "stages": stages, "gpu_launches": launches[0], "energy": energy[0], "clocks": clocks,
+        "grids": [list(plan.info.grid_dims[i]) for i in range(plan.info.n_tiled)], "mu": int(plan.info.mu),
+    })
+    plan.close()
+    return res
+
+
+def np_prod(v):
+    r = 1
+    for x in v:
+        r *= int(x)
+    return r
+
+
+def run_ours(args, rank: int, world: int):
+    import torch
+    from paper_2510_05961_b200.workloads import BASELINE_SWEEP, COMMENSURATE_SERIES, make_workload
+
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+    w = make_workload(args.workload)
+    m = measure(w, w.precision, local, dev, args.steps, args.warmup, world, flush, sampler)
+    extras = world == 1 and not args.main_only and args.workload == "cfg4_water1m"
+    fp64, sweep = None, None
+    if extras:
+        # the other half of the metric ("fp64, fp32"): the fp64 config 5 and the timed workload in fp64
+        k = max(5, args.steps // 2)
+        fp64 = {}
+        w5 = make_workload("cfg5_slab100k")
+        fp64["cfg5_slab100k"] = measure(w5, "fp64", local, dev, k, args.warmup, world, flush, sampler)
+        fp64["cfg4_water1m"] = measure(w, "fp64", local, dev, k, args.warmup, world, flush, sampler)
+        # time per evaluation vs N: the four BASELINE points and the commensurate h = 2.09 series
+        sweep = {"note": "ms per evaluation (fp32, all outputs, graph replay), L2 flushed between steps; "
+                         "BASELINE points have h = 1.94 / 2.09 / 2.25 / 1.68 (power-of-two grids, reading G1), "
+                         "the commensurate series has h = 2.09 at every N",
+                 "baseline_points": [], "commensurate_h2.09": []}
+        for key, names in (("baseline_points", BASELINE_SWEEP), ("commensurate_h2.09", COMMENSURATE_SERIES)):
+            for name in names:
+                ws = w if name == args.workload else make_workload(name)
+                r = measure(ws, "fp32", local, dev, k, args.warmup, world, flush, None, full=False)
+                r["workload"] = name
+                sweep[key].append(r)
+                del ws
+    if sampler:
+        sampler.stop()
+    if rank != 0:
+        return None
+    out = {
+        "metric": METRIC, "value": m["value"], "unit": UNIT,
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": m["ms_per_step"],
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": m["dtype"], "data": "synthetic",
+        "config": {"workload": args.workload, "particles": w.n, "box": list(w.box), "periodic": list(w.periodic),
+                   "p": w.p, "h_target": w.h, "a": w.a, "levels": w.levels, "mu": m["mu"], "grids": m["grids"],
+                   "outputs": "energy+forces+potentials+virial", "parallelism": "replicas" if world > 1 else "1gpu",
+                   "l2": "256 MiB fill between steps (outside the per-step event pairs)"},
+        "e2e": m["e2e"], "profiled": m["profiled"], "without_virial": m["without_virial"],
+        "gpu_launches": m["gpu_launches"], "clocks": m["clocks"], "roofline": m["roofline"], "stages": m["stages"],
+        "energy": m["energy"],
     }
+    if fp64:
+        out["fp64"] = fp64
+    if sweep:
+        out["sweep"] = sweep
     if world == 1 and args.grid_microbench > 0:
-        plan.close()
+        peaks, _ = load_peaks()
         out["grid_microbench"] = grid_microbench(args.grid_microbench, local, peaks["hbm_gbs"])
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.workload, 1, 0)[0]
@@ -381,8 +447,10 @@ def grid_microbench(M: int, local: int, hbm_gbs: float):
 
 
 # The oracle's bounded sample of each workload: same recipe, density and plan parameters, fewer
-# particles where the full case would take minutes on the host (about 10-30 s of CPU work).
-CPU_SAMPLE = {"cfg4_water1m": "cfg4_water300k"}
+# particles where the full case would take minutes on the host (the whole 10^6 case is one to two
+# minutes per evaluation; every other workload is timed whole).
+CPU_SAMPLE = {"cfg4_water1m": "cfg4_water300k", "cfg4_water1m_fp64": "cfg4_water300k",
+              "cfg4c_water1920k": "cfg4c_water240k"}
 
 
 def cpu_baseline(workload: str, steps: int, warmup: int):
@@ -405,7 +473,7 @@ def cpu_baseline(workload: str, steps: int, warmup: int):
         f"{sample}: {w.n} particles of the same recipe, density and plan parameters"
     return {"value": w.n * steps / total, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{note}; one full oracle evaluation (fp64, all outputs) per step",
-            "seconds_per_step": total / steps}, w
+            "sample_particles": w.n, "seconds_per_step": total / steps}, w
 
 
 def run_reference(args, rank: int):
@@ -429,6 +497,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4_water1m")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--main-only", action="store_true",
+                    help="skip the fp64 objects and the N sweep of the default run")
     ap.add_argument("--grid-microbench", type=int, default=512,
                     help="finest grid size M (power of two) of the HBM-bound grid-stage measurement; 0 skips it")
     ap.add_argument("--only-grid-microbench", action="store_true", help="print the grid_microbench object alone")

@@ -289,6 +289,8 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   p->pieces = new SplinePieces(prm->p);
 
   if (cudaSetDevice(prm->device) != cudaSuccess) return MSM_ERR_CUDA;
+  if (cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, prm->device) != cudaSuccess || p->sm_count < 1)
+    return MSM_ERR_CUDA;
 
   // ---- grids
   // slices per output tile of the convolution: enough one-warp units for ~3 resident waves
@@ -297,7 +299,7 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
     long long tiles = 0;
     for (int l = 1; l < p->n_t; ++l)
       tiles += (long long)((H.lev[l].M[0] + XTc - 1) / XTc) * ((H.lev[l].M[1] + 31) / 32) * ((H.lev[l].M[2] + 3) / 4);
-    const long long target = 148LL * 16 * 3;
+    const long long target = (long long)p->sm_count * 16 * 3;
     p->conv_slices = tiles > 0 ? (int)std::max<long long>(1, std::min<long long>(kMaxConvSlices, (target + tiles - 1) / tiles)) : 1;
     if (const char* e = std::getenv("MSM_CONV_SLICES")) p->conv_slices = std::max(1, std::atoi(e));
   }
@@ -402,12 +404,13 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   p->grec = dev_alloc(p, cap * 4 * p->esz);
   p->Fsr = dev_alloc(p, (size_t)kPairMaxSplit * cap * 3 * p->esz);   // per-split partials of the pair kernel
   p->Vsr = dev_alloc(p, (size_t)kPairMaxSplit * cap * p->esz);
-  p->pair_ymax = (int)((cap / 32 + p->pair_rows) / p->pair_rows + kPairWarps - 1) / kPairWarps + 1;
-  p->pair_wpart = (double*)dev_alloc(p, (size_t)p->pair_rows * p->pair_ymax * kPairMaxSplit * kPairWarps * 6 * sizeof(double));
+  const int pw = p->fp32 ? PairWarps<float>::value : PairWarps<double>::value;
+  p->pair_ymax = (int)((cap / kPairCluster + p->pair_rows) / p->pair_rows + pw - 1) / pw + 1;
+  p->pair_wpart = (double*)dev_alloc(p, (size_t)p->pair_rows * p->pair_ymax * kPairMaxSplit * pw * 6 * sizeof(double));
   p->n_eblocks = (int)((cap + 127) / 128);
   p->epart = (double*)dev_alloc(p, (size_t)p->n_eblocks * sizeof(double));
   {
-    const size_t rows = (size_t)p->pair_rows * p->pair_ymax * kPairMaxSplit * kPairWarps + p->conv.total_vunits + p->G + p->n_eblocks;
+    const size_t rows = (size_t)p->pair_rows * p->pair_ymax * kPairMaxSplit * pw + p->conv.total_vunits + p->G + p->n_eblocks;
     p->part_blocks = (int)(rows / 1024 + MSM_MAX_LEVELS + 8);
     p->part = (double*)dev_alloc(p, (size_t)p->part_blocks * 7 * sizeof(double));
   }

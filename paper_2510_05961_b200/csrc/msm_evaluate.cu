@@ -157,15 +157,16 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     // fp32 scan: exact cutoff in fp32 mode (the drain repeats the same arithmetic); in fp64 mode a
     // slack of 1e-4 relative covers the rounding of cell-relative coordinates (< 2^-24 * 8 edges)
     pp.a2_scan = sizeof(T) == 4 ? (float)(a * a) : (float)(a * a * (1.0 + 1e-4));
-    pp.a2 = (T)(a * a); pp.inv_a = (T)(1.0 / a); pp.inv_a2 = (T)(1.0 / (a * a)); pp.two_inv_a3 = (T)(2.0 / (a * a * a));
+    pp.a = (T)a; pp.a2 = (T)(a * a); pp.inv_a = (T)(1.0 / a); pp.inv_a2 = (T)(1.0 / (a * a)); pp.two_inv_a3 = (T)(2.0 / (a * a * a));
     for (int k = 0; k < 8; ++k) pp.c[k] = (T)p->S->c[k];
     pp.p = P;
-    // tiles of 32 particles per cell row, spread over gridDim.y blocks of kPairWarps warps
-    const int per_row = (n / 32 + p->pair_rows) / p->pair_rows;
+    // clusters of kPairCluster particles per cell row, spread over gridDim.y blocks of kPairWarps warps
+    constexpr int kPairWarps = PairWarps<T>::value;
+    const int per_row = (n / kPairCluster + p->pair_rows) / p->pair_rows;
     // few tiles (small systems): deal the dz planes of the neighbourhood to separate blocks
     const int nplanes = pp.omax[2] - pp.omin[2] + 1;
-    static const int split_tiles = std::getenv("MSM_PAIR_SPLIT_TILES") ? std::atoi(std::getenv("MSM_PAIR_SPLIT_TILES")) : 16384;
-    pp.nsplit = n / 32 < split_tiles ? std::min(nplanes, kPairMaxSplit) : 1;
+    // fewer clusters than ~16 warps per SM: deal the dz planes to separate blocks
+    pp.nsplit = n / kPairCluster < p->sm_count * 16 ? std::min(nplanes, kPairMaxSplit) : 1;
     pp.part_stride = (size_t)p->cap;
     p->pair_nsplit = pp.nsplit;
     const dim3 pgrid(p->pair_rows, std::max(1, std::min(p->pair_ymax, (per_row + kPairWarps - 1) / kPairWarps)),
@@ -239,8 +240,8 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     return sg;
   };
   // planes per block along the marching axis: enough blocks for ~8 per SM, at least min_planes each
-  auto stream_zseg = [](int columns, int nplanes, int min_planes) {
-    const int want = std::max(1, (148 * 8 + columns - 1) / columns);
+  auto stream_zseg = [&](int columns, int nplanes, int min_planes) {
+    const int want = std::max(1, (p->sm_count * 8 + columns - 1) / columns);
     return std::max(std::min(min_planes, nplanes), (nplanes + want - 1) / want);
   };
   for (int l = 1; l < p->n_t; ++l) {
@@ -309,7 +310,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
         // segments of planes: full waves of resident blocks against the 2 HW extra planes per segment
         auto launch = [&](auto kern, int minb, int ty, size_t sm) {
           const int ncols = fg.ntx * ((g.P[1] + ty - 1) / ty);
-          const int resident = 148 * minb, extra = Wt.n - 1;
+          const int resident = p->sm_count * minb, extra = Wt.n - 1;
           int best = 1; double best_eff = 0.0;
           for (int ns = 1; ns <= std::max(1, g.P[2] / 16); ++ns) {
             const long long nb = (long long)ncols * ns;
@@ -498,7 +499,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   // ---------------- S9 reductions
   if (want_virial) {
     Seg& s = fa.seg[nseg++];
-    s.ptr = p->pair_wpart; s.count = p->pair_blocks * kPairWarps; s.width = 6;
+    s.ptr = p->pair_wpart; s.count = p->pair_blocks * PairWarps<T>::value; s.width = 6;
     for (int k = 0; k < 6; ++k) s.scale[k] = 1.0;
   }
   {

@@ -46,6 +46,7 @@ struct msm_plan {
 
   std::vector<void*> allocs;
   size_t bytes = 0;
+  int sm_count = 148;        // cudaDevAttrMultiProcessorCount of the plan's device (148 on B200)
 
   msm::LevelDev lev[MSM_MAX_LEVELS + 1];
   void *tmpA = nullptr, *tmpB = nullptr;

@@ -168,11 +168,34 @@ def _water(name, n_molecules, seed, precision):
                     note="water-like periodic box, 1.0 g/cm^3")
 
 
+def _water_supercell(name, n_molecules_base, seed, reps, precision):
+    """A reps^3 supercell of a water box plus a small random rigid displacement of every molecule
+    (the way the paper builds its large systems): same density and plan parameters."""
+    pos, q, edge = water_box(n_molecules_base, seed)
+    rng = np.random.default_rng(seed + 1000)
+    shifts = np.stack(np.meshgrid(*[np.arange(reps)] * 3, indexing="ij"), axis=-1).reshape(-1, 3) * edge
+    big = (pos[None, :, :] + shifts[:, None, :]).reshape(-1, 3)
+    disp = rng.uniform(-0.05, 0.05, (big.shape[0] // 3, 3))
+    big = big + np.repeat(disp, 3, axis=0)
+    E = edge * reps
+    big -= E * np.floor(big / E)
+    big[big >= E] = 0.0
+    return Workload(name, big, np.tile(q, reps ** 3), (E,) * 3, (1, 1, 1), h=2.0, a=9.0, p=4,
+                    levels=_water_levels(E, 2.0), precision=precision,
+                    note="water-like periodic box, 1.0 g/cm^3, supercell")
+
+
+# The commensurate scaling series of SURVEY.md 8(d) config 4: identical h = 2.09 at every N
+# (box = 2^k * 33.44), so that linearity in N is not masked by the jumps of h that the power-of-two
+# grid counts (reading G1) cause at the BASELINE points.
+COMMENSURATE_SERIES = ["cfg4c_water3750", "cfg4c_water30k", "cfg4c_water240k", "cfg4c_water1920k"]
+BASELINE_SWEEP = ["cfg4_water3k", "cfg4_water30k", "cfg4_water300k", "cfg4_water1m"]
+
 WORKLOAD_NAMES = [
     "cfg1_open512", "cfg2_nacl4096", "cfg2_nacl4096_shifted", "cfg3_water30k_fp64",
     "cfg3_water30k_fp32", "cfg4_water3k", "cfg4_water30k", "cfg4_water300k", "cfg4_water1m",
-    "cfg5_slab100k",
-]
+    "cfg5_slab100k", "cfg4_water1m_fp64",
+] + COMMENSURATE_SERIES
 
 
 def make_workload(name: str) -> Workload:
@@ -198,6 +221,16 @@ def make_workload(name: str) -> Workload:
         return _water(name, 100000, 43, "fp32").as_precision("fp32")
     if name == "cfg4_water1m":
         return _water(name, 333333, 44, "fp32").as_precision("fp32")
+    if name == "cfg4_water1m_fp64":
+        return _water(name, 333333, 44, "fp64")
+    if name == "cfg4c_water3750":
+        return _water(name, 1250, 51, "fp32").as_precision("fp32")
+    if name == "cfg4c_water30k":
+        return _water(name, 10000, 52, "fp32").as_precision("fp32")
+    if name == "cfg4c_water240k":
+        return _water(name, 80000, 53, "fp32").as_precision("fp32")
+    if name == "cfg4c_water1920k":
+        return _water_supercell(name, 80000, 53, 2, "fp32").as_precision("fp32")
     if name == "cfg5_slab100k":
         pos, q = slab_random(100000, 100.0, 100.0, 40.0, 5)
         return Workload(name, pos, q, (100.0, 100.0, 40.0), (1, 1, 0), h=1.5, a=10.0, p=6,
