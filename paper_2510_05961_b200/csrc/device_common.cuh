@@ -84,9 +84,11 @@ __device__ __forceinline__ T spline_weight_row(const SplineTab<T, P>& tab, int j
 struct BinGeom {
   double box[3];
   int periodic[3];
-  // pair cells
+  // pair cells; along x every cell is cut into 2^sxs sub-bins (the sort key), so that a cell row
+  // is ordered by x finely enough for the pair kernel's windows
   int nc[3];
   double cell_edge[3];
+  int sxs;
   // level-1 grid cells (one per grid interval)
   int ng[3];        // number of grid cells per axis
   double h1[3];

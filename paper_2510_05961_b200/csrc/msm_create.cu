@@ -376,7 +376,11 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
     if (p->anterp_tiled)
       p->anterp_scratch = dev_alloc(p, (size_t)ntiles * p->at.split * p->at.D[0] * p->at.D[1] * p->at.D[2] * p->esz);
   }
-  const long long npc = (long long)bg.nc[0] * bg.nc[1] * bg.nc[2];
+  // x sub-bins per pair cell: 8, fewer when the bins would far outnumber the particles
+  bg.sxs = 3;
+  while (bg.sxs > 0 && (((long long)bg.nc[0] * bg.nc[1] * bg.nc[2]) << bg.sxs) > 8LL * prm->max_particles + (1 << 16)) --bg.sxs;
+  if (const char* e = std::getenv("MSM_PAIR_SUBBINS_LOG2")) bg.sxs = std::max(0, std::min(3, std::atoi(e)));
+  const long long npc = ((long long)bg.nc[0] * bg.nc[1] * bg.nc[2]) << bg.sxs;
   const long long ngc = (long long)bg.ng[0] * bg.ng[1] * bg.ng[2];
   if (npc > (1ll << 28) || ngc > (1ll << 28)) return MSM_ERR_UNSUPPORTED;
   p->n_pcells = (int)npc; p->n_gcells = (int)ngc;

@@ -154,6 +154,17 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     }
     (void)any_minimg;
     const double a = p->mp.a;
+    // x windows per row class: a row |dy| cells away starts max(|dy| - 1, 0) cell edges away, so the
+    // cutoff sphere reaches sqrt(a^2 - gy^2 - gz^2) along x there (rounded up to whole sub-bins)
+    pp.sxs = p->bg.sxs;
+    for (int ax = 0; ax < 3; ++ax) pp.edge_d[ax] = p->bg.cell_edge[ax];
+    for (int iy = 0; iy < 3; ++iy)
+      for (int iz = 0; iz < 3; ++iz) {
+        const double gy = std::max(iy - 1, 0) * p->bg.cell_edge[1], gz = std::max(iz - 1, 0) * p->bg.cell_edge[2];
+        const double rem = a * a - gy * gy - gz * gz;
+        const double sub = p->bg.cell_edge[0] / (double)(1 << p->bg.sxs);
+        pp.wb[iy][iz] = rem > 0.0 ? (int)std::ceil(std::sqrt(rem) * (1.0 + 1e-9) / sub) : -1;
+      }
     // fp32 scan: exact cutoff in fp32 mode (the drain repeats the same arithmetic); in fp64 mode a
     // slack of 1e-4 relative covers the rounding of cell-relative coordinates (< 2^-24 * 8 edges)
     pp.a2_scan = sizeof(T) == 4 ? (float)(a * a) : (float)(a * a * (1.0 + 1e-4));

@@ -2,30 +2,37 @@
 // (Eq. 5 first term; Eq. 21 l = 0), with forces and the pair virial.
 //
 // Cells have edge >= a/2, so the neighbourhood of a cell is 5 x 5 x 5 cells. The particles are
-// sorted by cell, x fastest, so the neighbours of a particle in one of the 25 neighbouring cell
-// rows (dy, dz) are ONE contiguous range of the sorted order (two when the x window wraps).
+// sorted by cell row (cy, cz) and, inside a row, by x in sub-bins of a fraction of a cell
+// (sort.cuh), so the neighbours of a particle in one of the 25 neighbouring rows (dy, dz) are ONE
+// contiguous range of the sorted order (two when the x window wraps around a periodic box).
 //
-// Work unit = one warp = a CLUSTER of 8 consecutive sorted particles of one cell row, laid out as
+// Work unit = one warp = a CLUSTER of 8 consecutive sorted particles of one row, laid out as
 // 8 i-particles x 4 j-phases: lane = 8 * jq + il owns particle il and every fourth PAIR of
-// candidates. A 32-particle tile (round 1) is as long as the cutoff itself, so its lanes scanned a
-// 7-cell x-range for a 5-cell need; a cluster of 8 is ~0.7 cells long, its window is 5-6 cells, and
-// each lane now walks only a quarter of it. The candidates of all 25 rows are staged through
-// shared memory in the cluster's frame (coordinates relative to the cluster's first cell: fp32
-// differences stay accurate), flattened into one list, so that every step of the inner loop is a
-// full 8 i x 8 j block of pairs with no ragged row ends.
+// candidates. A cluster is ~0.4 cutoffs long in x (a 32-particle tile is as long as the cutoff
+// itself), and the x window of every row is cut to the reach the cutoff sphere still has at that
+// row's (dy, dz) distance, in sub-bin units. The candidates of all rows are staged through shared
+// memory in the cluster's frame (coordinates relative to the cluster's first cell: fp32
+// differences stay accurate) as one flat list, so that every step of the inner loop is a full
+// 8 i x 8 j block of pairs with no ragged row ends.
 //
 // fp32: every staged candidate is evaluated in full with packed f32x2 arithmetic (FADD2 / FMUL2 /
 //   FFMA2: two pairs per instruction and lane) and masked by the cutoff test -- no hit lists, no
-//   divergence, no shared-memory traffic beyond two broadcast 16-byte loads per step. Only 25-30 %
+//   divergence, no shared-memory traffic beyond two broadcast 16-byte loads per step. Only ~30 %
 //   of the candidates are inside the cutoff, but filtering them costs as many issue slots as the
 //   interaction itself in packed fp32 (round 1's scan + drain kernel spent 71 % of its time in the
-//   shared-memory pipe on list bookkeeping).
-// fp64: DFMA runs at half the FP32 rate and the interaction needs ~45 of them, so here filtering
+//   shared-memory pipe on list bookkeeping). The loop is bound by the FP32 pipe.
+// fp64: DFMA runs at half the FP32 rate and the interaction needs ~40 of them, so here filtering
 //   pays: a packed fp32 scan (slightly widened cutoff) appends each lane's hits to its private
 //   list in shared memory, and the drain evaluates only those in fp64 (exact cutoff test repeated).
-// The virial is accumulated over HALF the neighbourhood: rows above the cluster's own row with
-// weight 1, the own row with weight 1/2 (both ends visit it), rows below not at all -- every
-// unordered pair exactly once.
+//
+// Virial. For a pair that interacts without a periodic image shift, sum_pairs f_ij (x) d_ij equals
+// sum_i F_i (x) r_i with absolute positions, so those pairs -- all of them in an open box, all but
+// the ones across a box face otherwise -- cost nothing extra: the force sums of the unshifted
+// candidates are kept apart and multiplied by r_i once per particle (in fp64). Only candidates
+// reached through a wrapped row or a wrapped x segment accumulate f (x) d pair by pair, over HALF
+// the neighbourhood (rows above the cluster's row with weight 1, its own row with weight 1/2, rows
+// below not at all), i.e. every image pair exactly once.
+//
 // Small systems have too few clusters to fill the GPU: the dz planes of the neighbourhood are then
 // dealt to up to kPairMaxSplit blocks (blockIdx.z) whose partial sums k_interpolate adds in order.
 // Every lane visits its candidates in a fixed order and the four phases of a particle are added
@@ -42,9 +49,12 @@ namespace msm {
 template <typename T> struct PairParams {
   int nc[3];
   int periodic[3];
-  int omin[3], omax[3];   // neighbour cell offsets per axis (y, z use these; x: +-2 around the cluster)
+  int omin[3], omax[3];   // neighbour cell offsets per axis (y, z)
   int minimg[3];          // periodic axis with fewer than 5 cells: explicit minimum image
+  int sxs;                // log2 of the x sub-bins per cell
+  int wb[3][3];           // half-width of the x window in sub-bins for rows with |dy|, |dz| = 0, 1, 2; -1: out of reach
   T edge[3];
+  double edge_d[3];
   T box[3], inv_box[3];
   T a, a2, inv_a, inv_a2, two_inv_a3;
   float a2_scan;          // cutoff^2 of the fp32 scan (widened by rounding slack in fp64 mode)
@@ -54,7 +64,6 @@ template <typename T> struct PairParams {
   size_t part_stride;     // elements between the per-split partial outputs (capacity)
 };
 
-constexpr int kPairWarpsMax = 4;
 // independent warps (clusters) per block: fp64 stages 14 KB per warp (48 KB static limit)
 template <typename T> struct PairWarps { static constexpr int value = sizeof(T) == 4 ? 4 : 2; };
 constexpr int kPairCluster = 8;     // i-particles per warp
@@ -108,18 +117,26 @@ __device__ __forceinline__ double rsqrt_fast(double x) {
   return y;
 }
 
-// accumulators of one lane: force factor sums, potential, virial (xx yy zz xy xz yz)
+// accumulators of one lane: force factor sums of the unshifted candidates (ax ay az), of the
+// image-shifted ones (bx by bz) with their pair virial (w: xx yy zz xy xz yz), potential
 template <typename T> struct PairAcc {
   T ax = 0, ay = 0, az = 0, av = 0;
+  T bx = 0, by = 0, bz = 0;
   T w[6] = {0, 0, 0, 0, 0, 0};
 };
 struct PairAcc2 {   // fp32 packed: two partial sums per quantity
   float2 ax = {0.f, 0.f}, ay = {0.f, 0.f}, az = {0.f, 0.f}, av = {0.f, 0.f};
+  float2 bx = {0.f, 0.f}, by = {0.f, 0.f}, bz = {0.f, 0.f};
   float2 w[6] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
 };
 
+// how a range of candidates is accumulated
+constexpr int kPairPlain = 0;     // unshifted: force sums a
+constexpr int kPairImage = 1;     // periodic images: force sums b + pair virial w
+constexpr int kPairImageF = 2;    // periodic images, forces only (their virial is taken from the other end)
+
 // one full interaction in precision T (scalar path: fp64 drain, minimum-image instances)
-template <typename T, int P, bool VIR>
+template <typename T, int P, int MODE>
 __device__ __forceinline__ void pair_interact(PairAcc<T>& A, T dx, T dy, T dz, T r2, T qj, T inv_a, T inv_a2,
                                               T two_inv_a3, const T (&cf)[P], const T (&cd)[P]) {
   const T rinv = rsqrt_fast(r2);
@@ -131,37 +148,48 @@ __device__ __forceinline__ void pair_interact(PairAcc<T>& A, T dx, T dy, T dz, T
   for (int k = P - 2; k >= 1; --k) dg = fma(dg, s, cd[k]);
   A.av = fma(qj, fma(-g, inv_a, rinv), A.av);
   const T fs = qj * fma(two_inv_a3, dg, rinv * rinv * rinv);
-  A.ax = fma(fs, dx, A.ax); A.ay = fma(fs, dy, A.ay); A.az = fma(fs, dz, A.az);
-  if (VIR) {
+  if (MODE == kPairImage) {
     const T fx = fs * dx, fy = fs * dy, fz = fs * dz;
+    A.bx = fma(fs, dx, A.bx); A.by = fma(fs, dy, A.by); A.bz = fma(fs, dz, A.bz);   // as in kPairImageF
     A.w[0] = fma(fx, dx, A.w[0]); A.w[1] = fma(fy, dy, A.w[1]); A.w[2] = fma(fz, dz, A.w[2]);
     A.w[3] = fma(fx, dy, A.w[3]); A.w[4] = fma(fx, dz, A.w[4]); A.w[5] = fma(fy, dz, A.w[5]);
+  } else if (MODE == kPairImageF) {
+    A.bx = fma(fs, dx, A.bx); A.by = fma(fs, dy, A.by); A.bz = fma(fs, dz, A.bz);
+  } else {
+    A.ax = fma(fs, dx, A.ax); A.ay = fma(fs, dy, A.ay); A.az = fma(fs, dz, A.az);
   }
 }
 
 template <typename T, int P, bool VIRIAL, bool MI>
 __global__ void __launch_bounds__(PairWarps<T>::value * 32, sizeof(T) == 4 ? 6 : 1)
 k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>::type* __restrict__ prec,
-       const int* __restrict__ pcellx, const int* __restrict__ porder, T* __restrict__ Fsr,
+       const int* __restrict__ pbinx, const int* __restrict__ porder, T* __restrict__ Fsr,
        T* __restrict__ Vsr, double* __restrict__ wpart) {
   using V4 = typename Vec4<T>::type;
   constexpr int CAP = PairStage<T>::kCap;
   constexpr int kPairWarps = PairWarps<T>::value;
   constexpr bool kPacked = sizeof(T) == 4 && !MI;     // fp32: brute force with packed arithmetic
   constexpr bool kLists = sizeof(T) == 8 && !MI;      // fp64: fp32 scan + hit lists + fp64 drain
+  // the candidate list has four regions (own-row images, images above, images below, unshifted),
+  // with or without the virial (same summation order, so the forces do not depend on whether the
+  // virial is asked for); the minimum-image instances have just one
+  constexpr bool kSplit = !MI;
   __shared__ PairStage<T> stage[kPairWarps];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int il = lane & 7, jq = lane >> 3;
   PairStage<T>& sj = stage[wid];
   const int row = blockIdx.x;                       // (cy, cz); blockIdx.y strides over the row's clusters
   const int cy = row % prm.nc[1], cz = row / prm.nc[1];
-  const int ncx = prm.nc[0];
-  const int row_s = pstart[row * ncx], row_e = pstart[(row + 1) * ncx];
+  const int sxs = prm.sxs;
+  const int nbx = prm.nc[0] << sxs;                 // sub-bins per row
+  const int row_s = pstart[row * nbx], row_e = pstart[(row + 1) * nbx];
   const int ntile = (row_e - row_s + kPairCluster - 1) / kPairCluster;
   const bool mix = MI && prm.minimg[0] != 0, miy = MI && prm.minimg[1] != 0, miz = MI && prm.minimg[2] != 0;
-  // a cluster pass may span at most span_max cells beyond its first one, so that its +-2
-  // neighbourhood never overlaps itself on a periodic axis and the window stays short
-  const int span_max = prm.periodic[0] && !mix ? max(min(ncx - 5, kPairSpanCap), 0) : kPairSpanCap;
+  // a cluster pass may span at most span_max sub-bins beyond its first one, so that its widest
+  // window never overlaps itself on a periodic axis and stays short
+  const int wmax = prm.wb[0][0];
+  const int span_max = prm.periodic[0] && !mix ? max(min(nbx - 2 * wmax - 1, kPairSpanCap << sxs), 0)
+                                               : (kPairSpanCap << sxs);
   const T a2 = prm.a2, inv_a = prm.inv_a, inv_a2 = prm.inv_a2, two_inv_a3 = prm.two_inv_a3;
   const float a2_scan = prm.a2_scan;
   T cf[P], cd[P];                                   // g(s) = sum cf[k] s^k, g'(s) = sum cd[k] s^(k-1)
@@ -169,13 +197,14 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
   for (int k = 0; k < P; ++k) { cf[k] = prm.c[k]; cd[k] = (T)k * prm.c[k]; }
   double W[6] = {0, 0, 0, 0, 0, 0};
 
-  // the neighbour rows of this block in class order: lane r describes row r.
-  //   class 1 (r = 0): the cluster's own row, virial weight 1/2;  class 2: rows above (dz > 0, or
-  //   dz = 0 and dy > 0), weight 1;  class 3: rows below, no virial. Minimum-image instances (fewer
-  //   than 5 cells on a periodic axis: offsets alias) put every row into class 1.
+  // the neighbour rows of this block: lane r describes row r.
+  //   class 1 (r = 0): the cluster's own row;  class 2: rows above (dz > 0, or dz = 0 and dy > 0);
+  //   class 3: rows below. Minimum-image instances (fewer than 5 cells on a periodic axis: offsets
+  //   alias) put every row into class 1. my_wrap: the row is reached across a periodic box face.
   const int ny_off = prm.omax[1] - prm.omin[1] + 1, nz_off = prm.omax[2] - prm.omin[2] + 1;
   const int nrows = ny_off * nz_off;                // <= 25
-  int my_dy = 0, my_dz = 0, my_class = 0, my_rowbase = 0;   // class 0: row absent
+  int my_dy = 0, my_dz = 0, my_class = 0, my_rowbase = 0, my_wb = 0;   // class 0: row absent
+  bool my_wrap = false;
   if (lane < nrows) {
     if (MI) {
       my_dy = prm.omin[1] + lane % ny_off; my_dz = prm.omin[2] + lane / ny_off;
@@ -192,69 +221,85 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
     }
     if ((my_dz - prm.omin[2]) % prm.nsplit != (int)blockIdx.z) my_class = 0;
     int cyj = cy + my_dy, czj = cz + my_dz;
-    if (prm.periodic[1]) cyj = imod(cyj, prm.nc[1]); else if (cyj < 0 || cyj >= prm.nc[1]) my_class = 0;
-    if (prm.periodic[2]) czj = imod(czj, prm.nc[2]); else if (czj < 0 || czj >= prm.nc[2]) my_class = 0;
-    my_rowbase = (czj * prm.nc[1] + cyj) * ncx;
+    if (cyj < 0 || cyj >= prm.nc[1]) { if (prm.periodic[1]) { cyj = imod(cyj, prm.nc[1]); my_wrap = true; } else my_class = 0; }
+    if (czj < 0 || czj >= prm.nc[2]) { if (prm.periodic[2]) { czj = imod(czj, prm.nc[2]); my_wrap = true; } else my_class = 0; }
+    my_rowbase = (czj * prm.nc[1] + cyj) * nbx;
+    my_wb = MI ? wmax : prm.wb[min(abs(my_dy), 2)][min(abs(my_dz), 2)];
+    if (my_wb < 0) my_class = 0;                    // the cutoff sphere does not reach this row
   }
+  const int r0 = MI ? (-prm.omin[1]) + (-prm.omin[2]) * ny_off : 0;   // lane of the cluster's own row
 
   for (int tile = blockIdx.y * kPairWarps + wid; tile < ntile; tile += kPairWarps * gridDim.y) {
     const int k0 = row_s + tile * kPairCluster;     // first sorted particle of the cluster
     const int ki = k0 + il;
     const bool inrow = ki < row_e;
     V4 ri = make_vec4<T>(0, 0, 0, 0);
-    int cxi = 0;
-    if (inrow) { ri = ldg4(prec + ki); cxi = pcellx[ki]; }
+    int bxi = 0;                                    // sub-bin of the particle along x
+    if (inrow) { ri = ldg4(prec + ki); bxi = pbinx[ki]; }
     const int last = min(kPairCluster - 1, row_e - 1 - k0);
-   // passes: consecutive particles whose cells span at most span_max (one pass unless the row is sparse)
+   // passes: consecutive particles whose sub-bins span at most span_max (one pass unless the row is sparse)
    for (int first = 0; first <= last;) {
-    const int cxf = __shfl_sync(0xffffffffu, cxi, first);
-    const unsigned fits = __ballot_sync(0xffffffffu, inrow && il >= first && cxi - cxf <= span_max) & 0xffu;
-    const int sub_last = 31 - __clz((int)fits);            // cells ascend with il
+    const int fp0 = first;
+    const int binf = __shfl_sync(0xffffffffu, bxi, first);
+    const unsigned fits = __ballot_sync(0xffffffffu, inrow && il >= first && bxi - binf <= span_max) & 0xffu;
+    const int sub_last = 31 - __clz((int)fits);            // sub-bins ascend with il
     const bool iv = il >= first && il <= sub_last;
-    const int cxl = __shfl_sync(0xffffffffu, cxi, sub_last);
+    const int binl = __shfl_sync(0xffffffffu, bxi, sub_last);
     first = sub_last + 1;
-    const T xi = ri.x + (T)(cxi - cxf) * prm.edge[0], yi = ri.y, zi = ri.z;
-    // x-range of neighbour cells in unwrapped cell coordinates
-    int xa = cxf - 2, xb = cxl + 2;
-    if (!prm.periodic[0]) { xa = max(xa, 0); xb = min(xb, ncx - 1); }
-    else if (mix) { xa = 0; xb = ncx - 1; }                 // fewer than 5 cells: each once + min. image
-    // this lane's row: up to two contiguous segments of the sorted order (main, wrapped)
+    const int cxf = binf >> sxs;                            // the frame: first particle's cell
+    const T xi = ri.x + (T)((bxi >> sxs) - cxf) * prm.edge[0], yi = ri.y, zi = ri.z;
+    // this lane's row: its x window in unwrapped sub-bins, as up to two contiguous segments of the
+    // sorted order (A: unshifted, B: through the periodic wrap in x)
     int sA = 0, lA = 0, sB = 0, lB = 0, shB = 0;
     if (my_class != 0) {
-      const int ca = max(xa, 0), cb = min(xb, ncx - 1);
+      int xa = binf - my_wb, xb = binl + my_wb;
+      if (!prm.periodic[0]) { xa = max(xa, 0); xb = min(xb, nbx - 1); }
+      else if (mix) { xa = 0; xb = nbx - 1; }               // fewer than 5 cells: each once + min. image
+      const int ca = max(xa, 0), cb = min(xb, nbx - 1);
       if (ca <= cb) { sA = pstart[my_rowbase + ca]; lA = pstart[my_rowbase + cb + 1] - sA; }
-      if (xa < 0) { sB = pstart[my_rowbase + xa + ncx]; lB = pstart[my_rowbase + ncx] - sB; shB = -ncx; }
-      else if (xb >= ncx) { sB = pstart[my_rowbase]; lB = pstart[my_rowbase + xb - ncx + 1] - sB; shB = ncx; }
+      if (xa < 0) { sB = pstart[my_rowbase + xa + nbx]; lB = pstart[my_rowbase + nbx] - sB; shB = -prm.nc[0]; }
+      else if (xb >= nbx) { sB = pstart[my_rowbase]; lB = pstart[my_rowbase + xb - nbx + 1] - sB; shB = prm.nc[0]; }
     }
-    // The candidates of all rows form ONE flat list (row after row, class after class); each class
-    // region is padded to a multiple of 8 so that a step of 8 candidates never straddles two classes.
-    const int len = lA + lB;
-    int incl = len;
+    // Flat candidate list. kSplit: region 0 = images in the own row (x wrap), 1 = images in rows
+    // above, 2 = images in rows below, 3 = unshifted candidates; each region is padded to a multiple
+    // of 8 so that a step never straddles two regions. Otherwise everything is in region 3.
+    const bool wrapA = kSplit && my_wrap;
+    int n0 = 0, n1 = 0, n2 = 0, n3 = 0;                     // this lane's contribution to the regions
+    if (kSplit) {
+      if (my_class == 1) n0 = lB;
+      else if (my_class == 2) n1 = lB + (wrapA ? lA : 0);
+      else if (my_class == 3) n2 = lB + (wrapA ? lA : 0);
+      if (!wrapA) n3 = lA;
+    } else {
+      n3 = lA + lB;
+    }
+    int i1 = n1, i2 = n2, i3 = n3;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      const int t = __shfl_up_sync(0xffffffffu, incl, o);
-      if (lane >= o) incl += t;
+      const int t1 = __shfl_up_sync(0xffffffffu, i1, o), t2 = __shfl_up_sync(0xffffffffu, i2, o);
+      const int t3 = __shfl_up_sync(0xffffffffu, i3, o);
+      if (lane >= o) { i1 += t1; i2 += t2; i3 += t3; }
     }
-    int r1e = 0, b1 = 1 << 30, r2e = 0, b2 = 1 << 30;       // raw and padded ends of the class 1 / 2 regions
-    if (!MI) {
-      r1e = __shfl_sync(0xffffffffu, incl, 0);
-      b1 = (r1e + 7) & ~7;
-      r2e = __shfl_sync(0xffffffffu, incl, 12) + (b1 - r1e);
-      b2 = (r2e + 7) & ~7;
+    // raw ends e_k and padded ends b_k of the regions
+    const int e0 = __shfl_sync(0xffffffffu, n0, 0), b0 = (e0 + 7) & ~7;
+    const int e1 = b0 + __shfl_sync(0xffffffffu, i1, 31), b1 = (e1 + 7) & ~7;
+    const int e2 = b1 + __shfl_sync(0xffffffffu, i2, 31), b2 = (e2 + 7) & ~7;
+    const int e3 = b2 + __shfl_sync(0xffffffffu, i3, 31), total = (e3 + 7) & ~7;
+    int offA, offB;                                          // flat positions of this lane's segments
+    if (kSplit) {
+      const int img = my_class == 2 ? b0 + i1 - n1 : b1 + i2 - n2;   // start of this row among the images
+      offA = wrapA ? img : b2 + i3 - n3;
+      offB = my_class == 1 ? 0 : img + (wrapA ? lA : 0);
+    } else {
+      offA = b2 + i3 - n3;
+      offB = offA + lA;
     }
-    const int off = incl - len + (!MI && lane >= 1 ? b1 - r1e : 0) + (!MI && lane >= 13 ? b2 - r2e : 0);
-    const int r3e = __shfl_sync(0xffffffffu, incl, 31) + (MI ? 0 : (b1 - r1e) + (b2 - r2e));
-    const int total = (r3e + 7) & ~7;
-    // flat position of the lane's own particle (in the cluster's own row), -1 if that row is absent
-    int selfpos = -1;
-    {
-      const int r0 = MI ? (-prm.omin[1]) + (-prm.omin[2]) * ny_off : 0;
-      const int a0 = __shfl_sync(0xffffffffu, sA, r0), la0 = __shfl_sync(0xffffffffu, lA, r0);
-      const int b0 = __shfl_sync(0xffffffffu, sB, r0), lb0 = __shfl_sync(0xffffffffu, lB, r0);
-      const int o0 = __shfl_sync(0xffffffffu, off, r0);
-      if (ki >= a0 && ki < a0 + la0) selfpos = o0 + ki - a0;
-      else if (ki >= b0 && ki < b0 + lb0) selfpos = o0 + la0 + ki - b0;
-    }
+    // flat positions of the active particles of the cluster (consecutive, in the own row's segment A)
+    const int sA0 = __shfl_sync(0xffffffffu, sA, r0), lA0 = __shfl_sync(0xffffffffu, lA, r0);
+    const int oA0 = __shfl_sync(0xffffffffu, offA, r0);
+    const bool own_present = lA0 > 0;                        // (absent: the own row belongs to another split)
+    const int sfirst = oA0 + (k0 + fp0 - sA0), slast = sfirst + (sub_last - fp0);
+    const int selfpos = own_present ? sfirst + (il - fp0) : -(1 << 20);
 
     PairAcc<T> A;                       // scalar accumulators (fp64, minimum image)
     PairAcc2 A2;                        // packed accumulators (fp32)
@@ -266,54 +311,60 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
 
     for (int base = 0; base < total; base += CAP) {
       const int hi = min(base + CAP, total);
-      // ---- pads of the three class regions
+      // ---- pads of the four regions
       {
-        const int gs = grp == 0 ? r1e : grp == 1 ? r2e : r3e, ge = grp == 0 ? b1 : grp == 1 ? b2 : total;
+        const int gs = grp == 0 ? e0 : grp == 1 ? e1 : grp == 2 ? e2 : e3;
+        const int ge = grp == 0 ? b0 : grp == 1 ? b1 : grp == 2 ? b2 : total;
         const int pos = gs + il;
-        if (grp < 3 && (!MI || grp == 2) && pos < ge && pos >= base && pos < hi)
-          sj.put(pos - base, make_vec4<T>(far, 0, 0, 0));
+        if (pos < ge && pos >= base && pos < hi) sj.put(pos - base, make_vec4<T>(far, 0, 0, 0));
       }
       // ---- stage: four rows at a time, eight lanes per row, into the cluster's frame
       for (int rr = 0; rr < nrows; rr += 4) {
         const int r = rr + grp;
-        const int o = __shfl_sync(0xffffffffu, off, r), la = __shfl_sync(0xffffffffu, lA, r);
-        const int lb = __shfl_sync(0xffffffffu, lB, r), sa = __shfl_sync(0xffffffffu, sA, r);
-        const int sb = __shfl_sync(0xffffffffu, sB, r), sh = __shfl_sync(0xffffffffu, shB, r);
         const T yoff = (T)__shfl_sync(0xffffffffu, my_dy, r) * prm.edge[1];
         const T zoff = (T)__shfl_sync(0xffffffffu, my_dz, r) * prm.edge[2];
-        const int t1 = min(la + lb, hi - o);
-        // four elements per lane and batch: all eight loads of a batch are issued before the first
-        // store, so a batch costs one global-memory latency instead of four
+        // elements [t0, t1) of a segment (source index s0, flat position o0, cell shift sh)
+        auto stage_seg = [&](int s0, int len, int o0, int sh) {
+          const int t1 = min(len, hi - o0);
+          // four elements per lane and batch: all eight loads of a batch are issued before the
+          // first store, so a batch costs one global-memory latency instead of four
 #pragma unroll 1
-        for (int tb = max(0, base - o) + il; tb < t1; tb += 32) {
-          V4 rj[4];
-          int cj[4];
+          for (int tb = max(0, base - o0) + il; tb < t1; tb += 32) {
+            V4 rj[4];
+            int cj[4];
 #pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            const int t = tb + 8 * k;
-            const bool inA = t < la;
-            const int src = t < t1 ? (inA ? sa + t : sb + (t - la)) : 0;
-            rj[k] = ldg4(prec + src);
-            cj[k] = pcellx[src] + (inA ? 0 : sh) - cxf;
-          }
+            for (int k = 0; k < 4; ++k) {
+              const int src = s0 + min(tb + 8 * k, t1 - 1);
+              rj[k] = ldg4(prec + src);
+              cj[k] = (pbinx[src] >> sxs) + sh - cxf;
+            }
 #pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            const int t = tb + 8 * k;
-            if (t < t1) {
-              rj[k].x += (T)cj[k] * prm.edge[0];
-              rj[k].y += yoff;
-              rj[k].z += zoff;
-              sj.put(o + t - base, rj[k]);
+            for (int k = 0; k < 4; ++k) {
+              const int t = tb + 8 * k;
+              if (t < t1) {
+                rj[k].x += (T)cj[k] * prm.edge[0];
+                rj[k].y += yoff;
+                rj[k].z += zoff;
+                sj.put(o0 + t - base, rj[k]);
+              }
             }
           }
-        }
+        };
+        stage_seg(__shfl_sync(0xffffffffu, sA, r), __shfl_sync(0xffffffffu, lA, r), __shfl_sync(0xffffffffu, offA, r), 0);
+        const int lb = __shfl_sync(0xffffffffu, lB, r);
+        if (__any_sync(0xffffffffu, lb > 0))
+          stage_seg(__shfl_sync(0xffffffffu, sB, r), lb, __shfl_sync(0xffffffffu, offB, r), __shfl_sync(0xffffffffu, shB, r));
       }
       __syncwarp();
 
-      // ---- candidates [lo, hi2) of the flat list (multiples of 8) against the 8 particles
-      auto run = [&](int lo, int hi2, auto virc) {
-        constexpr bool VIR = decltype(virc)::value;
+      // ---- candidates [lo, hi2) of the flat list (multiples of 8) against the 8 particles.
+      // MODE: kPairPlain / kPairImage / kPairImageF; SELF: the range may hold the cluster's own
+      // particles (index test)
+      auto run = [&](int lo, int hi2, auto modec, auto selfc) {
+        constexpr int MODE = decltype(modec)::value;
+        constexpr bool SELF = decltype(selfc)::value;
         const int nsteps = (hi2 - lo) >> 3;
+        if (nsteps <= 0) return;
         if constexpr (kPacked) {
           const float ia2 = (float)inv_a2, nia = -(float)inv_a, t3 = (float)two_inv_a3;
           const float2 xi2 = make_float2(xs, xs), yi2 = make_float2(ys, ys), zi2 = make_float2(zs, zs);
@@ -328,8 +379,13 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
             const float2 dz = __fadd2_rn(zi2, make_float2(-zq.x, -zq.y));
             // + 1e-20: no effect on a real pair; keeps the masked self pair finite
             const float2 r2 = __ffma2_rn(dx, dx, __ffma2_rn(dy, dy, __ffma2_rn(dz, dz, make_float2(1e-20f, 1e-20f))));
-            const float2 qj = make_float2((r2.x < a2_scan && jdx != 0) ? zq.z : 0.f,
-                                          (r2.y < a2_scan && jdx != -1) ? zq.w : 0.f);
+            float2 qj;
+            if (SELF) {
+              qj = make_float2((r2.x < a2_scan && jdx != 0) ? zq.z : 0.f, (r2.y < a2_scan && jdx != -1) ? zq.w : 0.f);
+              jdx += 8;
+            } else {
+              qj = make_float2(r2.x < a2_scan ? zq.z : 0.f, r2.y < a2_scan ? zq.w : 0.f);
+            }
             const float2 rinv = make_float2(rsqrt_fast(r2.x), rsqrt_fast(r2.y));
             const float2 sv = __ffma2_rn(r2, make_float2(ia2, ia2), make_float2(-1.f, -1.f));
             float2 g = make_float2((float)cf[P - 1], (float)cf[P - 1]), dg = make_float2((float)cd[P - 1], (float)cd[P - 1]);
@@ -338,16 +394,18 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
 #pragma unroll
             for (int k = P - 2; k >= 1; --k) dg = __ffma2_rn(dg, sv, make_float2((float)cd[k], (float)cd[k]));
             A2.av = __ffma2_rn(qj, __ffma2_rn(g, make_float2(nia, nia), rinv), A2.av);
-            const float2 rinv3 = __fmul2_rn(__fmul2_rn(rinv, rinv), rinv);
-            const float2 fs = __fmul2_rn(qj, __ffma2_rn(make_float2(t3, t3), dg, rinv3));
-            A2.ax = __ffma2_rn(fs, dx, A2.ax); A2.ay = __ffma2_rn(fs, dy, A2.ay); A2.az = __ffma2_rn(fs, dz, A2.az);
-            if (VIR) {
+            const float2 fs = __fmul2_rn(qj, __ffma2_rn(make_float2(t3, t3), dg, __fmul2_rn(__fmul2_rn(rinv, rinv), rinv)));
+            if (MODE == kPairImage) {
               const float2 fx = __fmul2_rn(fs, dx), fy = __fmul2_rn(fs, dy), fz = __fmul2_rn(fs, dz);
+              A2.bx = __ffma2_rn(fs, dx, A2.bx); A2.by = __ffma2_rn(fs, dy, A2.by); A2.bz = __ffma2_rn(fs, dz, A2.bz);
               A2.w[0] = __ffma2_rn(fx, dx, A2.w[0]); A2.w[1] = __ffma2_rn(fy, dy, A2.w[1]); A2.w[2] = __ffma2_rn(fz, dz, A2.w[2]);
               A2.w[3] = __ffma2_rn(fx, dy, A2.w[3]); A2.w[4] = __ffma2_rn(fx, dz, A2.w[4]); A2.w[5] = __ffma2_rn(fy, dz, A2.w[5]);
+            } else if (MODE == kPairImageF) {
+              A2.bx = __ffma2_rn(fs, dx, A2.bx); A2.by = __ffma2_rn(fs, dy, A2.by); A2.bz = __ffma2_rn(fs, dz, A2.bz);
+            } else {
+              A2.ax = __ffma2_rn(fs, dx, A2.ax); A2.ay = __ffma2_rn(fs, dy, A2.ay); A2.az = __ffma2_rn(fs, dz, A2.az);
             }
             fp += 32;
-            jdx += 8;
           }
         } else if constexpr (kLists) {
           // scan: packed fp32 distance test of this lane's candidate pairs, hits appended to its list
@@ -357,7 +415,7 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
             const float2 xi2 = make_float2(xs, xs), yi2 = make_float2(ys, ys), zi2 = make_float2(zs, zs);
             const float* fp = sj.f + (lo - base) * 4 + jq * 8;
             int idx = lo - base + 2 * jq;                   // index inside the chunk
-            const int selfl = selfpos - base;
+            const int selfl = SELF ? selfpos - base : -1;
             for (int s = 0; s < nsteps; ++s) {
               const float4 xy = *reinterpret_cast<const float4*>(fp);
               const float2 zz = *reinterpret_cast<const float2*>(fp + 4);
@@ -382,7 +440,7 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
               const V4 pj = sj.full(lp[r * 32]);
               const T dx = xi - pj.x, dy = yi - pj.y, dz = zi - pj.z;
               const T r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-              if (r2 < a2) pair_interact<T, P, VIR>(A, dx, dy, dz, r2, pj.w, inv_a, inv_a2, two_inv_a3, cf, cd);
+              if (r2 < a2) pair_interact<T, P, MODE>(A, dx, dy, dz, r2, pj.w, inv_a, inv_a2, two_inv_a3, cf, cd);
             }
           }
           __syncwarp();
@@ -398,16 +456,23 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
               if (miy) dy -= prm.box[1] * rint(dy * prm.inv_box[1]);
               if (miz) dz -= prm.box[2] * rint(dz * prm.inv_box[2]);
               const T r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-              if (iv && pos < r3e && pos != selfpos && r2 < a2)
-                pair_interact<T, P, VIR>(A, dx, dy, dz, r2, pj.w, inv_a, inv_a2, two_inv_a3, cf, cd);
+              if (iv && pos < e3 && pos != selfpos && r2 < a2)
+                pair_interact<T, P, MODE>(A, dx, dy, dz, r2, pj.w, inv_a, inv_a2, two_inv_a3, cf, cd);
             }
           }
         }
       };
-      if (VIRIAL) {
-        const int e1 = min(max(b1, base), hi), e2 = min(max(b2, base), hi);
-        run(base, e1, std::true_type());
-        if (!MI && b1 > base && b1 <= hi) {               // the own row is done: both ends visit its pairs
+      using Plain = std::integral_constant<int, kPairPlain>;
+      using Image = std::integral_constant<int, kPairImage>;
+      using ImageF = std::integral_constant<int, kPairImageF>;
+      using Yes = std::true_type;
+      using No = std::false_type;
+      auto clampc = [&](int v) { return min(max(v, base), hi); };
+      if (kSplit && !VIRIAL) {
+        run(base, clampc(b2), ImageF(), No());
+      } else if (kSplit) {
+        run(base, clampc(b0), Image(), No());              // images in the own row
+        if (b0 > base && b0 <= hi) {                       // done: both ends visit these pairs
           if constexpr (kPacked) {
 #pragma unroll
             for (int k = 0; k < 6; ++k) { A2.w[k].x *= 0.5f; A2.w[k].y *= 0.5f; }
@@ -416,29 +481,58 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
             for (int k = 0; k < 6; ++k) A.w[k] *= (T)0.5;
           }
         }
-        run(e1, e2, std::true_type());
-        run(e2, hi, std::false_type());
-      } else {
-        run(base, hi, std::false_type());
+        run(clampc(b0), clampc(b1), Image(), No());        // images above: weight 1
+        run(clampc(b1), clampc(b2), ImageF(), No());       // images below: forces only
+      }
+      {
+        // unshifted candidates (everything when the list has one region); only the one or two
+        // steps around the cluster's own particles need the index test
+        const int lo3 = kSplit ? clampc(b2) : base;
+        if (MI && VIRIAL) {
+          run(lo3, hi, Image(), Yes());
+        } else if (own_present) {
+          const int s0 = min(max(sfirst & ~7, lo3), hi), s1 = min(max((slast & ~7) + 8, lo3), hi);
+          run(lo3, s0, Plain(), No());
+          run(s0, s1, Plain(), Yes());
+          run(s1, hi, Plain(), No());
+        } else {
+          run(lo3, hi, Plain(), No());
+        }
       }
       __syncwarp();
     }
-    if (MI && VIRIAL) {                                   // every row in class 1: both ends visit every pair
-#pragma unroll
-      for (int k = 0; k < 6; ++k) A.w[k] *= (T)0.5;
-    }
     if constexpr (kPacked) {
       A.ax = A2.ax.x + A2.ax.y; A.ay = A2.ay.x + A2.ay.y; A.az = A2.az.x + A2.az.y; A.av = A2.av.x + A2.av.y;
+      A.bx = A2.bx.x + A2.bx.y; A.by = A2.by.x + A2.by.y; A.bz = A2.bz.x + A2.bz.y;
 #pragma unroll
       for (int k = 0; k < 6; ++k) A.w[k] = A2.w[k].x + A2.w[k].y;
     }
-    // the four phases of a particle, in a fixed order
+    const T qi = ri.w;
+    if (VIRIAL && iv) {
+      const double dq = (double)qi;
+      if (MI) {                                           // every pair is visited from both ends
+#pragma unroll
+        for (int k = 0; k < 6; ++k) W[k] += 0.5 * dq * (double)A.w[k];
+      } else {
+        // image pairs (counted once, see above) + this lane's share of F_i (x) r_i for the rest
+#pragma unroll
+        for (int k = 0; k < 6; ++k) W[k] += dq * (double)A.w[k];
+        // (positions from the box centre: sum F_i = 0 only up to rounding, and what is left of it
+        // is weighted by |r_i|)
+        const double rx = (double)ri.x + ((double)(bxi >> sxs) - 0.5 * (double)prm.nc[0]) * prm.edge_d[0];
+        const double ry = (double)ri.y + ((double)cy - 0.5 * (double)prm.nc[1]) * prm.edge_d[1];
+        const double rz = (double)ri.z + ((double)cz - 0.5 * (double)prm.nc[2]) * prm.edge_d[2];
+        const double fx = dq * (double)A.ax, fy = dq * (double)A.ay, fz = dq * (double)A.az;
+        W[0] += fx * rx; W[1] += fy * ry; W[2] += fz * rz;
+        W[3] += 0.5 * (fx * ry + fy * rx); W[4] += 0.5 * (fx * rz + fz * rx); W[5] += 0.5 * (fy * rz + fz * ry);
+      }
+    }
+    // total force factor sums; the four phases of a particle, in a fixed order
+    A.ax += A.bx; A.ay += A.by; A.az += A.bz;
     A.ax += __shfl_xor_sync(0xffffffffu, A.ax, 8); A.ay += __shfl_xor_sync(0xffffffffu, A.ay, 8);
     A.az += __shfl_xor_sync(0xffffffffu, A.az, 8); A.av += __shfl_xor_sync(0xffffffffu, A.av, 8);
     A.ax += __shfl_xor_sync(0xffffffffu, A.ax, 16); A.ay += __shfl_xor_sync(0xffffffffu, A.ay, 16);
     A.az += __shfl_xor_sync(0xffffffffu, A.az, 16); A.av += __shfl_xor_sync(0xffffffffu, A.av, 16);
-
-    const T qi = ri.w;
     if (iv && jq == 0) {
       const int orig = porder[ki];
       T* Fp = Fsr + (size_t)blockIdx.z * 3 * prm.part_stride;   // partial of this split
@@ -446,11 +540,6 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
       Fp[3 * (size_t)orig + 1] = qi * A.ay;
       Fp[3 * (size_t)orig + 2] = qi * A.az;
       Vsr[(size_t)blockIdx.z * prm.part_stride + orig] = A.av;
-    }
-    if (VIRIAL && iv) {
-      const double dq = (double)qi;      // every unordered pair is counted once (see the row classes)
-#pragma unroll
-      for (int k = 0; k < 6; ++k) W[k] += dq * (double)A.w[k];
     }
    }
   }

@@ -23,7 +23,7 @@ __global__ void k_bin(int n, const T* __restrict__ pos, BinGeom g, int* __restri
                       int* __restrict__ pslot, int* __restrict__ gslot, int* __restrict__ flag) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  int pc[3], gc[3];
+  int pc[3], gc[3], sub = 0;
   bool bad = false;
 #pragma unroll
   for (int ax = 0; ax < 3; ++ax) {
@@ -33,11 +33,16 @@ __global__ void k_bin(int n, const T* __restrict__ pos, BinGeom g, int* __restri
     x = wrap_coord(x, g.box[ax], g.periodic[ax]);
     int c = (int)floor(x / g.cell_edge[ax]);
     pc[ax] = min(max(c, 0), g.nc[ax] - 1);
+    if (ax == 0) {   // sub-bin of the cell along x
+      const int nsub = 1 << g.sxs;
+      const int sb = (int)floor((x - pc[0] * g.cell_edge[0]) * (double)nsub / g.cell_edge[0]);
+      sub = min(max(sb, 0), nsub - 1);
+    }
     int k = (int)floor(x / g.h1[ax]);
     gc[ax] = min(max(k, 0), g.ng[ax] - 1);
   }
   if (bad) atomicOr(flag, 1);
-  const int pci = (pc[2] * g.nc[1] + pc[1]) * g.nc[0] + pc[0];
+  const int pci = (pc[2] * g.nc[1] + pc[1]) * (g.nc[0] << g.sxs) + (pc[0] << g.sxs) + sub;
   const int gci = (gc[2] * g.ng[1] + gc[1]) * g.ng[0] + gc[0];
   pcell[i] = pci;
   gcell[i] = gci;
@@ -163,13 +168,15 @@ __global__ void k_build_records(int n, const T* __restrict__ pos, const T* __res
                                 const int* __restrict__ gorder, const int* __restrict__ gcell,
                                 typename Vec4<T>::type* __restrict__ prec,
                                 typename Vec4<T>::type* __restrict__ grec, int* __restrict__ gcell_sorted,
-                                int* __restrict__ pcellx) {
+                                int* __restrict__ pbinx) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= n) return;
   {
     const int i = porder[k];
     int c = pcell[i];
-    const int cx = c % g.nc[0]; c /= g.nc[0];
+    const int nbx = g.nc[0] << g.sxs;
+    const int bx = c % nbx; c /= nbx;                  // sub-bin along x
+    const int cx = bx >> g.sxs;
     const int cy = c % g.nc[1], cz = c / g.nc[1];
     const int cc[3] = {cx, cy, cz};
     T r[3];
@@ -182,7 +189,7 @@ __global__ void k_build_records(int n, const T* __restrict__ pos, const T* __res
       r[ax] = (T)(x - cc[ax] * g.cell_edge[ax]);
     }
     prec[k] = make_vec4<T>(r[0], r[1], r[2], q[i]);
-    pcellx[k] = cx;
+    pbinx[k] = bx;
   }
   {
     const int i = gorder[k];
