@@ -19,7 +19,7 @@ FP32_ENERGY_RTOL = 1e-5
 FP32_FORCE_RMS_RTOL = 1e-4
 # fp32 mode, outputs without a north-star bound (DESIGN.md section 3 "Tolerances"): key -> bound;
 # "Q" / "E" apply to the grids of every tiled level
-FP32_BOUNDS = {"force_rms": 3e-6, "force_max": 6e-6, "potential_max": 2e-5, "virial": 2e-5, "Q": 6e-6, "E": 3e-4}
+FP32_BOUNDS = {"force_rms": 1e-5, "force_max": 2e-5, "potential_max": 2e-5, "virial": 2e-5, "Q": 6e-6, "E": 3e-4}
 
 
 def run_oracle(w, mu=4, want_virial=True):
