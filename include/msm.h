@@ -97,19 +97,43 @@ msm_status_t msm_plan_info(const msm_plan_t *plan, msm_plan_info_t *info_out);
  *   h_virial     host, 6 doubles xx yy zz xy xz yz of -dU/d eps_ab (number of grid points and a
  *                fixed, reading V); may be NULL (the strain-derivative work is then skipped).
  * The caller owns all six buffers; the plan owns every scratch buffer and msm_evaluate allocates
- * nothing.  The work is ordered after everything already enqueued on cuda_stream, and the call
- * returns only when it is complete (it always reads back the status flag, the energy and the virial
- * in one small copy).  From the second consecutive call with identical arguments on, the launch
- * sequence is captured into a CUDA graph and replayed on a plan-owned stream (a small system is
- * otherwise bound by its ~40-60 dependent kernel launches); results are bit-identical either way.
- * MSM_NO_GRAPH=1 in the environment at plan creation disables this.  The short-range pair kernel
- * runs on a second plan-owned stream beside the grid pipeline and joins before the interpolation
- * (not while per-stage profiling is on; MSM_NO_OVERLAP=1 disables it).
+ * nothing. The work is stream-ordered: it starts after everything already enqueued on cuda_stream,
+ * and work enqueued on cuda_stream afterwards sees d_forces / d_potentials. If h_energy or
+ * h_virial is non-NULL the call waits for the evaluation and fills them (and reports
+ * MSM_ERR_OUT_OF_BOX); if both are NULL it returns as soon as the work is enqueued, without any
+ * host synchronisation (msm_get_results waits and reports later). A plan has one set of scratch
+ * buffers: a second evaluation, on whatever stream, is ordered on the device behind the first.
+ * From the second consecutive call with identical arguments on, the launch sequence is captured
+ * into a CUDA graph and replayed on a plan-owned stream that is forked from and joined back into
+ * cuda_stream (a small system is otherwise bound by its ~40-60 dependent kernel launches); results
+ * are bit-identical either way. The short-range pair kernel runs on a second plan-owned stream
+ * beside the grid pipeline and joins before the interpolation (not while per-stage profiling is
+ * on).
  * Neutrality is assumed on periodic axes: the single-point top level contributes zero (reading
- * T2), which for a non-neutral input is the neutralising-background convention. */
+ * T2), which for a non-neutral input is the neutralising-background convention.
+ *
+ * Environment knobs, read once at msm_plan_create (debugging and measurement only; none changes a
+ * result beyond rounding order): MSM_NO_GRAPH=1 (no CUDA-graph replay), MSM_NO_OVERLAP=1 (every
+ * kernel on the caller's stream), MSM_GRID_STREAM_MIN=<points> (finest-grid size from which the
+ * one-sweep restriction / prolongation / filter kernels run; default 4 Mi points for restriction
+ * and filter, 0 for prolongation), MSM_FILTER_STREAM_MIN=<points> (the same for the filter alone),
+ * MSM_CONV_SLICES=<n> (input-plane slices per convolution tile), MSM_CONV_GLOBAL_TAPS=1 (fp32
+ * convolution reads its stencil tables from global memory), MSM_ANTERP_TILED=0 /
+ * MSM_ANTERP_MIN_TILES=<n> (choice between the tiled and the gather anterpolation),
+ * MSM_PAIR_SUBBINS_LOG2=<0..3> (x sub-bins per pair cell). */
 msm_status_t msm_evaluate(msm_plan_t *plan, int n, const void *d_positions, const void *d_charges,
                           void *d_forces, void *d_potentials, double *h_energy, double *h_virial,
                           void *cuda_stream);
+
+/* msm_evaluate without host outputs: enqueue only, never synchronises. want_virial != 0 also runs
+ * the strain-derivative work (its result is read with msm_get_results). */
+msm_status_t msm_evaluate_async(msm_plan_t *plan, int n, const void *d_positions, const void *d_charges,
+                                void *d_forces, void *d_potentials, int want_virial, void *cuda_stream);
+
+/* Wait for the plan's last evaluation and return its energy (1 double) and virial (6 doubles,
+ * zeros if it was not requested); either pointer may be NULL. Returns MSM_ERR_OUT_OF_BOX if that
+ * evaluation saw a coordinate outside an open axis or a non-finite input. */
+msm_status_t msm_get_results(msm_plan_t *plan, double *h_energy, double *h_virial);
 
 /* The same call with HOST buffers (the end-to-end path): copies positions and charges to plan-
  * owned device staging, evaluates, copies forces and potentials back. Pointers are host memory

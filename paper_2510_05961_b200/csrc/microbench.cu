@@ -80,7 +80,10 @@ template <typename T> msm_status_t measure(double* tflops, bool packed = false) 
 
 extern "C" msm_status_t msm_measure_fma_peak(int device, int kind, double* tflops) {
   if (!tflops || kind < 0 || kind > 2) return MSM_ERR_INVALID_ARG;
+  int prev = -1;
+  if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
   if (cudaSetDevice(device) != cudaSuccess) return MSM_ERR_CUDA;
-  if (kind == 2) return measure<float>(tflops, true);
-  return kind == 0 ? measure<float>(tflops) : measure<double>(tflops);
+  const msm_status_t s = kind == 2 ? measure<float>(tflops, true) : (kind == 0 ? measure<float>(tflops) : measure<double>(tflops));
+  if (prev >= 0) cudaSetDevice(prev);
+  return s;
 }

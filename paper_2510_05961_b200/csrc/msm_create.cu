@@ -427,7 +427,8 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   for (int i = 0; i <= kMaxStages; ++i)
     if (cudaEventCreate(&p->ev[i]) != cudaSuccess) return MSM_ERR_CUDA;
   if (cudaStreamCreateWithFlags(&p->gstream, cudaStreamNonBlocking) != cudaSuccess ||
-      cudaEventCreateWithFlags(&p->gev, cudaEventDisableTiming) != cudaSuccess)
+      cudaEventCreateWithFlags(&p->gev, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->done_ev, cudaEventDisableTiming) != cudaSuccess)
     return MSM_ERR_CUDA;
   if (const char* e = std::getenv("MSM_NO_GRAPH")) p->graph_enabled = std::atoi(e) == 0;
   if (cudaStreamCreateWithFlags(&p->pstream, cudaStreamNonBlocking) != cudaSuccess ||
@@ -455,6 +456,8 @@ extern "C" {
 
 void msm_plan_destroy(msm_plan_t* p) {
   if (!p) return;
+  DeviceGuard dg(p->prm.device);
+  if (p->pending) cudaEventSynchronize(p->done_ev);
   for (void* d : p->allocs) cudaFree(d);
   if (p->pstream) cudaStreamDestroy(p->pstream);
   if (p->vstream) cudaStreamDestroy(p->vstream);
@@ -465,6 +468,7 @@ void msm_plan_destroy(msm_plan_t* p) {
   if (p->gexec) cudaGraphExecDestroy(p->gexec);
   if (p->gstream) cudaStreamDestroy(p->gstream);
   if (p->gev) cudaEventDestroy(p->gev);
+  if (p->done_ev) cudaEventDestroy(p->done_ev);
   if (p->h_results) cudaFreeHost(p->h_results);
   for (int i = 0; i <= kMaxStages; ++i)
     if (p->ev[i]) cudaEventDestroy(p->ev[i]);
@@ -479,6 +483,8 @@ msm_status_t msm_plan_create(const msm_params_t* params, msm_plan_t** plan_out) 
   msm_plan* p = new (std::nothrow) msm_plan();
   if (!p) return MSM_ERR_NOMEM;
   msm_status_t st;
+  int prev_dev = -1;
+  if (cudaGetDevice(&prev_dev) != cudaSuccess) { prev_dev = -1; cudaGetLastError(); }
   try {
     st = create_impl(params, p);
   } catch (const std::bad_alloc&) {
@@ -488,7 +494,13 @@ msm_status_t msm_plan_create(const msm_params_t* params, msm_plan_t** plan_out) 
   } catch (...) {
     st = MSM_ERR_CUDA;
   }
-  if (st != MSM_OK) { cudaGetLastError(); msm_plan_destroy(p); return st; }
+  if (st != MSM_OK) {
+    cudaGetLastError();
+    msm_plan_destroy(p);
+    if (prev_dev >= 0) cudaSetDevice(prev_dev);
+    return st;
+  }
+  if (prev_dev >= 0) cudaSetDevice(prev_dev);      // the caller's current device is left as it was
   *plan_out = p;
   return MSM_OK;
 }

@@ -546,9 +546,11 @@ msm_status_t enqueue(msm_plan* p, int n, const void* pos, const void* q, void* F
   return MSM_ERR_UNSUPPORTED;
 }
 
-// wait for the evaluation enqueued on st, then read the stage times
-msm_status_t finish(msm_plan* p, cudaStream_t st) {
-  if (cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }
+// wait for the last enqueued evaluation, then read the stage times
+msm_status_t finish(msm_plan* p) {
+  if (!p->pending) return MSM_OK;
+  p->pending = false;
+  if (cudaEventSynchronize(p->done_ev) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }
   if (cudaGetLastError() != cudaSuccess) return MSM_ERR_CUDA;
   if (p->profiling)
     for (int i = 0; i < p->n_stages; ++i) cudaEventElapsedTime(&p->stage_ms[i], p->ev[i], p->ev[i + 1]);
@@ -559,12 +561,18 @@ void drop_graph(msm_plan* p) {
   if (p->gexec) { cudaGraphExecDestroy(p->gexec); p->gexec = nullptr; }
 }
 
-// One evaluation. The ~40-60 dependent launches of a small system cost more than their work, so the
-// second consecutive call with the same arguments captures the launch sequence into a CUDA graph
-// (on a plan-owned stream) and later calls replay it; any change of arguments, or any failure of
-// the capture, falls back to direct launches on the caller's stream.
+// One evaluation, stream-ordered on st: returns as soon as the work is enqueued. The ~40-60 dependent
+// launches of a small system cost more than their work, so the second consecutive call with the
+// same arguments captures the launch sequence into a CUDA graph (on a plan-owned stream) and later
+// calls replay it, ordered after everything already enqueued on st and joined back into st (work
+// enqueued on st afterwards sees the outputs). Any change of arguments, or any failure of the
+// capture, falls back to direct launches on the caller's stream.
 msm_status_t run(msm_plan* p, int n, const void* pos, const void* q, void* F, void* V, bool wv, cudaStream_t st) {
+  // the plan's scratch buffers are single: an evaluation still running (possibly on another stream)
+  // is ordered in front of this one on the device; the host does not wait
+  if (p->pending && cudaStreamWaitEvent(st, p->done_ev, 0) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }
   const msm::GraphKey key{n, pos, q, F, V, wv, p->profiling};
+  p->pending_virial = wv;
   if (p->graph_enabled && p->gstream && key == p->gkey) {
     if (!p->gexec) {
       cudaGraph_t g = nullptr;
@@ -578,10 +586,12 @@ msm_status_t run(msm_plan* p, int n, const void* pos, const void* q, void* F, vo
       if (!p->gexec) { cudaGetLastError(); p->graph_enabled = false; }   // never try again on this plan
     }
     if (p->gexec) {
-      // order the replay after the caller's stream; the call synchronises before it returns
       if (cudaEventRecord(p->gev, st) == cudaSuccess && cudaStreamWaitEvent(p->gstream, p->gev, 0) == cudaSuccess &&
-          cudaGraphLaunch(p->gexec, p->gstream) == cudaSuccess)
-        return finish(p, p->gstream);
+          cudaGraphLaunch(p->gexec, p->gstream) == cudaSuccess && cudaEventRecord(p->done_ev, p->gstream) == cudaSuccess &&
+          cudaStreamWaitEvent(st, p->done_ev, 0) == cudaSuccess) {
+        p->pending = true;
+        return MSM_OK;
+      }
       cudaGetLastError();
       drop_graph(p);
       p->graph_enabled = false;
@@ -592,45 +602,75 @@ msm_status_t run(msm_plan* p, int n, const void* pos, const void* q, void* F, vo
   }
   const msm_status_t es = enqueue(p, n, pos, q, F, V, wv, st, false);
   if (es != MSM_OK) return es;
-  return finish(p, st);
+  if (cudaEventRecord(p->done_ev, st) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }
+  p->pending = true;
+  return MSM_OK;
+}
+
+msm_status_t check_args(msm_plan* p, int n, const void* pos, const void* q) {
+  if (!p || n < 0 || (n > 0 && (!pos || !q))) return MSM_ERR_INVALID_ARG;
+  if (n > p->cap) return MSM_ERR_TOO_MANY_PARTICLES;
+  return MSM_OK;
 }
 
 }  // namespace
 
 extern "C" {
 
-msm_status_t msm_evaluate(msm_plan_t* p, int n, const void* d_positions, const void* d_charges, void* d_forces,
-                          void* d_potentials, double* h_energy, double* h_virial, void* cuda_stream) {
-  if (!p || n < 0 || (n > 0 && (!d_positions || !d_charges))) return MSM_ERR_INVALID_ARG;
-  if (n > p->cap) return MSM_ERR_TOO_MANY_PARTICLES;
-  if (cudaSetDevice(p->prm.device) != cudaSuccess) return MSM_ERR_CUDA;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  const bool wv = h_virial != nullptr;
-  const msm_status_t s = run(p, n, d_positions, d_charges, d_forces, d_potentials, wv, st);
+msm_status_t msm_evaluate_async(msm_plan_t* p, int n, const void* d_positions, const void* d_charges, void* d_forces,
+                                void* d_potentials, int want_virial, void* cuda_stream) {
+  const msm_status_t a = check_args(p, n, d_positions, d_charges);
+  if (a != MSM_OK) return a;
+  DeviceGuard dg(p->prm.device);
+  if (!dg.ok) return MSM_ERR_CUDA;
+  return run(p, n, d_positions, d_charges, d_forces, d_potentials, want_virial != 0, (cudaStream_t)cuda_stream);
+}
+
+msm_status_t msm_get_results(msm_plan_t* p, double* h_energy, double* h_virial) {
+  if (!p) return MSM_ERR_INVALID_ARG;
+  DeviceGuard dg(p->prm.device);
+  if (!dg.ok) return MSM_ERR_CUDA;
+  const msm_status_t s = finish(p);
   if (s != MSM_OK) return s;
   if (h_energy) *h_energy = p->h_results[0];
-  if (h_virial) std::memcpy(h_virial, p->h_results + 1, 6 * sizeof(double));
+  if (h_virial) {
+    if (p->pending_virial) std::memcpy(h_virial, p->h_results + 1, 6 * sizeof(double));
+    else std::memset(h_virial, 0, 6 * sizeof(double));
+  }
   if (p->h_results[7] != 0.0) return MSM_ERR_OUT_OF_BOX;
   return MSM_OK;
 }
 
+msm_status_t msm_evaluate(msm_plan_t* p, int n, const void* d_positions, const void* d_charges, void* d_forces,
+                          void* d_potentials, double* h_energy, double* h_virial, void* cuda_stream) {
+  const msm_status_t s = msm_evaluate_async(p, n, d_positions, d_charges, d_forces, d_potentials, h_virial != nullptr,
+                                            cuda_stream);
+  if (s != MSM_OK) return s;
+  if (!h_energy && !h_virial) return MSM_OK;       // stream-ordered: no host output, no synchronisation
+  return msm_get_results(p, h_energy, h_virial);
+}
+
 msm_status_t msm_evaluate_host(msm_plan_t* p, int n, const void* h_positions, const void* h_charges, void* h_forces,
                                void* h_potentials, double* h_energy, double* h_virial, void* cuda_stream) {
-  if (!p || n < 0 || (n > 0 && (!h_positions || !h_charges))) return MSM_ERR_INVALID_ARG;
-  if (n > p->cap) return MSM_ERR_TOO_MANY_PARTICLES;
-  if (cudaSetDevice(p->prm.device) != cudaSuccess) return MSM_ERR_CUDA;
+  const msm_status_t a = check_args(p, n, h_positions, h_charges);
+  if (a != MSM_OK) return a;
+  DeviceGuard dg(p->prm.device);
+  if (!dg.ok) return MSM_ERR_CUDA;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t e = p->esz;
+  msm_status_t fs = finish(p);                      // the staging buffers may still be in use
+  if (fs != MSM_OK) return fs;
   if (cudaMemcpyAsync(p->in_pos, h_positions, (size_t)n * 3 * e, cudaMemcpyHostToDevice, st) != cudaSuccess ||
       cudaMemcpyAsync(p->in_q, h_charges, (size_t)n * e, cudaMemcpyHostToDevice, st) != cudaSuccess) {
     cudaGetLastError();
     return MSM_ERR_CUDA;
   }
-  const msm_status_t s = msm_evaluate(p, n, p->in_pos, p->in_q, h_forces ? p->out_F : nullptr,
-                                      h_potentials ? p->out_V : nullptr, h_energy, h_virial, cuda_stream);
-  if (s != MSM_OK && s != MSM_ERR_OUT_OF_BOX) return s;
+  msm_status_t s = msm_evaluate_async(p, n, p->in_pos, p->in_q, h_forces ? p->out_F : nullptr,
+                                      h_potentials ? p->out_V : nullptr, h_virial != nullptr, cuda_stream);
+  if (s != MSM_OK) return s;
   if (h_forces) cudaMemcpyAsync(h_forces, p->out_F, (size_t)n * 3 * e, cudaMemcpyDeviceToHost, st);
   if (h_potentials) cudaMemcpyAsync(h_potentials, p->out_V, (size_t)n * e, cudaMemcpyDeviceToHost, st);
+  s = msm_get_results(p, h_energy, h_virial);
   if (cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }
   return s;
 }
@@ -660,10 +700,14 @@ msm_status_t msm_debug_copy_grid(const msm_plan_t* p, int level, int kind, doubl
   if (!p || !h_out || level < 1 || level > p->n_t || (kind != 0 && kind != 1)) return MSM_ERR_INVALID_ARG;
   const size_t pts = p->H->lev[level].points();
   if (capacity < pts) return MSM_ERR_INVALID_ARG;
+  DeviceGuard dg(p->prm.device);
+  if (!dg.ok) return MSM_ERR_CUDA;
+  if (p->pending && cudaEventSynchronize(p->done_ev) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }
   const void* src = kind == 0 ? p->lev[level].Q : p->lev[level].E;
   if (p->fp32) {
-    std::vector<float> tmp(pts);
-    if (cudaMemcpy(tmp.data(), src, pts * 4, cudaMemcpyDeviceToHost) != cudaSuccess) return MSM_ERR_CUDA;
+    // fp32 values are exact in fp64: copy into the upper half of the caller's buffer, widen in place
+    float* tmp = reinterpret_cast<float*>(h_out) + pts;
+    if (cudaMemcpy(tmp, src, pts * 4, cudaMemcpyDeviceToHost) != cudaSuccess) return MSM_ERR_CUDA;
     for (size_t i = 0; i < pts; ++i) h_out[i] = tmp[i];
   } else if (cudaMemcpy(h_out, src, pts * 8, cudaMemcpyDeviceToHost) != cudaSuccess) {
     return MSM_ERR_CUDA;

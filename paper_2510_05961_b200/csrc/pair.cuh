@@ -161,7 +161,7 @@ __device__ __forceinline__ void pair_interact(PairAcc<T>& A, T dx, T dy, T dz, T
 }
 
 template <typename T, int P, bool VIRIAL, bool MI>
-__global__ void __launch_bounds__(PairWarps<T>::value * 32, sizeof(T) == 4 ? 6 : 1)
+__global__ void __launch_bounds__(PairWarps<T>::value * 32, sizeof(T) == 4 ? 6 : 8)
 k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>::type* __restrict__ prec,
        const int* __restrict__ pbinx, const int* __restrict__ porder, T* __restrict__ Fsr,
        T* __restrict__ Vsr, double* __restrict__ wpart) {

@@ -31,6 +31,17 @@ struct GraphKey {
   }
 };
 
+// makes the plan's device current for the duration of an entry point and restores the caller's
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+    ok = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 }  // namespace msm
 
 struct msm_plan {
@@ -94,6 +105,9 @@ struct msm_plan {
   cudaStream_t gstream = nullptr;
   cudaGraphExec_t gexec = nullptr;
   cudaEvent_t gev = nullptr;
+  // completion of the last enqueued evaluation (msm_get_results waits on it)
+  cudaEvent_t done_ev = nullptr;
+  bool pending = false, pending_virial = false;
 
   // fine grids with at least this many points take the one-sweep restriction / prolongation
   // kernels of gridops_stream.cuh (the restriction only pays when the grid does not fit the L2;

@@ -21,7 +21,8 @@ MSM_MAX_LEVELS = 32
 STATUS = {0: "MSM_OK", 1: "MSM_ERR_INVALID_ARG", 2: "MSM_ERR_UNSUPPORTED", 3: "MSM_ERR_CUTOFF_TOO_LARGE",
           4: "MSM_ERR_TOO_MANY_PARTICLES", 5: "MSM_ERR_OUT_OF_BOX", 6: "MSM_ERR_NOMEM", 7: "MSM_ERR_CUDA"}
 
-EXPORTS = ["msm_plan_create", "msm_plan_info", "msm_evaluate", "msm_evaluate_host", "msm_set_profiling",
+EXPORTS = ["msm_plan_create", "msm_plan_info", "msm_evaluate", "msm_evaluate_async", "msm_get_results",
+           "msm_evaluate_host", "msm_set_profiling",
            "msm_get_stage_times", "msm_get_launch_count", "msm_debug_copy_grid", "msm_plan_destroy",
            "msm_status_string", "msm_measure_fma_peak"]
 
@@ -57,6 +58,8 @@ def lib():
         L.msm_plan_create.restype = i; L.msm_plan_create.argtypes = [C.POINTER(Params), C.POINTER(vp)]
         L.msm_plan_info.restype = i; L.msm_plan_info.argtypes = [vp, C.POINTER(PlanInfo)]
         L.msm_evaluate.restype = i; L.msm_evaluate.argtypes = [vp, i, vp, vp, vp, vp, dp, dp, vp]
+        L.msm_evaluate_async.restype = i; L.msm_evaluate_async.argtypes = [vp, i, vp, vp, vp, vp, i, vp]
+        L.msm_get_results.restype = i; L.msm_get_results.argtypes = [vp, dp, dp]
         L.msm_evaluate_host.restype = i; L.msm_evaluate_host.argtypes = [vp, i, vp, vp, vp, vp, dp, dp, vp]
         L.msm_set_profiling.restype = i; L.msm_set_profiling.argtypes = [vp, i]
         L.msm_get_stage_times.restype = i
@@ -140,6 +143,31 @@ class Plan:
         if st:
             raise MsmError(st, "msm_evaluate")
         return (e.value if want_energy else None), (np.array(w[:]) if want_virial else None)
+
+    def evaluate_async(self, positions, charges, forces=None, potentials=None, want_virial=False, stream=None):
+        """Enqueue one evaluation on `stream` (default: torch's current stream) and return at once;
+        forces / potentials are valid for work enqueued on that stream afterwards. results() waits."""
+        import torch
+        n = int(charges.shape[0])
+        for t in (positions, charges, forces, potentials):
+            if t is not None:
+                assert t.is_cuda and t.dtype == self.torch_dtype and t.is_contiguous()
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        st = lib().msm_evaluate_async(self._h, n, positions.data_ptr(), charges.data_ptr(),
+                                      forces.data_ptr() if forces is not None else None,
+                                      potentials.data_ptr() if potentials is not None else None,
+                                      1 if want_virial else 0, C.c_void_p(s.cuda_stream))
+        if st:
+            raise MsmError(st, "msm_evaluate_async")
+
+    def results(self):
+        """Wait for the last evaluation -> (energy, virial ndarray(6))."""
+        e = C.c_double(0.0)
+        w = (C.c_double * 6)()
+        st = lib().msm_get_results(self._h, C.byref(e), w)
+        if st:
+            raise MsmError(st, "msm_get_results")
+        return e.value, np.array(w[:])
 
     def evaluate_host(self, positions, charges, forces=None, potentials=None, want_virial=True, stream=None):
         """The same call on HOST buffers (numpy arrays or pinned CPU tensors of the plan's dtype)."""

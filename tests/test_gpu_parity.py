@@ -475,3 +475,51 @@ def test_non_default_stream_and_null_outputs():
     V.zero_()
     U, W = plan.evaluate(pos, q, None, V, want_energy=False, want_virial=True)
     assert U is None and np.array_equal(W, W0) and torch.equal(V, V0)
+
+
+def test_stream_ordered_evaluation_overlaps_caller_work():
+    """msm_evaluate with no host output (msm_evaluate_async) only enqueues: the call returns while
+    the GPU is still busy, a caller kernel on another stream runs beside it, work enqueued on the
+    same stream afterwards sees the forces, and msm_get_results delivers energy and virial later;
+    a second evaluation is ordered behind the first on the device. Results are bit-identical to
+    the synchronous call."""
+    import time
+    import torch
+    from paper_2510_05961_b200 import msm
+    from paper_2510_05961_b200.workloads import make_workload
+    w = make_workload("cfg4_water300k")
+    dev = torch.device("cuda", 0)
+    plan = msm.Plan.for_workload(w, "fp32")
+    pos = torch.tensor(w.positions, dtype=torch.float32, device=dev); q = torch.tensor(w.charges, dtype=torch.float32, device=dev)
+    F = torch.zeros((w.n, 3), dtype=torch.float32, device=dev); V = torch.zeros(w.n, dtype=torch.float32, device=dev)
+    U0, W0 = plan.evaluate(pos, q, F, V)
+    F0, V0 = F.clone(), V.clone()
+    s1, s2 = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+    big = torch.zeros(64 << 20, dtype=torch.float32, device=dev)
+    torch.cuda.synchronize()
+    for rep in range(3):                       # direct launches, capture, replay
+        F.zero_(); V.zero_()
+        torch.cuda.synchronize()
+        ev0, ev1, ev2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        with torch.cuda.stream(s1):
+            ev0.record()
+            t0 = time.perf_counter()
+            plan.evaluate_async(pos, q, F, V, want_virial=True, stream=s1)
+            t_call = time.perf_counter() - t0
+            Fsum = F.sum()                     # same stream: must see the forces
+            ev1.record()
+        with torch.cuda.stream(s2):            # caller work on another stream, not serialised behind the evaluation
+            big.add_(1.0)
+            ev2.record()
+        busy = not ev1.query()                 # the call came back before the GPU finished
+        U, W = plan.results()
+        torch.cuda.synchronize()
+        assert U == U0 and np.array_equal(W, W0) and torch.equal(F, F0) and torch.equal(V, V0)
+        assert float(Fsum) == float(F0.sum())
+        assert t_call < 0.5e-3 * 20 and (busy or rep == 0), (t_call, busy)
+    # two evaluations back to back without reading results in between: the second waits on the device
+    plan.evaluate_async(pos, q, F, V, want_virial=True, stream=s1)
+    plan.evaluate_async(pos, q, F, V, want_virial=True, stream=s2)
+    U, W = plan.results()
+    torch.cuda.synchronize()
+    assert U == U0 and np.array_equal(W, W0) and torch.equal(F, F0)
