@@ -435,13 +435,18 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
           for (int o = 16; o > 0; o >>= 1) nmax = max(nmax, __shfl_xor_sync(0xffffffffu, nmax, o));
           __syncwarp();
           // drain: hit r of every lane that has one, in full precision (exact cutoff test)
-          for (int r = 0; r < nmax; ++r) {
-            if (r < n) {
-              const V4 pj = sj.full(lp[r * 32]);
-              const T dx = xi - pj.x, dy = yi - pj.y, dz = zi - pj.z;
-              const T r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-              if (r2 < a2) pair_interact<T, P, MODE>(A, dx, dy, dz, r2, pj.w, inv_a, inv_a2, two_inv_a3, cf, cd);
-            }
+          // Two hits per lane and round, branch-free (a missing hit or one outside the exact cutoff
+          // takes charge 0 and a harmless distance), so that the two dependent chains of ~45 DFMA
+          // interleave instead of running one after the other.
+          for (int r = 0; r < nmax; r += 2) {
+            const bool v0 = r < n, v1 = r + 1 < n;
+            const V4 p0 = sj.full(v0 ? lp[r * 32] : 0), p1 = sj.full(v1 ? lp[(r + 1) * 32] : 0);
+            const T dx0 = xi - p0.x, dy0 = yi - p0.y, dz0 = zi - p0.z;
+            const T dx1 = xi - p1.x, dy1 = yi - p1.y, dz1 = zi - p1.z;
+            const T s0 = fma(dx0, dx0, fma(dy0, dy0, dz0 * dz0)), s1 = fma(dx1, dx1, fma(dy1, dy1, dz1 * dz1));
+            const T q0 = (v0 && s0 < a2) ? p0.w : (T)0, q1 = (v1 && s1 < a2) ? p1.w : (T)0;
+            pair_interact<T, P, MODE>(A, dx0, dy0, dz0, max(s0, (T)1e-30), q0, inv_a, inv_a2, two_inv_a3, cf, cd);
+            pair_interact<T, P, MODE>(A, dx1, dy1, dz1, max(s1, (T)1e-30), q1, inv_a, inv_a2, two_inv_a3, cf, cd);
           }
           __syncwarp();
         } else {
