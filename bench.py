@@ -332,6 +332,43 @@ def measure(w, prec, local, dev, steps, warmup, world, flush, sampler=None, full
     return res
 
 
+def batch_bench(local, dev, B=64, steps=10, warmup=3):
+    """Section 8(f) rank 2: B systems of config 1's shape (512 charges, open 20 A cube, fp64, p = 4,
+    h = 2, a = 6, 3 levels) evaluated one at a time (msm_evaluate, graph replay) and as one batch
+    (msm_evaluate_batch): particles/s of both and their ratio; energy + forces + potentials + virial."""
+    import numpy as np
+    import torch
+    from paper_2510_05961_b200 import msm
+    cap = 512
+    rng = np.random.default_rng(7)
+    pos = rng.random((B, cap, 3)) * 20.0
+    q = np.tile(np.where(np.arange(cap) % 2 == 0, 1.0, -1.0), (B, 1))
+    tp = torch.tensor(pos, device=dev); tq = torch.tensor(q, device=dev)
+    F = torch.zeros((B, cap, 3), dtype=torch.float64, device=dev); V = torch.zeros((B, cap), dtype=torch.float64, device=dev)
+    n = [cap] * B
+
+    def timed(fn):
+        for _ in range(warmup):
+            fn()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for s in range(steps):
+            ev[s][0].record(); fn(); ev[s][1].record()
+            torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in ev) / steps
+
+    plan = msm.Plan((20.0,) * 3, (0, 0, 0), 2.0, 6.0, 4, 3, "fp64", max_particles=cap, device=local)
+    p0, q0, F0, V0 = tp[0].contiguous(), tq[0].contiguous(), F[0], V[0]
+    ms_one = timed(lambda: plan.evaluate(p0, q0, F0, V0))
+    plan.close()
+    batch = msm.Batch(B, (20.0,) * 3, (0, 0, 0), 2.0, 6.0, 4, 3, "fp64", max_particles=cap, device=local)
+    ms_batch = timed(lambda: batch.evaluate(n, tp, tq, F, V))
+    batch.close()
+    return {"systems": B, "particles_per_system": cap, "dtype": "f64", "workload": "cfg1_open512 shape",
+            "one_at_a_time": {"ms_per_system": ms_one, "value": cap / (ms_one * 1e-3), "unit": UNIT},
+            "batched": {"ms_per_batch": ms_batch, "value": B * cap / (ms_batch * 1e-3), "unit": UNIT},
+            "speedup": ms_one * B / ms_batch}
+
+
 def np_prod(v):
     r = 1
     for x in v:
@@ -376,6 +413,7 @@ def run_ours(args, rank: int, world: int):
                 r["workload"] = name
                 sweep[key].append(r)
                 del ws
+    batch = batch_bench(local, dev) if extras else None
     if sampler:
         sampler.stop()
     if rank != 0:
@@ -396,6 +434,8 @@ def run_ours(args, rank: int, world: int):
         out["fp64"] = fp64
     if sweep:
         out["sweep"] = sweep
+    if batch:
+        out["batch"] = batch
     if world == 1 and args.grid_microbench > 0:
         peaks, _ = load_peaks()
         out["grid_microbench"] = grid_microbench(args.grid_microbench, local, peaks["hbm_gbs"])
@@ -502,11 +542,17 @@ def main():
     ap.add_argument("--grid-microbench", type=int, default=512,
                     help="finest grid size M (power of two) of the HBM-bound grid-stage measurement; 0 skips it")
     ap.add_argument("--only-grid-microbench", action="store_true", help="print the grid_microbench object alone")
+    ap.add_argument("--only-batch", action="store_true", help="print the batch object alone")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.only_grid_microbench:
         print(json.dumps({"grid_microbench": grid_microbench(args.grid_microbench, 0, load_peaks()[0]["hbm_gbs"])}), flush=True)
+        return
+    if args.only_batch:
+        import torch
+        torch.cuda.set_device(0)
+        print(json.dumps({"batch": batch_bench(0, torch.device("cuda", 0))}), flush=True)
         return
     if args.impl == "reference":
         args.steps = args.steps if args.steps is not None else 2

@@ -28,6 +28,7 @@ extern "C" {
 #endif
 
 typedef struct msm_plan msm_plan_t; /* opaque; owns all device and host scratch buffers */
+typedef struct msm_batch msm_batch_t; /* opaque; B plans of one geometry + the graph that runs them together */
 
 typedef enum {
   MSM_OK = 0,
@@ -159,6 +160,24 @@ msm_status_t msm_debug_copy_grid(const msm_plan_t *plan, int level, int kind, do
                                  size_t capacity);
 
 void msm_plan_destroy(msm_plan_t *plan);
+
+/* Batched evaluation of `batch` independent small systems that share one geometry (box,
+ * periodicity, h, a, p, levels, precision): the paper's batching of structures with fixed grid
+ * counts and zero-charge padding, for the regime where one small system is dominated
+ * by a constant overhead. Every system gets its own scratch buffers; the launch sequences
+ * of all systems are captured as parallel branches of one CUDA graph and run side by side.
+ *   h_n           host, batch ints: particles of each system (<= params->max_particles)
+ *   d_positions   device, [batch][max_particles][3]; d_charges device, [batch][max_particles]:
+ *                 system b uses the first h_n[b] entries of its slot (the rest is padding)
+ *   d_forces / d_potentials  device, same layout, may be NULL
+ *   h_energy      host, batch doubles; h_virial host, batch x 6 doubles; either may be NULL. With
+ *                 both NULL the call is stream-ordered and does not synchronise.
+ * The graph is rebuilt when any argument changes. Results equal msm_evaluate's for each system. */
+msm_status_t msm_batch_create(const msm_params_t *params, int batch, msm_batch_t **batch_out);
+msm_status_t msm_evaluate_batch(msm_batch_t *batch, const int *h_n, const void *d_positions,
+                                const void *d_charges, void *d_forces, void *d_potentials,
+                                double *h_energy, double *h_virial, void *cuda_stream);
+void msm_batch_destroy(msm_batch_t *batch);
 
 const char *msm_status_string(msm_status_t s);
 

@@ -716,3 +716,156 @@ msm_status_t msm_debug_copy_grid(const msm_plan_t* p, int level, int kind, doubl
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// Batched evaluation of many small systems of one geometry (msmJAX batches structures
+// with vmap, fixed grid counts and zero-charge padding; a small system is dominated by a
+// constant overhead). One evaluation of a 512-particle system is a chain of ~40 dependent kernel
+// launches that leaves the GPU almost empty; a batch is B such chains captured as parallel branches
+// of ONE CUDA graph: every system has its own scratch (a plan of the shared geometry), the
+// branches are spread over a pool of streams, and one graph launch runs them side by side.
+struct msm_batch {
+  int B = 0, device = 0, cap = 0, nstreams = 0;
+  size_t esz = 8;
+  std::vector<msm_plan*> plans;
+  std::vector<cudaStream_t> streams;
+  std::vector<cudaEvent_t> join_ev;
+  cudaStream_t origin = nullptr;
+  cudaEvent_t fork_ev = nullptr, in_ev = nullptr, done_ev = nullptr;
+  cudaGraphExec_t gexec = nullptr;
+  // arguments of the captured graph
+  std::vector<int> n;
+  const void *pos = nullptr, *q = nullptr;
+  void *F = nullptr, *V = nullptr;
+  bool virial = false;
+};
+
+namespace {
+constexpr int kBatchStreams = 32;
+
+void batch_drop_graph(msm_batch* b) {
+  if (b->gexec) { cudaGraphExecDestroy(b->gexec); b->gexec = nullptr; }
+}
+}  // namespace
+
+extern "C" {
+
+void msm_batch_destroy(msm_batch_t* b) {
+  if (!b) return;
+  DeviceGuard dg(b->device);
+  if (b->origin) cudaStreamSynchronize(b->origin);
+  batch_drop_graph(b);
+  for (msm_plan* p : b->plans) msm_plan_destroy(p);
+  for (cudaStream_t s : b->streams) cudaStreamDestroy(s);
+  for (cudaEvent_t e : b->join_ev) cudaEventDestroy(e);
+  if (b->fork_ev) cudaEventDestroy(b->fork_ev);
+  if (b->in_ev) cudaEventDestroy(b->in_ev);
+  if (b->done_ev) cudaEventDestroy(b->done_ev);
+  if (b->origin) cudaStreamDestroy(b->origin);
+  delete b;
+}
+
+msm_status_t msm_batch_create(const msm_params_t* params, int batch, msm_batch_t** batch_out) {
+  if (!batch_out) return MSM_ERR_INVALID_ARG;
+  *batch_out = nullptr;
+  if (!params || batch < 1 || batch > 65536) return MSM_ERR_INVALID_ARG;
+  msm_batch* b = new (std::nothrow) msm_batch();
+  if (!b) return MSM_ERR_NOMEM;
+  b->B = batch; b->device = params->device; b->cap = params->max_particles;
+  b->esz = params->precision == MSM_FP32 ? 4 : 8;
+  try {
+    b->plans.reserve(batch);
+    for (int i = 0; i < batch; ++i) {
+      msm_plan_t* p = nullptr;
+      const msm_status_t s = msm_plan_create(params, &p);
+      if (s != MSM_OK) { msm_batch_destroy(b); return s; }
+      p->graph_enabled = false;                     // the batch owns the graph
+      b->plans.push_back(p);
+    }
+  } catch (...) { msm_batch_destroy(b); return MSM_ERR_NOMEM; }
+  DeviceGuard dg(b->device);
+  if (!dg.ok) { msm_batch_destroy(b); return MSM_ERR_CUDA; }
+  b->nstreams = std::min(batch, kBatchStreams);
+  bool ok = cudaStreamCreateWithFlags(&b->origin, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaEventCreateWithFlags(&b->fork_ev, cudaEventDisableTiming) == cudaSuccess &&
+            cudaEventCreateWithFlags(&b->in_ev, cudaEventDisableTiming) == cudaSuccess &&
+            cudaEventCreateWithFlags(&b->done_ev, cudaEventDisableTiming) == cudaSuccess;
+  for (int i = 0; ok && i < b->nstreams; ++i) {
+    cudaStream_t s = nullptr;
+    cudaEvent_t e = nullptr;
+    ok = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking) == cudaSuccess &&
+         cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
+    if (s) b->streams.push_back(s);
+    if (e) b->join_ev.push_back(e);
+  }
+  if (!ok) { cudaGetLastError(); msm_batch_destroy(b); return MSM_ERR_CUDA; }
+  *batch_out = b;
+  return MSM_OK;
+}
+
+msm_status_t msm_evaluate_batch(msm_batch_t* b, const int* h_n, const void* d_positions, const void* d_charges,
+                                void* d_forces, void* d_potentials, double* h_energy, double* h_virial,
+                                void* cuda_stream) {
+  if (!b || !h_n || !d_positions || !d_charges) return MSM_ERR_INVALID_ARG;
+  for (int i = 0; i < b->B; ++i) {
+    if (h_n[i] < 0) return MSM_ERR_INVALID_ARG;
+    if (h_n[i] > b->cap) return MSM_ERR_TOO_MANY_PARTICLES;
+  }
+  DeviceGuard dg(b->device);
+  if (!dg.ok) return MSM_ERR_CUDA;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const bool wv = h_virial != nullptr;
+  bool same = b->gexec && b->pos == d_positions && b->q == d_charges && b->F == d_forces && b->V == d_potentials &&
+              b->virial == wv && (int)b->n.size() == b->B;
+  for (int i = 0; same && i < b->B; ++i) same = b->n[i] == h_n[i];
+  if (!same) {
+    if (cudaStreamSynchronize(b->origin) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }
+    batch_drop_graph(b);
+    const size_t cap = (size_t)b->cap, e = b->esz;
+    cudaGraph_t g = nullptr;
+    msm_status_t es = MSM_OK;
+    if (cudaStreamBeginCapture(b->origin, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }
+    cudaEventRecord(b->fork_ev, b->origin);
+    for (int s = 0; s < b->nstreams; ++s) cudaStreamWaitEvent(b->streams[s], b->fork_ev, 0);
+    for (int i = 0; i < b->B && es == MSM_OK; ++i) {
+      const char* pp = (const char*)d_positions + (size_t)i * cap * 3 * e;
+      const char* qq = (const char*)d_charges + (size_t)i * cap * e;
+      char* ff = d_forces ? (char*)d_forces + (size_t)i * cap * 3 * e : nullptr;
+      char* vv = d_potentials ? (char*)d_potentials + (size_t)i * cap * e : nullptr;
+      es = enqueue(b->plans[i], h_n[i], pp, qq, ff, vv, wv, b->streams[i % b->nstreams], true);
+    }
+    for (int s = 0; s < b->nstreams; ++s) {
+      cudaEventRecord(b->join_ev[s], b->streams[s]);
+      cudaStreamWaitEvent(b->origin, b->join_ev[s], 0);
+    }
+    const cudaError_t ce = cudaStreamEndCapture(b->origin, &g);
+    if (es != MSM_OK || ce != cudaSuccess || !g || cudaGraphInstantiate(&b->gexec, g, 0) != cudaSuccess) {
+      if (g) cudaGraphDestroy(g);
+      b->gexec = nullptr;
+      cudaGetLastError();
+      return es != MSM_OK ? es : MSM_ERR_CUDA;
+    }
+    cudaGraphDestroy(g);
+    b->n.assign(h_n, h_n + b->B);
+    b->pos = d_positions; b->q = d_charges; b->F = d_forces; b->V = d_potentials; b->virial = wv;
+  }
+  // ordered after the caller's stream, joined back into it
+  if (cudaEventRecord(b->in_ev, st) != cudaSuccess || cudaStreamWaitEvent(b->origin, b->in_ev, 0) != cudaSuccess ||
+      cudaGraphLaunch(b->gexec, b->origin) != cudaSuccess || cudaEventRecord(b->done_ev, b->origin) != cudaSuccess ||
+      cudaStreamWaitEvent(st, b->done_ev, 0) != cudaSuccess) {
+    cudaGetLastError();
+    return MSM_ERR_CUDA;
+  }
+  if (!h_energy && !h_virial) return MSM_OK;        // stream-ordered, as msm_evaluate
+  if (cudaEventSynchronize(b->done_ev) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }
+  msm_status_t rs = MSM_OK;
+  for (int i = 0; i < b->B; ++i) {
+    const double* r = b->plans[i]->h_results;
+    if (h_energy) h_energy[i] = r[0];
+    if (h_virial) std::memcpy(h_virial + 6 * (size_t)i, r + 1, 6 * sizeof(double));
+    if (r[7] != 0.0) rs = MSM_ERR_OUT_OF_BOX;
+  }
+  return rs;
+}
+
+}  // extern "C"

@@ -24,7 +24,8 @@ STATUS = {0: "MSM_OK", 1: "MSM_ERR_INVALID_ARG", 2: "MSM_ERR_UNSUPPORTED", 3: "M
 EXPORTS = ["msm_plan_create", "msm_plan_info", "msm_evaluate", "msm_evaluate_async", "msm_get_results",
            "msm_evaluate_host", "msm_set_profiling",
            "msm_get_stage_times", "msm_get_launch_count", "msm_debug_copy_grid", "msm_plan_destroy",
-           "msm_status_string", "msm_measure_fma_peak"]
+           "msm_status_string", "msm_measure_fma_peak", "msm_batch_create", "msm_evaluate_batch",
+           "msm_batch_destroy"]
 
 
 class MsmError(RuntimeError):
@@ -67,6 +68,10 @@ def lib():
                                           C.POINTER(C.POINTER(C.c_float))]
         L.msm_get_launch_count.restype = i; L.msm_get_launch_count.argtypes = [vp, C.POINTER(i)]
         L.msm_debug_copy_grid.restype = i; L.msm_debug_copy_grid.argtypes = [vp, i, i, dp, C.c_size_t]
+        L.msm_batch_create.restype = i; L.msm_batch_create.argtypes = [C.POINTER(Params), i, C.POINTER(vp)]
+        L.msm_evaluate_batch.restype = i
+        L.msm_evaluate_batch.argtypes = [vp, C.POINTER(i), vp, vp, vp, vp, dp, dp, vp]
+        L.msm_batch_destroy.restype = None; L.msm_batch_destroy.argtypes = [vp]
         L.msm_plan_destroy.restype = None; L.msm_plan_destroy.argtypes = [vp]
         L.msm_status_string.restype = C.c_char_p; L.msm_status_string.argtypes = [i]
         L.msm_measure_fma_peak.restype = i; L.msm_measure_fma_peak.argtypes = [i, i, dp]
@@ -211,6 +216,49 @@ class Plan:
         if st:
             raise MsmError(st, "msm_debug_copy_grid")
         return out
+
+
+class Batch:
+    """msm_batch_create / msm_evaluate_batch: B systems of one geometry, tensors [B, max_particles, ...]."""
+
+    def __init__(self, batch, box, periodic, h, a, p, levels, precision="fp64", mu=-1, max_particles=1024, device=0):
+        prm = Params()
+        prm.box[:] = [float(b) for b in box]
+        prm.periodic[:] = [int(b) for b in periodic]
+        prm.h, prm.a, prm.p, prm.levels = float(h), float(a), int(p), int(levels)
+        prm.precision = MSM_FP32 if precision == "fp32" else MSM_FP64
+        prm.mu, prm.max_particles, prm.device = int(mu), int(max_particles), int(device)
+        self._h = C.c_void_p()
+        st = lib().msm_batch_create(C.byref(prm), int(batch), C.byref(self._h))
+        if st:
+            self._h = None
+            raise MsmError(st, "msm_batch_create")
+        self.batch, self.cap, self.precision, self.device = int(batch), int(max_particles), precision, int(device)
+
+    def close(self):
+        if getattr(self, "_h", None) and lib is not None:
+            lib().msm_batch_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def evaluate(self, n, positions, charges, forces=None, potentials=None, want_energy=True, want_virial=True,
+                 stream=None):
+        """n: B particle counts; positions [B, cap, 3], charges [B, cap] CUDA tensors of the batch's
+        dtype. Returns (energies ndarray(B) or None, virials ndarray(B, 6) or None)."""
+        import torch
+        nn = (C.c_int * self.batch)(*[int(v) for v in n])
+        e = (C.c_double * self.batch)()
+        w = (C.c_double * (6 * self.batch))()
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        st = lib().msm_evaluate_batch(self._h, nn, positions.data_ptr(), charges.data_ptr(),
+                                      forces.data_ptr() if forces is not None else None,
+                                      potentials.data_ptr() if potentials is not None else None,
+                                      e if want_energy else None, w if want_virial else None,
+                                      C.c_void_p(s.cuda_stream))
+        if st:
+            raise MsmError(st, "msm_evaluate_batch")
+        return (np.array(e[:]) if want_energy else None), (np.array(w[:]).reshape(self.batch, 6) if want_virial else None)
 
 
 def evaluate_workload(w, precision=None, mu=-1, want_virial=True, device=0):

@@ -523,3 +523,51 @@ def test_stream_ordered_evaluation_overlaps_caller_work():
     U, W = plan.results()
     torch.cuda.synchronize()
     assert U == U0 and np.array_equal(W, W0) and torch.equal(F, F0)
+
+
+def test_batched_small_systems_against_their_own_oracle_runs():
+    """msm_evaluate_batch (batching with fixed grid counts and padding): 64 systems of
+    config 1's shape (open 20 A cube, p = 4, h = 2, a = 6, 3 levels) with different particle counts
+    (zero-charge padding fills the slots), each compared with its own oracle run at 1e-10; graph
+    replay reproduces the first call bit for bit; one system of the batch equals a plain plan."""
+    import torch
+    from oracle import Oracle
+    from paper_2510_05961_b200 import msm
+    B, cap = 64, 512
+    dev = torch.device("cuda", 0)
+    rng = np.random.default_rng(2024)
+    n = [int(v) for v in rng.integers(300, cap + 1, B)]
+    n[0], n[1] = cap, 1
+    pos = np.zeros((B, cap, 3)); q = np.zeros((B, cap))
+    for b in range(B):
+        pos[b, :n[b]] = rng.random((n[b], 3)) * 20.0
+        pos[b, n[b]:] = 10.0                                   # padding: zero charges somewhere in the box
+        q[b, :n[b]] = np.where(np.arange(n[b]) % 2 == 0, 1.0, -1.0) * rng.uniform(0.5, 1.0, n[b])
+    batch = msm.Batch(B, (20.0,) * 3, (0, 0, 0), 2.0, 6.0, 4, 3, "fp64", max_particles=cap)
+    tp = torch.tensor(pos, device=dev); tq = torch.tensor(q, device=dev)
+    F = torch.zeros((B, cap, 3), dtype=torch.float64, device=dev); V = torch.zeros((B, cap), dtype=torch.float64, device=dev)
+    U, W = batch.evaluate(n, tp, tq, F, V)
+    F0, V0 = F.clone(), V.clone()
+    for _ in range(2):                                         # replays of the captured graph
+        F.zero_(); V.zero_()
+        U2, W2 = batch.evaluate(n, tp, tq, F, V)
+        assert np.array_equal(U2, U) and np.array_equal(W2, W) and torch.equal(F, F0) and torch.equal(V, V0)
+    Fh, Vh = F.cpu().numpy(), V.cpu().numpy()
+    orc = Oracle((20.0,) * 3, (0, 0, 0), 2.0, 6.0, 4, 3)
+    for b in range(B):
+        ref = orc.evaluate(pos[b, :n[b]], q[b, :n[b]])
+        es = max(abs(ref["energy"]), 1e-3)
+        assert abs(U[b] - ref["energy"]) <= 1e-10 * es, (b, n[b], U[b], ref["energy"])
+        fs = max(np.abs(ref["forces"]).max(), 1e-3)
+        assert np.abs(Fh[b, :n[b]] - ref["forces"]).max() <= 1e-10 * fs
+        assert np.abs(Vh[b, :n[b]] - ref["potentials"]).max() <= 1e-10 * max(np.abs(ref["potentials"]).max(), 1e-3)
+        assert np.abs(W[b] - ref["virial"]).max() <= 1e-10 * max(np.abs(ref["virial"]).max(), es)
+    # padding with zero charges changes nothing (P:326): the full slot gives the same energy
+    nfull = [cap] * B
+    U3, _ = batch.evaluate(nfull, tp, tq, F, V)
+    assert np.abs(U3 - U).max() <= 1e-11 * np.abs(U).max()
+    # one system through a plain plan: identical bits
+    plan = msm.Plan((20.0,) * 3, (0, 0, 0), 2.0, 6.0, 4, 3, "fp64", max_particles=cap)
+    F1 = torch.zeros((n[5], 3), dtype=torch.float64, device=dev)
+    U1, W1 = plan.evaluate(tp[5, :n[5]].contiguous(), tq[5, :n[5]].contiguous(), F1)
+    assert U1 == U[5] and np.array_equal(W1, W[5]) and torch.equal(F1, F0[5, :n[5]])
