@@ -117,7 +117,10 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   cudaMemsetAsync(p->ibuf, 0, p->ibuf_count * sizeof(int), st);
   MSM_LAUNCH(p, (k_bin<T><<<blocks_for(n, 256), 256, 0, st>>>(n, pos, p->bg, p->pcell, p->gcell, p->phist,
                                                                p->ghist, p->pslot, p->gslot, p->flag)));
-  {
+  if (p->n_pcells <= kScanSerialMax && p->n_gcells <= kScanSerialMax) {
+    MSM_LAUNCH(p, (k_scan_serial2<<<2, kScanThreads, 0, st>>>(p->n_pcells, p->phist, p->pstart, p->n_gcells, p->ghist,
+                                                                p->gstart, n)));
+  } else {
     const int tp = (p->n_pcells + kScanTile - 1) / kScanTile, tg = (p->n_gcells + kScanTile - 1) / kScanTile;
     MSM_LAUNCH(p, (k_scan_tiles<<<tp, kScanThreads, 0, st>>>(p->n_pcells, p->phist, p->pstart, p->ptotals)));
     MSM_LAUNCH(p, (k_scan_tiles<<<tg, kScanThreads, 0, st>>>(p->n_gcells, p->ghist, p->gstart, p->gtotals)));
@@ -128,8 +131,8 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   }
   MSM_LAUNCH(p, (k_scatter<<<blocks_for(n, 256), 256, 0, st>>>(n, p->pcell, p->gcell, p->pstart, p->gstart,
                                                                  p->pslot, p->gslot, p->porder, p->gorder)));
-  MSM_LAUNCH(p, (k_sort_cells<<<blocks_for(p->n_pcells, 128), 128, 0, st>>>(p->n_pcells, p->pstart, p->porder)));
-  MSM_LAUNCH(p, (k_sort_cells<<<blocks_for(p->n_gcells, 128), 128, 0, st>>>(p->n_gcells, p->gstart, p->gorder)));
+  MSM_LAUNCH(p, (k_sort_cells<<<dim3(blocks_for(std::max(p->n_pcells, p->n_gcells), 128), 2), 128, 0, st>>>(
+                    p->n_pcells, p->pstart, p->porder, p->n_gcells, p->gstart, p->gorder)));
   MSM_LAUNCH(p, (k_build_records<T><<<blocks_for(n, 256), 256, 0, st>>>(
                     n, pos, q, p->bg, p->porder, p->pcell, p->gorder, p->gcell, (V4*)p->prec, (V4*)p->grec,
                     p->gcell_sorted, p->pcellx)));

@@ -130,6 +130,60 @@ __global__ void k_scan_totals(int nt, int* __restrict__ totals) {  // one block,
   }
 }
 
+// Both exclusive scans of a small system in ONE launch: block 0 scans the pair bins, block 1 the
+// grid cells, tile after tile with a running carry (used while each array has at most
+// kScanSerialMax elements; a small system is bound by its launch count, not by this loop).
+constexpr int kScanSerialMax = 16 * kScanTile;
+__global__ void __launch_bounds__(kScanThreads)
+k_scan_serial2(int m0, const int* __restrict__ in0, int* __restrict__ out0, int m1, const int* __restrict__ in1,
+               int* __restrict__ out1, int n_total) {
+  __shared__ int wsum[32];
+  __shared__ int carry_s;
+  const int m = blockIdx.x == 0 ? m0 : m1;
+  const int* __restrict__ in = blockIdx.x == 0 ? in0 : in1;
+  int* __restrict__ out = blockIdx.x == 0 ? out0 : out1;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  for (int t0 = 0; t0 < m; t0 += kScanTile) {
+    const int base = t0 + threadIdx.x * kScanPerThread;
+    int v[kScanPerThread], s = 0;
+#pragma unroll
+    for (int k = 0; k < kScanPerThread; ++k) {
+      v[k] = (base + k < m) ? in[base + k] : 0;
+      s += v[k];
+    }
+    int inc = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += t;
+    }
+    if (lane == 31) wsum[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+      int t = wsum[lane];
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int u = __shfl_up_sync(0xffffffffu, t, o);
+        if (lane >= o) t += u;
+      }
+      wsum[lane] = t;
+    }
+    __syncthreads();
+    int excl = carry_s + inc - s + (wid > 0 ? wsum[wid - 1] : 0);
+#pragma unroll
+    for (int k = 0; k < kScanPerThread; ++k) {
+      if (base + k < m) out[base + k] = excl;
+      excl += v[k];
+    }
+    __syncthreads();
+    if (threadIdx.x == kScanThreads - 1) carry_s = excl;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[m] = n_total;
+}
+
 __global__ void k_scan_add(int m, int* __restrict__ out, const int* __restrict__ totals, int n_total) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < m) out[i] += totals[i / kScanTile];
@@ -148,7 +202,12 @@ __global__ void k_scatter(int n, const int* __restrict__ pcell, const int* __res
 }
 
 // pass 3: canonical order inside each cell (ascending original index): insertion sort per cell
-__global__ void k_sort_cells(int ncell, const int* __restrict__ start, int* __restrict__ order) {
+// (blockIdx.y = 0: the pair bins, 1: the grid cells)
+__global__ void k_sort_cells(int ncell0, const int* __restrict__ start0, int* __restrict__ order0, int ncell1,
+                             const int* __restrict__ start1, int* __restrict__ order1) {
+  const int ncell = blockIdx.y == 0 ? ncell0 : ncell1;
+  const int* __restrict__ start = blockIdx.y == 0 ? start0 : start1;
+  int* __restrict__ order = blockIdx.y == 0 ? order0 : order1;
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= ncell) return;
   const int s = start[c], e = start[c + 1];
