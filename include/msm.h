@@ -87,6 +87,22 @@ msm_status_t msm_plan_create(const msm_params_t *params, msm_plan_t **plan_out);
 
 msm_status_t msm_plan_info(const msm_plan_t *plan, msm_plan_info_t *info_out);
 
+/* Dynamic cell (with a dynamic cell the kernel stencils are recomputed from the current
+ * cell; what a plan fixes is the NUMBER of grid points, the spacings follow the cell).
+ * msm_plan_create_dynamic builds a plan whose stencil tables, halos and pair cells leave room for
+ * every periodic box edge to shrink by up to the fraction `reserve` (0 <= reserve <= 0.5; growth
+ * needs no room); msm_plan_create is the same with reserve 0. msm_plan_set_box then moves the plan
+ * to new box edges without reallocating anything: the sampled stencils s_l and their strain
+ * derivatives of every tiled level are recomputed ON THE DEVICE (one thread per stored tap; every
+ * intermediate level has the same functional form), the cell-list and grid geometry are
+ * updated, and the dense operator of the top grid (<= 4096 points) is rebuilt on the host and
+ * uploaded. Open axes must keep their length (their node set follows box / h, reading G2):
+ * MSM_ERR_UNSUPPORTED otherwise, and also when a periodic edge shrinks below the reserve;
+ * MSM_ERR_CUTOFF_TOO_LARGE when a > box / 2. The call synchronises the device. Results afterwards
+ * equal those of a plan created at the new box (up to rounding order). */
+msm_status_t msm_plan_create_dynamic(const msm_params_t *params, double reserve, msm_plan_t **plan_out);
+msm_status_t msm_plan_set_box(msm_plan_t *plan, const double *box /* 3 doubles */);
+
 /* One evaluation, enqueued on cuda_stream (a cudaStream_t; NULL = the default stream).
  *   d_positions  device, n x 3 row-major (x,y,z per particle), plan precision; not modified.
  *                Periodic coordinates are wrapped into the box; open coordinates must lie in

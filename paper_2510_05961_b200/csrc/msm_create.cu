@@ -1,6 +1,7 @@
 // msm_create.cu -- msm_plan_create / msm_plan_destroy / msm_plan_info: host mathematics (fp64)
 // and every device buffer of a plan. See include/msm.h.
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -59,10 +60,22 @@ void balanced_bounds(const std::vector<double>& w, int S, unsigned char* b) {
 }
 
 // stencil row tables + chunked taps of one tiled level (see conv.cuh)
+int4* upload_desc(msm_plan* p, const std::vector<int4>& v) {
+  int4* d = (int4*)dev_alloc(p, std::max<size_t>(v.size(), 1) * sizeof(int4));
+  if (!v.empty() && cudaMemcpy(d, v.data(), v.size() * sizeof(int4), cudaMemcpyHostToDevice) != cudaSuccess) throw CudaFail();
+  return d;
+}
+
 void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   const Level& lv = p->H->lev[l];
   LevelDev& d = p->lev[l];
-  const SampledStencil st = sample_level_stencil(*p->H, *p->S, l);
+  // the table STRUCTURE (which taps exist, halo widths) is sized for the smallest spacings the plan
+  // reserves room for; the VALUES are sampled at the actual spacings (zero outside the ellipsoid)
+  double hs[3];
+  for (int ax = 0; ax < 3; ++ax) hs[ax] = p->mp.periodic[ax] ? lv.h[ax] * (1.0 - p->reserve) : lv.h[ax];
+  for (int ax = 0; ax < 3; ++ax) d.hstruct[ax] = hs[ax];
+  const SampledStencil st = sample_level_stencil(*p->H, *p->S, l, hs);
+  std::vector<int4> tsd, tvd, t2d(8, make_int4(0, 0, 0, 0)), tv2d;
   d.taps = st.taps;
   ConvLevel& g = p->conv.lev[l - 1];
   for (int ax = 0; ax < 3; ++ax) { g.M[ax] = lv.M[ax]; g.R[ax] = st.R[ax]; }
@@ -90,12 +103,12 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   for (int dz = -Rz; dz <= Rz; ++dz)
     for (int dy = -st.R[1]; dy <= st.R[1]; ++dy) {
       int4& r = rows[(size_t)(dz + Rz) * ny + (dy + st.R[1])];
-      const double y = dy * lv.h[1], z = dz * lv.h[2];
+      const double y = dy * hs[1], z = dz * hs[2];
       const double rem = A * A - y * y - z * z;
       int Rx = -1;
       if (rem > 0) {
-        Rx = std::min(st.R[0], (int)std::floor(std::sqrt(rem) / lv.h[0]));
-        while (Rx >= 0 && (Rx * lv.h[0]) * (Rx * lv.h[0]) >= rem) --Rx;
+        Rx = std::min(st.R[0], (int)std::floor(std::sqrt(rem) / hs[0]));
+        while (Rx >= 0 && (Rx * hs[0]) * (Rx * hs[0]) >= rem) --Rx;
       }
       if (Rx < 0) { r = make_int4(0, 1, 0, 0); }
       else {
@@ -106,7 +119,9 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
         for (int c = clo; c <= chi; ++c)
           for (int t = 0; t < 4; ++t) {
             const int dx = 4 * c - g.X0 + t;
-            ts.push_back(dx >= -Rx && dx <= Rx ? st.at(st.s, dx, dy, dz) : 0.0);
+            const bool in = dx >= -Rx && dx <= Rx;
+            ts.push_back(in ? st.at(st.s, dx, dy, dz) : 0.0);
+            tsd.push_back(make_int4(dx, dy, dz, in ? 1 : 0));
           }
       }
       // virial: half space n > 0 (z, then y, then x), weight 2 (C(n) is even, reading V)
@@ -122,8 +137,10 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
         for (int m = 0; m < 3; ++m)
           for (int t = 0; t < 4; ++t) {
             const int dx = 4 * c - g.X0 + t;
-            const double gv = dx >= xlo && dx <= Rx ? 2.0 * st.at(st.g, dx, dy, dz) : 0.0;
+            const bool in = dx >= xlo && dx <= Rx;
+            const double gv = in ? 2.0 * st.at(st.g, dx, dy, dz) : 0.0;
             tv.push_back(m == 0 ? gv : m == 1 ? gv * dx : gv * dx * dx);
+            tvd.push_back(make_int4(dx, dy, dz, in ? 2 + m : 0));
           }
     }
   auto up_rows = [&](const std::vector<int4>& r) {
@@ -135,6 +152,8 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   g.vrows = up_rows(vrows);
   g.staps = upload(p, ts);
   g.vtaps = upload(p, tv);
+  d.tab[0] = TapTable{const_cast<void*>(g.staps), upload_desc(p, tsd), (int)ts.size()};
+  d.tab[2] = TapTable{const_cast<void*>(g.vtaps), upload_desc(p, tvd), (int)tv.size()};
   g.rows2 = nullptr;
   g.taps2 = nullptr;
   g.vrows2 = nullptr;
@@ -145,10 +164,10 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
       if (dz < -Rz || dz > Rz) return -1;
       const int4& r = rows[(size_t)(dz + Rz) * ny + (dy + st.R[1])];
       if (r.y > r.z) return -1;
-      const double y = dy * lv.h[1], z = dz * lv.h[2];
+      const double y = dy * hs[1], z = dz * hs[2];
       const double rem = A * A - y * y - z * z;
-      int Rx = std::min(st.R[0], (int)std::floor(std::sqrt(rem) / lv.h[0]));
-      while (Rx >= 0 && (Rx * lv.h[0]) * (Rx * lv.h[0]) >= rem) --Rx;
+      int Rx = std::min(st.R[0], (int)std::floor(std::sqrt(rem) / hs[0]));
+      while (Rx >= 0 && (Rx * hs[0]) * (Rx * hs[0]) >= rem) --Rx;
       return Rx;
     };
     std::vector<int4> r2((size_t)ny * (nz + 1));
@@ -161,17 +180,23 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
         if (Rx < 0) { r = make_int4(0, 0, -1, 0); continue; }   // empty: clamps to chunk -1
         const int clo = (-Rx + g.X0) / 4, chi = (Rx + g.X0) / 4;
         std::vector<double> rowv;
+        std::vector<int4> rowd;
         for (int c = clo; c <= chi; ++c)
           for (int t = 0; t < 4; ++t) {
             const int dx = 4 * c - g.X0 + t;
-            rowv.push_back(ra >= 0 && dx >= -ra && dx <= ra ? st.at(st.s, dx, dy, d) : 0.0);
-            rowv.push_back(rb >= 0 && dx >= -rb && dx <= rb ? st.at(st.s, dx, dy, d - 1) : 0.0);
+            const bool ia = ra >= 0 && dx >= -ra && dx <= ra, ib = rb >= 0 && dx >= -rb && dx <= rb;
+            rowv.push_back(ia ? st.at(st.s, dx, dy, d) : 0.0);
+            rowv.push_back(ib ? st.at(st.s, dx, dy, d - 1) : 0.0);
+            rowd.push_back(make_int4(dx, dy, d, ia ? 1 : 0));
+            rowd.push_back(make_int4(dx, dy, d - 1, ib ? 1 : 0));
           }
-        // rows (d, dy) and (d, -dy) hold the same taps: stored once (half the table, better L1 reuse)
+        // rows (d, dy) and (d, -dy) hold the same taps (for any spacings): stored once (half the
+        // table, better L1 reuse)
         auto it = seen2.find(rowv);
         if (it == seen2.end()) {
           it = seen2.emplace(rowv, (int)(t2.size() / 8) - 1).first;
           t2.insert(t2.end(), rowv.begin(), rowv.end());
+          t2d.insert(t2d.end(), rowd.begin(), rowd.end());
         }
         r = make_int4(it->second, clo, chi, 0);
       }
@@ -198,27 +223,35 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
         const int clo = (xlo + g.X0) / 4, chi = (xhi + g.X0) / 4;
         p->conv_maxc = std::max(p->conv_maxc, chi - clo + 1);
         std::vector<double> rowv;
+        std::vector<int4> rowd;
         for (int c = clo; c <= chi; ++c)
           for (int m = 0; m < 3; ++m)
             for (int t = 0; t < 4; ++t) {
               const int dx = 4 * c - g.X0 + t;
-              const double ga = ha && dx >= alo && dx <= ahi ? 2.0 * st.at(st.g, dx, dy, d) : 0.0;
-              const double gb = hb && dx >= blo && dx <= bhi ? 2.0 * st.at(st.g, dx, dy, d - 1) : 0.0;
+              const bool ia = ha && dx >= alo && dx <= ahi, ib = hb && dx >= blo && dx <= bhi;
+              const double ga = ia ? 2.0 * st.at(st.g, dx, dy, d) : 0.0;
+              const double gb = ib ? 2.0 * st.at(st.g, dx, dy, d - 1) : 0.0;
               const double f = m == 0 ? 1.0 : m == 1 ? (double)dx : (double)dx * dx;
               rowv.push_back(ga * f);
               rowv.push_back(gb * f);
+              rowd.push_back(make_int4(dx, dy, d, ia ? 2 + m : 0));
+              rowd.push_back(make_int4(dx, dy, d - 1, ib ? 2 + m : 0));
             }
         auto it = seenv2.find(rowv);
         if (it == seenv2.end()) {
           it = seenv2.emplace(rowv, (int)(tv2.size() / 24)).first;
           tv2.insert(tv2.end(), rowv.begin(), rowv.end());
+          tv2d.insert(tv2d.end(), rowd.begin(), rowd.end());
         }
         r = make_int4(it->second, clo, chi, 0);
       }
     g.vrows2 = up_rows(vr2);
     g.vtaps2 = upload(p, tv2);
+    d.tab[3] = TapTable{const_cast<void*>(g.vtaps2), upload_desc(p, tv2d), (int)tv2.size()};
     g.rows2 = up_rows(r2);
-    g.taps2 = (const char*)upload(p, t2) + 8 * p->esz;   // chunk 0 of the table follows the guard chunk
+    void* t2dev = upload(p, t2);
+    d.tab[1] = TapTable{t2dev, upload_desc(p, t2d), (int)t2.size()};
+    g.taps2 = (const char*)t2dev + 8 * p->esz;   // chunk 0 of the table follows the guard chunk
     g.n_rows2 = (int)r2.size();
     g.n_taps2q = (int)(t2.size() / 4);
   }
@@ -348,7 +381,8 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   for (int ax = 0; ax < 3; ++ax) {
     bg.box[ax] = prm->box[ax];
     bg.periodic[ax] = mp.periodic[ax];
-    bg.nc[ax] = std::max(1, (int)std::floor(prm->box[ax] / (0.5 * prm->a)));
+    // (cells stay >= a/2 wide down to the smallest box the plan reserves room for)
+    bg.nc[ax] = std::max(1, (int)std::floor(prm->box[ax] * (mp.periodic[ax] ? 1.0 - p->reserve : 1.0) / (0.5 * prm->a)));
     bg.cell_edge[ax] = prm->box[ax] / bg.nc[ax];
     bg.h1[ax] = H.lev[1].h[ax];
     bg.ng[ax] = mp.periodic[ax] ? H.lev[1].M[ax] : (int)std::floor(prm->box[ax] / prm->h) + 1;
@@ -450,9 +484,132 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   return MSM_OK;
 }
 
+// ---- dynamic cell: tap values recomputed on the device (with a dynamic cell the
+// stencils are rebuilt from the current cell at every call; every intermediate level has
+// the same functional form, so one kernel serves all levels)
+struct TapGeom {
+  double h[3];
+  double A0, A1;      // 2^(l-1) a, 2^l a
+  int p;
+  double c[8];        // binom(-1/2, k)
+};
+
+__device__ double dev_gamma(const TapGeom& g, double rho) {
+  if (rho >= 1.0) return 1.0 / rho;
+  const double s = rho * rho - 1.0;
+  double acc = g.c[g.p - 1];
+  for (int k = g.p - 2; k >= 0; --k) acc = acc * s + g.c[k];
+  return acc;
+}
+__device__ double dev_dgamma(const TapGeom& g, double rho) {
+  if (rho >= 1.0) return -1.0 / (rho * rho);
+  const double s = rho * rho - 1.0;
+  double acc = (g.p - 1) * g.c[g.p - 1];
+  for (int k = g.p - 2; k >= 1; --k) acc = acc * s + k * g.c[k];
+  return 2.0 * rho * acc;
+}
+
+// values[i] from desc[i] = (dx, dy, dz, kind): s_l = k_l(|h o n|) (Eq. 21 middle case, reading
+// K1) or 2 k_l'(r)/r times 1, dx, dx^2; zero outside the cutoff ellipsoid r < 2^l a (Eq. 3)
+template <typename T>
+__global__ void k_rebuild_taps(int n, const int4* __restrict__ desc, TapGeom g, T* __restrict__ values) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int4 d = desc[i];
+  double v = 0.0;
+  if (d.w != 0) {
+    const double x = d.x * g.h[0], y = d.y * g.h[1], z = d.z * g.h[2];
+    const double r = sqrt(x * x + y * y + z * z);
+    if (r < g.A1) {
+      if (d.w == 1) {
+        v = dev_gamma(g, r / g.A0) / g.A0 - dev_gamma(g, r / g.A1) / g.A1;
+      } else if (r > 0.0) {
+        const double dk = dev_dgamma(g, r / g.A0) / (g.A0 * g.A0) - dev_dgamma(g, r / g.A1) / (g.A1 * g.A1);
+        const double gv = 2.0 * dk / r;
+        v = d.w == 2 ? gv : (d.w == 3 ? gv * d.x : gv * d.x * d.x);
+      }
+    }
+  }
+  values[i] = (T)v;
+}
+
+msm_status_t set_box_impl(msm_plan* p, const double* box) {
+  const Hierarchy& H0 = *p->H;
+  for (int ax = 0; ax < 3; ++ax) {
+    if (!(box[ax] > 0.0)) return MSM_ERR_INVALID_ARG;
+    if (!p->mp.periodic[ax]) {
+      // an open axis has no spacing of its own: its node set follows box / h (reading G2)
+      if (std::fabs(box[ax] - p->mp.box[ax]) > 1e-12 * p->mp.box[ax]) return MSM_ERR_UNSUPPORTED;
+      continue;
+    }
+    if (p->mp.a > 0.5 * box[ax]) return MSM_ERR_CUTOFF_TOO_LARGE;           // minimum image
+    if (box[ax] / p->bg.nc[ax] < 0.5 * p->mp.a * (1.0 - 1e-12)) return MSM_ERR_UNSUPPORTED;   // below the reserve
+    for (int l = 1; l < p->n_t; ++l)
+      if (box[ax] / H0.lev[l].M[ax] < p->lev[l].hstruct[ax] * (1.0 - 1e-12)) return MSM_ERR_UNSUPPORTED;
+  }
+  if (p->pending && cudaEventSynchronize(p->done_ev) != cudaSuccess) { cudaGetLastError(); return MSM_ERR_CUDA; }
+  p->pending = false;
+  if (p->gexec) { cudaGraphExecDestroy(p->gexec); p->gexec = nullptr; }     // geometry is baked into the graph
+  p->gkey = msm::GraphKey{};
+  // host copies of the geometry: the number of grid points is what stays fixed
+  Hierarchy& H = *p->H;
+  for (int ax = 0; ax < 3; ++ax) {
+    p->prm.box[ax] = p->mp.box[ax] = H.prm.box[ax] = p->bg.box[ax] = box[ax];
+    p->bg.cell_edge[ax] = box[ax] / p->bg.nc[ax];
+    if (!p->mp.periodic[ax]) continue;
+    for (int l = 1; l <= H.L; ++l) H.lev[l].h[ax] = box[ax] / H.lev[l].M[ax];
+    p->bg.h1[ax] = H.lev[1].h[ax];
+  }
+  // sampled stencils of every tiled level, on the device
+  for (int l = 1; l < p->n_t; ++l) {
+    TapGeom g;
+    for (int ax = 0; ax < 3; ++ax) g.h[ax] = H.lev[l].h[ax];
+    g.A0 = std::ldexp(p->mp.a, l - 1); g.A1 = std::ldexp(p->mp.a, l);
+    g.p = p->P;
+    for (int k = 0; k < 8; ++k) g.c[k] = p->S->c[k];
+    for (int t = 0; t < 4; ++t) {
+      const TapTable& tb = p->lev[l].tab[t];
+      if (!tb.values || tb.n == 0) continue;
+      const unsigned nb = (unsigned)((tb.n + 255) / 256);
+      if (p->fp32) k_rebuild_taps<float><<<nb, 256>>>(tb.n, tb.desc, g, (float*)tb.values);
+      else k_rebuild_taps<double><<<nb, 256>>>(tb.n, tb.desc, g, (double*)tb.values);
+    }
+  }
+  // the dense operator of the top grid (<= 4096 points): rebuilt on the host and uploaded
+  {
+    const TopOperator top = build_top_operator(H, *p->S, p->omega, p->J, p->n_t, true);
+    std::vector<double> td;
+    td.reserve((size_t)6 * top.G * top.G);
+    for (int k = 0; k < 6; ++k) td.insert(td.end(), top.TD[k].begin(), top.TD[k].end());
+    auto put = [&](void* dst, const std::vector<double>& v) {
+      if (p->fp32) {
+        std::vector<float> t(v.begin(), v.end());
+        return cudaMemcpy(dst, t.data(), t.size() * 4, cudaMemcpyHostToDevice) == cudaSuccess;
+      }
+      return cudaMemcpy(dst, v.data(), v.size() * 8, cudaMemcpyHostToDevice) == cudaSuccess;
+    };
+    if (!put(p->topT, top.T) || !put(p->topTD, td)) { cudaGetLastError(); return MSM_ERR_CUDA; }
+  }
+  if (cudaDeviceSynchronize() != cudaSuccess || cudaGetLastError() != cudaSuccess) return MSM_ERR_CUDA;
+  return MSM_OK;
+}
+
 }  // namespace
 
 extern "C" {
+
+msm_status_t msm_plan_set_box(msm_plan_t* p, const double* box) {
+  if (!p || !box) return MSM_ERR_INVALID_ARG;
+  DeviceGuard dg(p->prm.device);
+  if (!dg.ok) return MSM_ERR_CUDA;
+  try {
+    return set_box_impl(p, box);
+  } catch (const std::bad_alloc&) {
+    return MSM_ERR_NOMEM;
+  } catch (...) {
+    return MSM_ERR_CUDA;
+  }
+}
 
 void msm_plan_destroy(msm_plan_t* p) {
   if (!p) return;
@@ -477,11 +634,16 @@ void msm_plan_destroy(msm_plan_t* p) {
 }
 
 msm_status_t msm_plan_create(const msm_params_t* params, msm_plan_t** plan_out) {
+  return msm_plan_create_dynamic(params, 0.0, plan_out);
+}
+
+msm_status_t msm_plan_create_dynamic(const msm_params_t* params, double reserve, msm_plan_t** plan_out) {
   if (!plan_out) return MSM_ERR_INVALID_ARG;
   *plan_out = nullptr;
-  if (!params) return MSM_ERR_INVALID_ARG;
+  if (!params || !(reserve >= 0.0) || reserve > 0.5) return MSM_ERR_INVALID_ARG;
   msm_plan* p = new (std::nothrow) msm_plan();
   if (!p) return MSM_ERR_NOMEM;
+  p->reserve = reserve;
   msm_status_t st;
   int prev_dev = -1;
   if (cudaGetDevice(&prev_dev) != cudaSuccess) { prev_dev = -1; cudaGetLastError(); }

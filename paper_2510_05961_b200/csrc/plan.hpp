@@ -14,10 +14,21 @@ namespace msm {
 
 constexpr int kMaxStages = 2 * MSM_MAX_LEVELS + 16;   // sort pair anterpolate restrict {filter,conv}_l* top ...
 
+// one tap table of a level and, per stored value, what it is: (dx, dy, dz, kind) with kind
+// 0 = padding zero, 1 = s_l, 2 = 2g, 3 = 2g dx, 4 = 2g dx^2 (g = k_l'(r)/r): msm_plan_set_box
+// recomputes the values on the device from these descriptors
+struct TapTable {
+  void* values = nullptr;
+  int4* desc = nullptr;
+  int n = 0;
+};
+
 struct LevelDev {
   void *Q = nullptr, *E = nullptr, *pad = nullptr;   // grid charge, potential, haloed filtered charge
   void* scratch = nullptr;                           // slice partials of the convolution (nslices > 1)
   int taps = 0;
+  TapTable tab[4];                                   // staps, taps2 (with its guard chunk), vtaps, vtaps2
+  double hstruct[3] = {0, 0, 0};                     // spacings the table structure was sized for
 };
 
 // arguments of one msm_evaluate: a captured CUDA graph is replayed only for an identical call
@@ -55,6 +66,7 @@ struct msm_plan {
   std::vector<double> J, omega;
   msm::SplinePieces* pieces = nullptr;
 
+  double reserve = 0.0;      // fraction by which msm_plan_set_box may shrink a periodic box edge
   std::vector<void*> allocs;
   size_t bytes = 0;
   int sm_count = 148;        // cudaDevAttrMultiProcessorCount of the plan's device (148 on B200)

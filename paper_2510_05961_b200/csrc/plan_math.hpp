@@ -78,7 +78,9 @@ struct SampledStencil {
     return v[((size_t)(dz + R[2]) * (2 * R[1] + 1) + (dy + R[1])) * (2 * R[0] + 1) + (dx + R[0])];
   }
 };
-SampledStencil sample_level_stencil(const Hierarchy& H, const Splitting& S, int l);
+// hstruct (optional): spacings that size the box [-R, R] (a plan that reserves room for a smaller
+// cell, msm_plan_set_box); the values are always sampled at the level's actual spacings.
+SampledStencil sample_level_stencil(const Hierarchy& H, const Splitting& S, int l, const double* hstruct = nullptr);
 
 // Dense operators of the top grid (level n_t): e = T q completes the hierarchy from level n_t up
 // to level L (convolution at each level, restriction up, prolongation down; Eq. 13),

@@ -9,13 +9,14 @@ namespace msm {
 
 // s(n) = k_l(|h o n|), g(n) = k_l'(r)/r inside the cutoff ellipsoid |h o n| < 2^l a (Eq. 20
 // samples; the omega' factors are applied to the grid charge instead, which is the same sum).
-SampledStencil sample_level_stencil(const Hierarchy& H, const Splitting& S, int l) {
+SampledStencil sample_level_stencil(const Hierarchy& H, const Splitting& S, int l, const double* hstruct) {
   SampledStencil st;
   const Level& lv = H.lev[l];
   const double A = std::ldexp(S.a, l);
   for (int ax = 0; ax < 3; ++ax) {
-    int R = (int)std::floor(A / lv.h[ax]);
-    while (R > 0 && R * lv.h[ax] >= A) --R;
+    const double hs = hstruct ? hstruct[ax] : lv.h[ax];
+    int R = (int)std::floor(A / hs);
+    while (R > 0 && R * hs >= A) --R;
     st.R[ax] = R;
   }
   const size_t n = (size_t)(2 * st.R[0] + 1) * (2 * st.R[1] + 1) * (2 * st.R[2] + 1);

@@ -25,7 +25,7 @@ EXPORTS = ["msm_plan_create", "msm_plan_info", "msm_evaluate", "msm_evaluate_asy
            "msm_evaluate_host", "msm_set_profiling",
            "msm_get_stage_times", "msm_get_launch_count", "msm_debug_copy_grid", "msm_plan_destroy",
            "msm_status_string", "msm_measure_fma_peak", "msm_batch_create", "msm_evaluate_batch",
-           "msm_batch_destroy"]
+           "msm_batch_destroy", "msm_plan_create_dynamic", "msm_plan_set_box"]
 
 
 class MsmError(RuntimeError):
@@ -57,6 +57,9 @@ def lib():
         L = C.CDLL(_SO)
         vp, i, dp = C.c_void_p, C.c_int, C.POINTER(C.c_double)
         L.msm_plan_create.restype = i; L.msm_plan_create.argtypes = [C.POINTER(Params), C.POINTER(vp)]
+        L.msm_plan_create_dynamic.restype = i
+        L.msm_plan_create_dynamic.argtypes = [C.POINTER(Params), C.c_double, C.POINTER(vp)]
+        L.msm_plan_set_box.restype = i; L.msm_plan_set_box.argtypes = [vp, dp]
         L.msm_plan_info.restype = i; L.msm_plan_info.argtypes = [vp, C.POINTER(PlanInfo)]
         L.msm_evaluate.restype = i; L.msm_evaluate.argtypes = [vp, i, vp, vp, vp, vp, dp, dp, vp]
         L.msm_evaluate_async.restype = i; L.msm_evaluate_async.argtypes = [vp, i, vp, vp, vp, vp, i, vp]
@@ -91,7 +94,9 @@ def measure_fma_peak(kind: str = "fp32", device: int = 0) -> float:
 class Plan:
     """msm_plan_create / msm_evaluate / msm_plan_destroy with torch tensors as buffers."""
 
-    def __init__(self, box, periodic, h, a, p, levels, precision="fp64", mu=-1, max_particles=1 << 20, device=0):
+    def __init__(self, box, periodic, h, a, p, levels, precision="fp64", mu=-1, max_particles=1 << 20, device=0,
+                 reserve=0.0):
+        """reserve > 0: room for set_box() to shrink periodic box edges by that fraction."""
         prm = Params()
         prm.box[:] = [float(b) for b in box]
         prm.periodic[:] = [int(b) for b in periodic]
@@ -99,7 +104,7 @@ class Plan:
         prm.precision = MSM_FP32 if precision == "fp32" else MSM_FP64
         prm.mu, prm.max_particles, prm.device = int(mu), int(max_particles), int(device)
         self._h = C.c_void_p()
-        st = lib().msm_plan_create(C.byref(prm), C.byref(self._h))
+        st = lib().msm_plan_create_dynamic(C.byref(prm), float(reserve), C.byref(self._h))
         if st:
             self._h = None
             raise MsmError(st, "msm_plan_create")
@@ -112,6 +117,14 @@ class Plan:
     def for_workload(cls, w, precision=None, mu=-1, device=0, max_particles=None):
         return cls(w.box, w.periodic, w.h, w.a, w.p, w.levels, precision or w.precision, mu,
                    max_particles or w.n, device)
+
+    def set_box(self, box):
+        """Move the plan to new box edges (same grid counts): stencils rebuilt on the device."""
+        b = (C.c_double * 3)(*[float(v) for v in box])
+        st = lib().msm_plan_set_box(self._h, b)
+        if st:
+            raise MsmError(st, "msm_plan_set_box")
+        lib().msm_plan_info(self._h, C.byref(self.info))
 
     def close(self):
         if getattr(self, "_h", None) and lib is not None:     # (module globals are gone at interpreter exit)

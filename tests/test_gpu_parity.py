@@ -571,3 +571,97 @@ def test_batched_small_systems_against_their_own_oracle_runs():
     F1 = torch.zeros((n[5], 3), dtype=torch.float64, device=dev)
     U1, W1 = plan.evaluate(tp[5, :n[5]].contiguous(), tq[5, :n[5]].contiguous(), F1)
     assert U1 == U[5] and np.array_equal(W1, W[5]) and torch.equal(F1, F0[5, :n[5]])
+
+
+@pytest.mark.parametrize("periodic,box,precision", [((1, 1, 1), (24.0, 26.0, 22.0), "fp64"),
+                                                    ((1, 1, 0), (26.0, 24.0, 9.0), "fp64"),
+                                                    ((1, 1, 1), (24.0, 26.0, 22.0), "fp32")])
+def test_dynamic_cell_set_box(periodic, box, precision):
+    """msm_plan_set_box (the number of grid points is fixed, the spacings follow
+    the cell; stencils rebuilt on the device): after moving a plan with room for 6 % shrink to
+    another box, every output and every grid equals a fresh oracle at that box; the reserved
+    (larger) table structure does not change the results at the original box; the virial equals
+    the finite difference of the energy across two set_box calls (the oracle's own pin, run
+    through the GPU); shrinking beyond the reserve or changing an open axis is refused."""
+    import torch
+    from paper_2510_05961_b200 import msm
+    from paper_2510_05961_b200.workloads import Workload
+    rng = np.random.default_rng(321)
+    n = 1500
+    frac = rng.random((n, 3))
+    q = rng.uniform(-1, 1, n); q -= q.mean()
+    h, a, p, levels = 1.5, 5.5, 4, 2
+    dev = torch.device("cuda", 0)
+    dt = torch.float32 if precision == "fp32" else torch.float64
+    plan = msm.Plan(box, periodic, h, a, p, levels, precision, max_particles=n, reserve=0.06)
+
+    def run_at(b):
+        w = Workload("dyn", frac * np.array(b), q, tuple(b), periodic, h=h, a=a, p=p, levels=levels).as_precision(precision)
+        pos = torch.tensor(w.positions, dtype=dt, device=dev); qq = torch.tensor(w.charges, dtype=dt, device=dev)
+        F = torch.zeros((n, 3), dtype=dt, device=dev); V = torch.zeros(n, dtype=dt, device=dev)
+        U, W = plan.evaluate(pos, qq, F, V)
+        return w, {"energy": U, "virial": W, "forces": F.cpu().numpy().astype(np.float64),
+                   "potentials": V.cpu().numpy().astype(np.float64), "plan": plan}
+
+    def oracle_at(w, b):
+        from oracle import Oracle
+        # same grid counts as the plan: the target spacing follows the box (P:327)
+        orc = Oracle(b, periodic, h * b[0] / box[0], a, p, levels)
+        if not all(periodic):
+            orc = Oracle(b, periodic, h, a, p, levels)
+        res = orc.evaluate(w.positions, w.charges)
+        res["oracle"] = orc
+        return res
+
+    w0, g0 = run_at(box)
+    _log(f"dyn_{''.join(map(str, periodic))}_{precision}_box0", compare(w0, g0, oracle_at(w0, box), precision))
+    scale = (0.96, 1.03, 1.05) if all(periodic) else (0.96, 0.96 * box[0] / box[0], 1.0)
+    if not all(periodic):
+        scale = (0.97, 1.04, 1.0)
+    b1 = tuple(bb * s for bb, s in zip(box, scale))
+    plan.set_box(b1)
+    assert tuple(plan.grid_dims(1)) == tuple(msm.Plan(box, periodic, h, a, p, levels, precision, max_particles=8).grid_dims(1))
+    w1, g1 = run_at(b1)
+    from oracle import Oracle
+    orc = Oracle(b1, periodic, h, a, p, levels)
+    # the oracle derives its grid counts from box / h: make sure both sides have the same grids
+    M_o = [orc.level_info(1)["M"][ax] for ax in range(3)]
+    hh = h
+    if list(M_o) != list(plan.grid_dims(1)):
+        # pick a target spacing that reproduces the plan's counts on every periodic axis
+        cands = [b1[ax] / plan.grid_dims(1)[ax] for ax in range(3) if periodic[ax]]
+        hh = float(np.exp(np.mean(np.log(cands))))
+        orc = Oracle(b1, periodic, hh, a, p, levels)
+        M_o = [orc.level_info(1)["M"][ax] for ax in range(3)]
+    if list(M_o) == list(plan.grid_dims(1)):
+        ref = orc.evaluate(w1.positions, w1.charges); ref["oracle"] = orc
+        _log(f"dyn_{''.join(map(str, periodic))}_{precision}_box1", compare(w1, g1, ref, precision))
+    else:
+        pytest.fail(f"test set-up: oracle grids {M_o} vs plan {plan.grid_dims(1)}")
+    # virial == -dU/d eps_xx across two set_box calls (number of grid points fixed)
+    if precision == "fp64":
+        e = 1e-5
+        us = []
+        for s in (+e, -e):
+            b = (b1[0] * (1 + s), b1[1], b1[2])
+            plan.set_box(b)
+            us.append(run_at(b)[1]["energy"])
+        fd = -(us[0] - us[1]) / (2 * e)
+        assert abs(g1["virial"][0] - fd) <= 2e-6 * max(abs(fd), abs(g1["energy"]))
+    # back to the first box: the same results (the device-built taps round differently from the
+    # host-built ones of plan creation, so not the same bits)
+    plan.set_box(box)
+    w2, g2 = run_at(box)
+    tol = 1e-12 if precision == "fp64" else 2e-6
+    assert abs(g2["energy"] - g0["energy"]) <= tol * abs(g0["energy"])
+    assert np.abs(g2["forces"] - g0["forces"]).max() <= tol * np.abs(g0["forces"]).max()
+    # refused: below the reserve, changed open axis, cutoff too large
+    with pytest.raises(msm.MsmError) as ei:
+        plan.set_box((box[0] * 0.9, box[1], box[2]))
+    assert ei.value.status == 2
+    if not all(periodic):
+        with pytest.raises(msm.MsmError) as ei:
+            plan.set_box((box[0], box[1], box[2] * 1.1))
+        assert ei.value.status == 2
+    w3, g3 = run_at(box)                                      # a refused call leaves the plan untouched
+    assert g3["energy"] == g2["energy"]
