@@ -381,14 +381,24 @@ __device__ __forceinline__ void conv_f2_unit(const ConvLevel& g, const ConvUnit&
 #pragma unroll
         for (int k = 0; k < ZP; ++k) {
           if (on[k]) {
-            const unsigned long long t0 = pack2(tq[k][0].x, tq[k][0].y), t1 = pack2(tq[k][0].z, tq[k][0].w);
-            const unsigned long long t2 = pack2(tq[k][1].x, tq[k][1].y), t3 = pack2(tq[k][1].z, tq[k][1].w);
+            // the row's taps start / end inside a chunk: its empty 2-tap half is skipped
+            // (re.w = first | last << 16 half-chunk that holds a tap; warp-uniform)
+            const bool lo = 2 * c >= (re[k].w & 0xffff), hi = 2 * c + 1 <= (re[k].w >> 16);
+            if (lo) {
+              const unsigned long long t0 = pack2(tq[k][0].x, tq[k][0].y), t1 = pack2(tq[k][0].z, tq[k][0].w);
 #pragma unroll
-            for (int i = 0; i < XT; ++i) {
-              ffma2_bcast(acc[k][i], win[i], t0);
-              ffma2_bcast(acc[k][i], win[i + 1], t1);
-              ffma2_bcast(acc[k][i], win[i + 2], t2);
-              ffma2_bcast(acc[k][i], win[i + 3], t3);
+              for (int i = 0; i < XT; ++i) {
+                ffma2_bcast(acc[k][i], win[i], t0);
+                ffma2_bcast(acc[k][i], win[i + 1], t1);
+              }
+            }
+            if (hi) {
+              const unsigned long long t2 = pack2(tq[k][1].x, tq[k][1].y), t3 = pack2(tq[k][1].z, tq[k][1].w);
+#pragma unroll
+              for (int i = 0; i < XT; ++i) {
+                ffma2_bcast(acc[k][i], win[i + 2], t2);
+                ffma2_bcast(acc[k][i], win[i + 3], t3);
+              }
             }
           }
         }
@@ -678,8 +688,10 @@ k_conv_virial_f2(const ConvTable* __restrict__ tabp, ConvSmemLayout sl) {
             float4 gq[6];
 #pragma unroll
             for (int m = 0; m < 6; ++m) gq[m] = tp[m];
+            const bool lo = 2 * c >= (re[k].w & 0xffff), hi = 2 * c + 1 <= (re[k].w >> 16);
 #pragma unroll
             for (int t = 0; t < 4; ++t) {
+              if (t < 2 ? !lo : !hi) continue;          // empty 2-tap half of the row's first / last chunk
               unsigned long long c0 = 0ull, c1 = 0ull;
 #pragma unroll
               for (int i = 0; i < XT; i += 2) {

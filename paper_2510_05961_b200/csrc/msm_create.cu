@@ -179,6 +179,9 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
         int4& r = r2[(size_t)(d + Rz) * ny + (dy + st.R[1])];
         if (Rx < 0) { r = make_int4(0, 0, -1, 0); continue; }   // empty: clamps to chunk -1
         const int clo = (-Rx + g.X0) / 4, chi = (Rx + g.X0) / 4;
+        // first and last 2-tap half-chunk that holds a tap: the kernel skips the empty half of the
+        // first and of the last chunk of a row
+        const int halves = ((-Rx + g.X0) / 2) | (((Rx + g.X0) / 2) << 16);
         std::vector<double> rowv;
         std::vector<int4> rowd;
         for (int c = clo; c <= chi; ++c)
@@ -198,7 +201,7 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
           t2.insert(t2.end(), rowv.begin(), rowv.end());
           t2d.insert(t2d.end(), rowd.begin(), rowd.end());
         }
-        r = make_int4(it->second, clo, chi, 0);
+        r = make_int4(it->second, clo, chi, halves);
       }
     // virial, packed: half-space rows d and d - 1 merged, per chunk 24 floats (2g, 2g dx, 2g dx^2)
     // x 4 taps x (row d, row d - 1)
@@ -221,6 +224,7 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
         const int xlo = ha && hb ? std::min(alo, blo) : (ha ? alo : blo);
         const int xhi = ha && hb ? std::max(ahi, bhi) : (ha ? ahi : bhi);
         const int clo = (xlo + g.X0) / 4, chi = (xhi + g.X0) / 4;
+        const int halves = ((xlo + g.X0) / 2) | (((xhi + g.X0) / 2) << 16);
         p->conv_maxc = std::max(p->conv_maxc, chi - clo + 1);
         std::vector<double> rowv;
         std::vector<int4> rowd;
@@ -243,7 +247,7 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
           tv2.insert(tv2.end(), rowv.begin(), rowv.end());
           tv2d.insert(tv2d.end(), rowd.begin(), rowd.end());
         }
-        r = make_int4(it->second, clo, chi, 0);
+        r = make_int4(it->second, clo, chi, halves);
       }
     g.vrows2 = up_rows(vr2);
     g.vtaps2 = upload(p, tv2);
