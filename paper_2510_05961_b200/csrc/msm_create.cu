@@ -464,15 +464,19 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   if (cudaMallocHost((void**)&p->h_results, 8 * sizeof(double)) != cudaSuccess) return MSM_ERR_NOMEM;
   for (int i = 0; i <= kMaxStages; ++i)
     if (cudaEventCreate(&p->ev[i]) != cudaSuccess) return MSM_ERR_CUDA;
-  if (cudaStreamCreateWithFlags(&p->gstream, cudaStreamNonBlocking) != cudaSuccess ||
+  // stream priorities: the grid pipeline first, the pair kernel last, so that the convolution blocks
+  // take the slots the pair kernel leaves free instead of queueing behind its whole grid
+  int prio_lo = 0, prio_hi = 0;
+  cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+  if (cudaStreamCreateWithPriority(&p->gstream, cudaStreamNonBlocking, prio_hi) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->gev, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->done_ev, cudaEventDisableTiming) != cudaSuccess)
     return MSM_ERR_CUDA;
   if (const char* e = std::getenv("MSM_NO_GRAPH")) p->graph_enabled = std::atoi(e) == 0;
-  if (cudaStreamCreateWithFlags(&p->pstream, cudaStreamNonBlocking) != cudaSuccess ||
+  if (cudaStreamCreateWithPriority(&p->pstream, cudaStreamNonBlocking, prio_lo) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->fork_ev, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->join_ev, cudaEventDisableTiming) != cudaSuccess ||
-      cudaStreamCreateWithFlags(&p->vstream, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaStreamCreateWithPriority(&p->vstream, cudaStreamNonBlocking, prio_hi) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->fork2_ev, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->join2_ev, cudaEventDisableTiming) != cudaSuccess)
     return MSM_ERR_CUDA;
