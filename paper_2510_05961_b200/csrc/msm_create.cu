@@ -357,7 +357,17 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
   }
   p->conv.nlev = p->n_t - 1;
   if (p->conv.nlev > 0) {
-    p->conv_wpart = (double*)dev_alloc(p, (size_t)p->conv.total_vunits * 6 * sizeof(double));
+    // the exact dynamic shared memory of the convolution launches (conv_layout in msm_evaluate.cu:
+    // plane | row entries | two row-tap buffers) has to fit an SM; refuse here, not at the launch
+    auto total = [&](int elems_per_chunk, int layers) {
+      const size_t rows_off = (p->conv_smem + 15) / 16 * 16;
+      return rows_off + (size_t)layers * p->conv_ny_max * 16 + 2 * (size_t)layers * p->conv_maxc * elems_per_chunk * p->esz;
+    };
+    const size_t need = p->fp32 ? std::max(total(24, 2), total(8, 2)) : std::max(total(12, 4), total(4, 4));
+    if (need > 227 * 1024) return MSM_ERR_UNSUPPORTED;
+    for (int l = 1; l < p->n_t; ++l)
+      if (2 * p->conv.lev[l - 1].R[2] + 4 > 255) return MSM_ERR_UNSUPPORTED;   // plane indices are bytes
+    p->conv_wpart =(double*)dev_alloc(p, (size_t)p->conv.total_vunits * 6 * sizeof(double));
     for (int l = 1; l < p->n_t; ++l) {
       ConvLevel& g = p->conv.lev[l - 1];
       g.wpart = p->conv_wpart + (size_t)g.vunit0 * 6;
