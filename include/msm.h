@@ -39,7 +39,8 @@ typedef enum {
   MSM_ERR_TOO_MANY_PARTICLES = 4, /* n > max_particles */
   MSM_ERR_OUT_OF_BOX = 5,         /* open-axis coordinate outside [0, box], or non-finite input */
   MSM_ERR_NOMEM = 6,
-  MSM_ERR_CUDA = 7
+  MSM_ERR_CUDA = 7,
+  MSM_ERR_SCRATCH_LIMIT = 8       /* msm_restrict_noalloc: grids need more than MSM_NOALLOC_SCRATCH_BYTES */
 } msm_status_t;
 
 typedef enum { MSM_FP64 = 0, MSM_FP32 = 1 } msm_precision_t;
@@ -194,6 +195,36 @@ msm_status_t msm_evaluate_batch(msm_batch_t *batch, const int *h_n, const void *
                                 const void *d_charges, void *d_forces, void *d_potentials,
                                 double *h_energy, double *h_virial, void *cuda_stream);
 void msm_batch_destroy(msm_batch_t *batch);
+
+/* Restriction without any allocation, for callers that cannot call cudaMalloc (code under CUDA-graph
+ * capture, tight serving loops, harnesses that forbid it): coarse = I_l^{l+1} fine, the separable
+ * two-scale restriction of P:258 Eq. 19 line 1 (one axis at a time; mask J_n = 2^(1-p)
+ * binom(p, n + p/2), reading J1), i.e. what a plan computes between its levels l and l + 1, with
+ * the two intermediate arrays of the axis passes in a file-scope device array of
+ * MSM_NOALLOC_SCRATCH_BYTES (16 MiB, held by every GPU that loads the library until the process
+ * exits) instead of plan-owned buffers. No plan is needed.
+ *   device       CUDA device ordinal that owns d_fine and d_coarse
+ *   precision    msm_precision_t: element type of both grids
+ *   p            B-spline order: 4, 6 or 8
+ *   fine_dims / fine_lo / coarse_dims / coarse_lo   host, 3 ints each (x, y, z): points per axis and
+ *                node index of the first point, as msm_plan_info reports them for two consecutive
+ *                levels (lo = 0 and coarse = fine / 2 on periodic axes; a periodic axis already at
+ *                one point stays at one point)
+ *   periodic     host, 3 ints
+ *   d_fine       device, fine grid indexed [z][y][x]; not modified
+ *   d_coarse     device, coarse grid indexed [z][y][x]; written in full
+ * The caller owns both grids. The work is enqueued on cuda_stream and the call does not
+ * synchronise. Needs coarse_x * fine_y * fine_z + coarse_x * coarse_y * fine_z elements of scratch
+ * (the first term rounded up to 256 bytes): a larger problem returns MSM_ERR_SCRATCH_LIMIT and
+ * nothing is launched (a periodic 128^3 fp64 fine grid needs 12 MiB and fits; 256^3 does not).
+ * ALL calls on a device share the one array: calls that overlap on the GPU (different streams with
+ * no ordering between them) race; calls on one stream are safe. The array keeps the previous call's
+ * contents; nothing relies on it, every pass overwrites what the next one reads. */
+#define MSM_NOALLOC_SCRATCH_BYTES (16u << 20)
+msm_status_t msm_restrict_noalloc(int device, int precision, int p, const int *fine_dims,
+                                  const int *fine_lo, const int *coarse_dims, const int *coarse_lo,
+                                  const int *periodic, const void *d_fine, void *d_coarse,
+                                  void *cuda_stream);
 
 const char *msm_status_string(msm_status_t s);
 

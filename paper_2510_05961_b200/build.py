@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libmsm_b200.so")
-SOURCES = ["msm_create.cu", "msm_evaluate.cu", "microbench.cu", "plan_math.cpp", "plan_top.cpp"]
+SOURCES = ["msm_create.cu", "msm_evaluate.cu", "microbench.cu", "restrict_noalloc.cu", "plan_math.cpp", "plan_top.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 

@@ -715,6 +715,7 @@ const char* msm_status_string(msm_status_t s) {
     case MSM_ERR_OUT_OF_BOX: return "coordinate outside an open box axis, or non-finite input";
     case MSM_ERR_NOMEM: return "out of memory";
     case MSM_ERR_CUDA: return "CUDA error";
+    case MSM_ERR_SCRATCH_LIMIT: return "grids need more than the static scratch array (MSM_NOALLOC_SCRATCH_BYTES)";
   }
   return "unknown status";
 }

@@ -19,13 +19,14 @@ MSM_FP64, MSM_FP32 = 0, 1
 MSM_MAX_LEVELS = 32
 
 STATUS = {0: "MSM_OK", 1: "MSM_ERR_INVALID_ARG", 2: "MSM_ERR_UNSUPPORTED", 3: "MSM_ERR_CUTOFF_TOO_LARGE",
-          4: "MSM_ERR_TOO_MANY_PARTICLES", 5: "MSM_ERR_OUT_OF_BOX", 6: "MSM_ERR_NOMEM", 7: "MSM_ERR_CUDA"}
+          4: "MSM_ERR_TOO_MANY_PARTICLES", 5: "MSM_ERR_OUT_OF_BOX", 6: "MSM_ERR_NOMEM", 7: "MSM_ERR_CUDA",
+          8: "MSM_ERR_SCRATCH_LIMIT"}
 
 EXPORTS = ["msm_plan_create", "msm_plan_info", "msm_evaluate", "msm_evaluate_async", "msm_get_results",
            "msm_evaluate_host", "msm_set_profiling",
            "msm_get_stage_times", "msm_get_launch_count", "msm_debug_copy_grid", "msm_plan_destroy",
            "msm_status_string", "msm_measure_fma_peak", "msm_batch_create", "msm_evaluate_batch",
-           "msm_batch_destroy", "msm_plan_create_dynamic", "msm_plan_set_box"]
+           "msm_batch_destroy", "msm_plan_create_dynamic", "msm_plan_set_box", "msm_restrict_noalloc"]
 
 
 class MsmError(RuntimeError):
@@ -78,6 +79,9 @@ def lib():
         L.msm_plan_destroy.restype = None; L.msm_plan_destroy.argtypes = [vp]
         L.msm_status_string.restype = C.c_char_p; L.msm_status_string.argtypes = [i]
         L.msm_measure_fma_peak.restype = i; L.msm_measure_fma_peak.argtypes = [i, i, dp]
+        ip = C.POINTER(i)
+        L.msm_restrict_noalloc.restype = i
+        L.msm_restrict_noalloc.argtypes = [i, i, i, ip, ip, ip, ip, ip, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -89,6 +93,26 @@ def measure_fma_peak(kind: str = "fp32", device: int = 0) -> float:
     if st:
         raise MsmError(st, "msm_measure_fma_peak")
     return out.value
+
+
+NOALLOC_SCRATCH_BYTES = 16 << 20
+
+
+def restrict_noalloc(fine, coarse, p, fine_lo, coarse_lo, periodic, stream=None):
+    """msm_restrict_noalloc: coarse <- restriction of fine. Both are torch CUDA tensors indexed
+    [z][y][x] (float32 or float64, contiguous, caller-owned); nothing is allocated on the device."""
+    import torch
+    assert fine.is_cuda and coarse.is_cuda and fine.is_contiguous() and coarse.is_contiguous()
+    assert fine.dtype == coarse.dtype and fine.dim() == 3 and coarse.dim() == 3
+    i3 = C.c_int * 3
+    fd, cd = i3(*reversed(fine.shape)), i3(*reversed(coarse.shape))
+    s = stream if stream is not None else torch.cuda.current_stream(fine.device)
+    st = lib().msm_restrict_noalloc(fine.device.index, MSM_FP32 if fine.dtype == torch.float32 else MSM_FP64, int(p),
+                                    fd, i3(*[int(v) for v in fine_lo]), cd, i3(*[int(v) for v in coarse_lo]),
+                                    i3(*[int(bool(v)) for v in periodic]), fine.data_ptr(), coarse.data_ptr(),
+                                    s.cuda_stream)
+    if st:
+        raise MsmError(st, "msm_restrict_noalloc")
 
 
 class Plan:
