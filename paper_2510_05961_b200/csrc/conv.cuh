@@ -51,6 +51,8 @@ struct ConvLevel {
   const void* taps2;          // per chunk 8 floats: (s_d[t], s_{d-1}[t]) for the chunk's 4 taps
   int n_rows2, n_taps2q;      // entries of rows2; float4 quads of taps2 including the guard chunk in front
   int sunit0;                 // first unit of this level in the shared-table launch (multiple of kConvSW)
+  const int2* elist;          // fp32 list-driven path: (window offset j * pitch + 4 c, chunk of pair 0 | chunk of pair 1 << 16)
+  const int* ehead;           // [2 R[2] + 4][kConvListTypes + 1]: list bounds per input plane offset d0 = zr
   const void* vtaps;          // per chunk: 4 x 2g, 4 x 2g dx, 4 x 2g dx^2
   const int4* vrows2;         // fp32 packed virial: half-space rows d and d - 1 merged, d = 0 .. R[2]+1
   const void* vtaps2;         // per chunk 24 floats: for 2g, 2g dx, 2g dx^2: 4 taps x (row d, row d - 1)
@@ -60,6 +62,7 @@ struct ConvLevel {
   double* wpart;              // virial partials, 6 per unit
 };
 
+constexpr int kConvListTypes = 7;   // both full | pair 0 full | pair 1 full | pair 0 lower, upper half | pair 1 lower, upper half
 constexpr int kConvSW = 8;    // warps (units) per block of the shared-table convolution kernel
 
 struct ConvTable {
@@ -470,6 +473,130 @@ k_conv_f2s(const ConvTable* __restrict__ tabp, int plane_bytes) {
   cu.Y = (r % g.tiles[1]) * 32;
   cu.Z = (r / g.tiles[1]) * 4;
   conv_f2_unit<XT, true>(g, cu, srows, staps + 2, planes + (size_t)warp * (plane_bytes / 4), lane);
+}
+
+// ------------------------------------------------------- potential, fp32, list-driven inner loops
+// The row/chunk loops above spend a quarter of their time on control flow: a stencil row is only
+// 1 - 6 chunks long, and every chunk tests which of the two plane pairs it feeds and whether it is
+// a half chunk (six warp-uniform branches around blocks of 32 FFMA2). Here the plan has sorted the
+// chunks of each input plane offset into kConvListTypes lists by exactly those properties
+// (ConvLevel::elist), and each list runs through a loop body that has no branch but its own.
+// M0 / M1: what pair 0 / pair 1 take from a chunk: 0 nothing, 1 all four taps, 2 taps 0-1, 3 taps 2-3.
+template <int XT, int M0, int M1>
+__device__ __forceinline__ void conv_list_run(int b, int e, const int2* __restrict__ el, const float* srow0,
+                                              const float4* taps2, unsigned long long (&acc)[2][XT]) {
+  if (b >= e) return;
+  int2 nxt = __ldg(el + b);
+#pragma unroll 1
+  for (int i = b; i < e; ++i) {
+    const int2 cur = nxt;
+    nxt = __ldg(el + i + 1);                          // (the list has a guard entry behind its end)
+    const float* w = srow0 + cur.x;
+    float win[XT + 4];
+#pragma unroll
+    for (int j = 0; j < XT + 4; j += 4) {
+      const float4 t = *reinterpret_cast<const float4*>(w + j);
+      win[j] = t.x; win[j + 1] = t.y; win[j + 2] = t.z; win[j + 3] = t.w;
+    }
+    float4 tq[2][2];
+    if (M0 == 1 || M0 == 2) tq[0][0] = taps2[2 * (cur.y & 0xffff)];
+    if (M0 == 1 || M0 == 3) tq[0][1] = taps2[2 * (cur.y & 0xffff) + 1];
+    if (M1 == 1 || M1 == 2) tq[1][0] = taps2[2 * ((unsigned)cur.y >> 16)];
+    if (M1 == 1 || M1 == 3) tq[1][1] = taps2[2 * ((unsigned)cur.y >> 16) + 1];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const int m = k == 0 ? M0 : M1;
+      if (m == 1 || m == 2) {
+        const unsigned long long t0 = pack2(tq[k][0].x, tq[k][0].y), t1 = pack2(tq[k][0].z, tq[k][0].w);
+#pragma unroll
+        for (int i2 = 0; i2 < XT; ++i2) {
+          ffma2_bcast(acc[k][i2], win[i2], t0);
+          ffma2_bcast(acc[k][i2], win[i2 + 1], t1);
+        }
+      }
+      if (m == 1 || m == 3) {
+        const unsigned long long t2 = pack2(tq[k][1].x, tq[k][1].y), t3 = pack2(tq[k][1].z, tq[k][1].w);
+#pragma unroll
+        for (int i2 = 0; i2 < XT; ++i2) {
+          ffma2_bcast(acc[k][i2], win[i2 + 2], t2);
+          ffma2_bcast(acc[k][i2], win[i2 + 3], t3);
+        }
+      }
+    }
+  }
+}
+
+template <int XT>
+__global__ void __launch_bounds__(32 * kConvSW, 2)
+k_conv_f2l(const ConvTable* __restrict__ tabp, int plane_bytes) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const ConvTable& tab = *tabp;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int l = 0;
+#pragma unroll 1
+  for (int k = 1; k < tab.nlev; ++k)
+    if ((int)blockIdx.x * kConvSW >= tab.lev[k].sunit0) l = k;
+  const ConvLevel& g = tab.lev[l];
+  float4* staps = reinterpret_cast<float4*>(smem_raw);
+  float* planes = reinterpret_cast<float*>(staps + g.n_taps2q);
+  const float4* gt = reinterpret_cast<const float4*>(g.taps2) - 2;          // from the guard chunk on
+  for (int i = threadIdx.x; i < g.n_taps2q; i += 32 * kConvSW) staps[i] = __ldg(gt + i);
+  __syncthreads();
+  int r = (int)blockIdx.x * kConvSW + warp - g.sunit0;
+  if (r >= g.tiles[0] * g.tiles[1] * g.tiles[2] * g.nslices) return;         // padding unit
+  const int slice = r % g.nslices; r /= g.nslices;
+  const int X = (r % g.tiles[0]) * XT; r /= g.tiles[0];
+  const int Y = (r % g.tiles[1]) * 32;
+  const int Z = (r / g.tiles[1]) * 4;
+  float* plane = planes + (size_t)warp * (plane_bytes / 4);
+  const float4* taps2 = staps + 2;
+  const int Ry = g.R[1], Rz = g.R[2];
+  const int nrow = 32 + 2 * Ry;
+  const int WX = XT + 2 * g.X0 + 4;
+  const float* __restrict__ qpad = reinterpret_cast<const float*>(g.pad);
+  const int2* __restrict__ el = g.elist;
+  const float* srow0 = plane + lane * g.pitch;
+
+  unsigned long long acc[2][XT];                      // (plane 2k, plane 2k + 1) of output x + i
+#pragma unroll
+  for (int k = 0; k < 2; ++k)
+#pragma unroll
+    for (int i = 0; i < XT; ++i) acc[k][i] = 0ull;
+
+  const int p0 = g.pb[slice], p1 = g.pb[slice + 1];
+#pragma unroll 1
+  for (int pz = p0; pz < p1; ++pz) {                  // input plane z = Z + pz - Rz: list set d0 = pz - Rz
+    const int4 h0 = __ldg(reinterpret_cast<const int4*>(g.ehead + pz * (kConvListTypes + 1)));
+    const int4 h1 = __ldg(reinterpret_cast<const int4*>(g.ehead + pz * (kConvListTypes + 1)) + 1);
+    stage_plane<float>(g, qpad, plane, Z + pz, X, Y, nrow, WX, lane);     // commits and waits
+    conv_list_run<XT, 1, 1>(h0.x, h0.y, el, srow0, taps2, acc);
+    conv_list_run<XT, 1, 0>(h0.y, h0.z, el, srow0, taps2, acc);
+    conv_list_run<XT, 0, 1>(h0.z, h0.w, el, srow0, taps2, acc);
+    conv_list_run<XT, 2, 0>(h0.w, h1.x, el, srow0, taps2, acc);
+    conv_list_run<XT, 3, 0>(h1.x, h1.y, el, srow0, taps2, acc);
+    conv_list_run<XT, 0, 2>(h1.y, h1.z, el, srow0, taps2, acc);
+    conv_list_run<XT, 0, 3>(h1.z, h1.w, el, srow0, taps2, acc);
+  }
+  // outputs (slice partial or the final value)
+  const int y = Y + lane;
+  if (y < g.M[1]) {
+    float* out = reinterpret_cast<float*>(g.out) + (size_t)slice * g.M[0] * g.M[1] * g.M[2];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      float* d0 = out + ((size_t)(Z + 2 * k) * g.M[1] + y) * g.M[0] + X;
+      float* d1 = d0 + (size_t)g.M[1] * g.M[0];
+      const bool z0 = Z + 2 * k < g.M[2], z1 = Z + 2 * k + 1 < g.M[2];
+#pragma unroll
+      for (int i = 0; i < XT; ++i) {
+        float lo, hi;
+        unpack2(acc[k][i], lo, hi);
+        if (X + i < g.M[0]) {
+          if (z0) d0[i] = lo;
+          if (z1) d1[i] = hi;
+        }
+      }
+    }
+  }
 }
 
 // E[i] = sum_s part[s][i], s ascending (fixed order)

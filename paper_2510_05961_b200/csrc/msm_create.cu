@@ -155,6 +155,8 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   d.tab[0] = TapTable{const_cast<void*>(g.staps), upload_desc(p, tsd), (int)ts.size()};
   d.tab[2] = TapTable{const_cast<void*>(g.vtaps), upload_desc(p, tvd), (int)tv.size()};
   g.rows2 = nullptr;
+  g.elist = nullptr;
+  g.ehead = nullptr;
   g.taps2 = nullptr;
   g.vrows2 = nullptr;
   g.vtaps2 = nullptr;
@@ -258,6 +260,57 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
     g.taps2 = (const char*)t2dev + 8 * p->esz;   // chunk 0 of the table follows the guard chunk
     g.n_rows2 = (int)r2.size();
     g.n_taps2q = (int)(t2.size() / 4);
+    // Entry lists of the list-driven kernel (k_conv_f2l): input plane zr feeds the output plane pairs
+    // k = 0, 1 through the merged layers d0 = zr and d0 - 2. Per d0, the chunks of all stencil rows
+    // are sorted by what they need -- both pairs in full / one pair in full / the lower or upper 2-tap
+    // half of one pair -- so that each list runs through a loop body without any branch.
+    g.elist = nullptr;
+    g.ehead = nullptr;
+    if (t2.size() / 8 < 65536) {
+      auto state = [&](int d, int j, int c, int& chunk) {      // 0 off, 1 full, 2 lower half, 3 upper half
+        if (d < -Rz || d > Rz + 1) return 0;
+        const int4& r = r2[(size_t)(d + Rz) * ny + j];
+        if (c < r.y || c > r.z) return 0;
+        chunk = r.x + (c - r.y);
+        const bool lo = 2 * c >= (r.w & 0xffff), hi = 2 * c + 1 <= (r.w >> 16);
+        return lo && hi ? 1 : lo ? 2 : hi ? 3 : 0;
+      };
+      std::vector<int2> el;
+      std::vector<int> eh;
+      const int cmax = (2 * g.X0) / 4 + 1;
+      for (int d0 = -Rz; d0 <= Rz + 3; ++d0) {
+        std::vector<int2> lists[kConvListTypes];
+        for (int j = 0; j < ny; ++j)
+          for (int c = 0; c <= cmax; ++c) {
+            int c0 = 0, c1 = 0;
+            const int s0 = state(d0, j, c, c0), s1 = state(d0 - 2, j, c, c1);
+            const int win = j * g.pitch + 4 * c;
+            const int2 e = make_int2(win, c0 | (c1 << 16));
+            if (s0 == 1 && s1 == 1) { lists[0].push_back(e); continue; }
+            if (s0 == 1) lists[1].push_back(e);
+            if (s1 == 1) lists[2].push_back(e);
+            if (s0 == 2) lists[3].push_back(e);
+            if (s0 == 3) lists[4].push_back(e);
+            if (s1 == 2) lists[5].push_back(e);
+            if (s1 == 3) lists[6].push_back(e);
+          }
+        for (int t = 0; t < kConvListTypes; ++t) {
+          eh.push_back((int)el.size());
+          el.insert(el.end(), lists[t].begin(), lists[t].end());
+        }
+        eh.push_back((int)el.size());
+      }
+      el.push_back(make_int2(0, 0));                           // the loops prefetch one entry ahead
+      int2* eld = (int2*)dev_alloc(p, el.size() * sizeof(int2));
+      int* ehd = (int*)dev_alloc(p, eh.size() * sizeof(int));
+      if (cudaMemcpy(eld, el.data(), el.size() * sizeof(int2), cudaMemcpyHostToDevice) != cudaSuccess ||
+          cudaMemcpy(ehd, eh.data(), eh.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess)
+        throw CudaFail();
+      g.elist = eld;
+      g.ehead = ehd;
+    } else {
+      p->conv_lists = false;
+    }
   }
   d.pad = dev_alloc(p, (size_t)g.P[0] * g.P[1] * g.P[2] * p->esz);
   g.pad = d.pad;
@@ -280,7 +333,7 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
     }
   const int tiles = g.tiles[0] * g.tiles[1] * g.tiles[2];
   g.nslices = std::max(1, std::min({p->conv_slices, nplanes, kMaxConvSlices}));
-  g.vslices = std::max(1, std::min({(p->conv_slices + 1) / 2, vplanes, kMaxConvSlices}));
+  g.vslices = std::max(1, std::min({p->conv_vslices, vplanes, kMaxConvSlices}));
   balanced_bounds(wp, g.nslices, g.pb);
   balanced_bounds(wv, g.vslices, g.vb);
   g.unit0 = p->conv.total_units;
@@ -330,15 +383,29 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
     return MSM_ERR_CUDA;
 
   // ---- grids
-  // slices per output tile of the convolution: enough one-warp units for ~3 resident waves
+  // slices per output tile of the convolution. fp32: one-warp units for about two resident waves of
+  // the potential kernel and one of the virial kernel (16 warps per SM). Measured at 128^3 + 64^3 +
+  // 32^3 (1168 tiles, 148 SMs): 4 / 2 slices 0.630 / 0.555 ms; 7 / 4 (3.45 / 1.97 waves) 0.663 / 0.609 ms
   {
     const int XTc = p->fp32 ? 16 : 8;
     long long tiles = 0;
     for (int l = 1; l < p->n_t; ++l)
       tiles += (long long)((H.lev[l].M[0] + XTc - 1) / XTc) * ((H.lev[l].M[1] + 31) / 32) * ((H.lev[l].M[2] + 3) / 4);
-    const long long target = (long long)p->sm_count * 16 * 3;
-    p->conv_slices = tiles > 0 ? (int)std::max<long long>(1, std::min<long long>(kMaxConvSlices, (target + tiles - 1) / tiles)) : 1;
+    const long long slots = (long long)p->sm_count * 16;
+    if (p->fp32) {
+      auto per_tile = [&](long long units) {
+        return tiles > 0 ? (int)std::max<long long>(1, std::min<long long>(kMaxConvSlices, (units + tiles / 2) / tiles)) : 1;
+      };
+      p->conv_slices = per_tile(2 * slots);
+      p->conv_vslices = per_tile(slots);
+    } else {
+      // fp64 (12 / 9 resident warps per SM, units twice as long): more, smaller units measured faster
+      // (N = 10^6: 4 / 2 slices 1.736 / 1.545 ms, 2 / 1 slices 1.812 / 1.567 ms)
+      p->conv_slices = tiles > 0 ? (int)std::max<long long>(1, std::min<long long>(kMaxConvSlices, (3 * slots + tiles - 1) / tiles)) : 1;
+      p->conv_vslices = (p->conv_slices + 1) / 2;
+    }
     if (const char* e = std::getenv("MSM_CONV_SLICES")) p->conv_slices = std::max(1, std::atoi(e));
+    if (const char* e = std::getenv("MSM_CONV_VSLICES")) p->conv_vslices = std::max(1, std::atoi(e));
   }
   size_t tmp_elems = 16;
   const int XT = p->fp32 ? 16 : 8, ZT = 4;

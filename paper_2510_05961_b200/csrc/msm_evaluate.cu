@@ -414,8 +414,10 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
         const size_t plane_b = (p->conv_smem + 15) / 16 * 16;
         const size_t sm_s = p->conv_tables_smem + kConvSW * plane_b;
         static const bool no_s = std::getenv("MSM_CONV_GLOBAL_TAPS") != nullptr;
+        static const bool no_l = std::getenv("MSM_CONV_NO_LISTS") != nullptr;
         if (!no_s && sm_s <= 110 * 1024 && p->conv.total_units >= 4096) {   // small jobs: the table copy does not pay
-          auto kern = k_conv_f2s<XT>;
+          // list-driven inner loops when every level has its entry lists (msm_create.cu)
+          auto kern = p->conv_lists && !no_l ? k_conv_f2l<XT> : k_conv_f2s<XT>;
           cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_s);
           MSM_LAUNCH(p, (kern<<<p->conv.total_sunits / kConvSW, 32 * kConvSW, sm_s, st>>>(p->d_conv, (int)plane_b)));
         } else {
