@@ -51,7 +51,7 @@ struct ConvLevel {
   const void* taps2;          // per chunk 8 floats: (s_d[t], s_{d-1}[t]) for the chunk's 4 taps
   int n_rows2, n_taps2q;      // entries of rows2; float4 quads of taps2 including the guard chunk in front
   int sunit0;                 // first unit of this level in the shared-table launch (multiple of kConvSW)
-  const int2* elist;          // fp32 list-driven path: (window offset j * pitch + 4 c, chunk of pair 0 | chunk of pair 1 << 16)
+  const int4* elist;          // fp32 list-driven path: byte offsets of (window j * pitch + 4 c in the lane's rows, chunk of pair 0, of pair 1 in taps2)
   const int* ehead;           // [2 R[2] + 4][kConvListTypes + 1]: list bounds per input plane offset d0 = zr
   const void* vtaps;          // per chunk: 4 x 2g, 4 x 2g dx, 4 x 2g dx^2
   const int4* vrows2;         // fp32 packed virial: half-space rows d and d - 1 merged, d = 0 .. R[2]+1
@@ -482,45 +482,53 @@ k_conv_f2s(const ConvTable* __restrict__ tabp, int plane_bytes) {
 // chunks of each input plane offset into kConvListTypes lists by exactly those properties
 // (ConvLevel::elist), and each list runs through a loop body that has no branch but its own.
 // M0 / M1: what pair 0 / pair 1 take from a chunk: 0 nothing, 1 all four taps, 2 taps 0-1, 3 taps 2-3.
+// 16-byte shared-memory load at a 32-bit shared-space address + immediate (the address arithmetic of
+// a list entry is one integer add; generic pointers cost the compiler a 64-bit add and, under the
+// register cap, a recomputation of the lane's row address in every iteration)
+template <int OFF>
+__device__ __forceinline__ float4 lds128(unsigned addr) {
+  float4 v;
+  asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+%5];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr), "n"(OFF));
+  return v;
+}
+
 template <int XT, int M0, int M1>
-__device__ __forceinline__ void conv_list_run(int b, int e, const int2* __restrict__ el, const float* srow0,
-                                              const float4* taps2, unsigned long long (&acc)[2][XT]) {
+__device__ __forceinline__ void conv_list_run(int b, int e, const int4* __restrict__ el, unsigned srow0, unsigned taps2,
+                                              unsigned long long (&acc)[2][XT]) {
   if (b >= e) return;
-  int2 nxt = __ldg(el + b);
+  int4 nxt = __ldg(el + b);
 #pragma unroll 1
   for (int i = b; i < e; ++i) {
-    const int2 cur = nxt;
+    const int4 cur = nxt;                             // (window, taps of pair 0, taps of pair 1) byte offsets
     nxt = __ldg(el + i + 1);                          // (the list has a guard entry behind its end)
-    const float* w = srow0 + cur.x;
+    const unsigned w = srow0 + (unsigned)cur.x;
     float win[XT + 4];
-#pragma unroll
-    for (int j = 0; j < XT + 4; j += 4) {
-      const float4 t = *reinterpret_cast<const float4*>(w + j);
-      win[j] = t.x; win[j + 1] = t.y; win[j + 2] = t.z; win[j + 3] = t.w;
+    {
+      const float4 t0 = lds128<0>(w), t1 = lds128<16>(w), t2 = lds128<32>(w), t3 = lds128<48>(w), t4 = lds128<64>(w);
+      static_assert(XT == 16, "window of 20 floats");
+      win[0] = t0.x; win[1] = t0.y; win[2] = t0.z; win[3] = t0.w;
+      win[4] = t1.x; win[5] = t1.y; win[6] = t1.z; win[7] = t1.w;
+      win[8] = t2.x; win[9] = t2.y; win[10] = t2.z; win[11] = t2.w;
+      win[12] = t3.x; win[13] = t3.y; win[14] = t3.z; win[15] = t3.w;
+      win[16] = t4.x; win[17] = t4.y; win[18] = t4.z; win[19] = t4.w;
     }
     float4 tq[2][2];
-    if (M0 == 1 || M0 == 2) tq[0][0] = taps2[2 * (cur.y & 0xffff)];
-    if (M0 == 1 || M0 == 3) tq[0][1] = taps2[2 * (cur.y & 0xffff) + 1];
-    if (M1 == 1 || M1 == 2) tq[1][0] = taps2[2 * ((unsigned)cur.y >> 16)];
-    if (M1 == 1 || M1 == 3) tq[1][1] = taps2[2 * ((unsigned)cur.y >> 16) + 1];
+    if (M0 == 1 || M0 == 2) tq[0][0] = lds128<0>(taps2 + (unsigned)cur.y);
+    if (M0 == 1 || M0 == 3) tq[0][1] = lds128<16>(taps2 + (unsigned)cur.y);
+    if (M1 == 1 || M1 == 2) tq[1][0] = lds128<0>(taps2 + (unsigned)cur.z);
+    if (M1 == 1 || M1 == 3) tq[1][1] = lds128<16>(taps2 + (unsigned)cur.z);
+    // tap by tap over all accumulators: consecutive FFMA2 are independent (the next one into the
+    // same accumulator is 16 or 32 instructions away)
 #pragma unroll
-    for (int k = 0; k < 2; ++k) {
-      const int m = k == 0 ? M0 : M1;
-      if (m == 1 || m == 2) {
-        const unsigned long long t0 = pack2(tq[k][0].x, tq[k][0].y), t1 = pack2(tq[k][0].z, tq[k][0].w);
+    for (int t = 0; t < 4; ++t) {
 #pragma unroll
-        for (int i2 = 0; i2 < XT; ++i2) {
-          ffma2_bcast(acc[k][i2], win[i2], t0);
-          ffma2_bcast(acc[k][i2], win[i2 + 1], t1);
-        }
-      }
-      if (m == 1 || m == 3) {
-        const unsigned long long t2 = pack2(tq[k][1].x, tq[k][1].y), t3 = pack2(tq[k][1].z, tq[k][1].w);
+      for (int k = 0; k < 2; ++k) {
+        const int m = k == 0 ? M0 : M1;
+        if (!(m == 1 || (m == 2 && t < 2) || (m == 3 && t >= 2))) continue;
+        const float4 q = tq[k][t >> 1];
+        const unsigned long long tp = (t & 1) ? pack2(q.z, q.w) : pack2(q.x, q.y);
 #pragma unroll
-        for (int i2 = 0; i2 < XT; ++i2) {
-          ffma2_bcast(acc[k][i2], win[i2 + 2], t2);
-          ffma2_bcast(acc[k][i2], win[i2 + 3], t3);
-        }
+        for (int i2 = 0; i2 < XT; ++i2) ffma2_bcast(acc[k][i2], win[i2 + t], tp);
       }
     }
   }
@@ -549,13 +557,15 @@ k_conv_f2l(const ConvTable* __restrict__ tabp, int plane_bytes) {
   const int Y = (r % g.tiles[1]) * 32;
   const int Z = (r / g.tiles[1]) * 4;
   float* plane = planes + (size_t)warp * (plane_bytes / 4);
-  const float4* taps2 = staps + 2;
   const int Ry = g.R[1], Rz = g.R[2];
   const int nrow = 32 + 2 * Ry;
   const int WX = XT + 2 * g.X0 + 4;
   const float* __restrict__ qpad = reinterpret_cast<const float*>(g.pad);
-  const int2* __restrict__ el = g.elist;
-  const float* srow0 = plane + lane * g.pitch;
+  const int4* __restrict__ el = g.elist;
+  // (opaque moves: the compiler would otherwise recompute the lane's row address in every iteration)
+  unsigned srow0, taps2;
+  asm volatile("mov.u32 %0, %1;" : "=r"(srow0) : "r"((unsigned)__cvta_generic_to_shared(plane + lane * g.pitch)));
+  asm volatile("mov.u32 %0, %1;" : "=r"(taps2) : "r"((unsigned)__cvta_generic_to_shared(staps + 2)));
 
   unsigned long long acc[2][XT];                      // (plane 2k, plane 2k + 1) of output x + i
 #pragma unroll

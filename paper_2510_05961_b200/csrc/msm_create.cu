@@ -266,7 +266,7 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
     // half of one pair -- so that each list runs through a loop body without any branch.
     g.elist = nullptr;
     g.ehead = nullptr;
-    if (t2.size() / 8 < 65536) {
+    {
       auto state = [&](int d, int j, int c, int& chunk) {      // 0 off, 1 full, 2 lower half, 3 upper half
         if (d < -Rz || d > Rz + 1) return 0;
         const int4& r = r2[(size_t)(d + Rz) * ny + j];
@@ -275,17 +275,16 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
         const bool lo = 2 * c >= (r.w & 0xffff), hi = 2 * c + 1 <= (r.w >> 16);
         return lo && hi ? 1 : lo ? 2 : hi ? 3 : 0;
       };
-      std::vector<int2> el;
+      std::vector<int4> el;
       std::vector<int> eh;
       const int cmax = (2 * g.X0) / 4 + 1;
       for (int d0 = -Rz; d0 <= Rz + 3; ++d0) {
-        std::vector<int2> lists[kConvListTypes];
+        std::vector<int4> lists[kConvListTypes];
         for (int j = 0; j < ny; ++j)
           for (int c = 0; c <= cmax; ++c) {
             int c0 = 0, c1 = 0;
             const int s0 = state(d0, j, c, c0), s1 = state(d0 - 2, j, c, c1);
-            const int win = j * g.pitch + 4 * c;
-            const int2 e = make_int2(win, c0 | (c1 << 16));
+            const int4 e = make_int4((j * g.pitch + 4 * c) * 4, c0 * 32, c1 * 32, 0);   // bytes
             if (s0 == 1 && s1 == 1) { lists[0].push_back(e); continue; }
             if (s0 == 1) lists[1].push_back(e);
             if (s1 == 1) lists[2].push_back(e);
@@ -300,16 +299,14 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
         }
         eh.push_back((int)el.size());
       }
-      el.push_back(make_int2(0, 0));                           // the loops prefetch one entry ahead
-      int2* eld = (int2*)dev_alloc(p, el.size() * sizeof(int2));
+      el.push_back(make_int4(0, 0, 0, 0));                           // the loops prefetch one entry ahead
+      int4* eld = (int4*)dev_alloc(p, el.size() * sizeof(int4));
       int* ehd = (int*)dev_alloc(p, eh.size() * sizeof(int));
-      if (cudaMemcpy(eld, el.data(), el.size() * sizeof(int2), cudaMemcpyHostToDevice) != cudaSuccess ||
+      if (cudaMemcpy(eld, el.data(), el.size() * sizeof(int4), cudaMemcpyHostToDevice) != cudaSuccess ||
           cudaMemcpy(ehd, eh.data(), eh.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess)
         throw CudaFail();
       g.elist = eld;
       g.ehead = ehd;
-    } else {
-      p->conv_lists = false;
     }
   }
   d.pad = dev_alloc(p, (size_t)g.P[0] * g.P[1] * g.P[2] * p->esz);
