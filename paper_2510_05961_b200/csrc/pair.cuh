@@ -6,14 +6,17 @@
 // (sort.cuh), so the neighbours of a particle in one of the 25 neighbouring rows (dy, dz) are ONE
 // contiguous range of the sorted order (two when the x window wraps around a periodic box).
 //
-// Work unit = one warp = a CLUSTER of 8 consecutive sorted particles of one row, laid out as
-// 8 i-particles x 4 j-phases: lane = 8 * jq + il owns particle il and every fourth PAIR of
-// candidates. A cluster is ~0.4 cutoffs long in x (a 32-particle tile is as long as the cutoff
+// Work unit = one warp = a CLUSTER of 16 consecutive sorted particles of one row, laid out as
+// 16 i-particles x 2 j-phases: lane = 16 * jq + il owns particle il and every second PAIR of
+// candidates. A cluster is ~0.85 cutoffs long in x at liquid density: its candidate windows are 18 %
+// longer than those of an 8-particle cluster, but they are staged (and the 25 rows set up) once for
+// twice as many particles, and staging + set-up were half of the 8-particle kernel's instructions
+// (a 32-particle tile is twice as long as the cutoff
 // itself), and the x window of every row is cut to the reach the cutoff sphere still has at that
 // row's (dy, dz) distance, in sub-bin units. The candidates of all rows are staged through shared
 // memory in the cluster's frame (coordinates relative to the cluster's first cell: fp32
 // differences stay accurate) as one flat list, so that every step of the inner loop is a full
-// 8 i x 8 j block of pairs with no ragged row ends.
+// 16 i x 4 j block of pairs with no ragged row ends.
 //
 // fp32: every staged candidate is evaluated in full with packed f32x2 arithmetic (FADD2 / FMUL2 /
 //   FFMA2: two pairs per instruction and lane) and masked by the cutoff test -- no hit lists, no
@@ -35,7 +38,7 @@
 //
 // Small systems have too few clusters to fill the GPU: the dz planes of the neighbourhood are then
 // dealt to up to kPairMaxSplit blocks (blockIdx.z) whose partial sums k_interpolate adds in order.
-// Every lane visits its candidates in a fixed order and the four phases of a particle are added
+// Every lane visits its candidates in a fixed order and the two phases of a particle are added
 // in a fixed order, so the sums are run-to-run deterministic.
 // -k_0'(r)/r = 1/r^3 + (2/a^3) g'(s), s = r^2/a^2 - 1: one rsqrt per pair is the only special
 // function.
@@ -66,9 +69,11 @@ template <typename T> struct PairParams {
 
 // independent warps (clusters) per block: fp64 stages 14 KB per warp (48 KB static limit)
 template <typename T> struct PairWarps { static constexpr int value = sizeof(T) == 4 ? 4 : 2; };
-constexpr int kPairCluster = 8;     // i-particles per warp
+constexpr int kPairCluster = 16;    // i-particles per warp
+constexpr int kPairPhases = 32 / kPairCluster;   // lanes per i-particle: each takes every kPairPhases-th PAIR of candidates
+constexpr int kPairStep = 2 * kPairPhases;       // candidates per step of the inner loop
 constexpr int kPairMaxSplit = 5;
-constexpr int kPairSpanCap = 2;     // a cluster pass spans at most this many cells beyond its first
+constexpr int kPairSpanCap = 3;     // a cluster pass spans at most this many cells beyond its first
 
 // Shared-memory staging of one warp. fp32 records are interleaved in pairs of candidates,
 // (x0 x1 | y0 y1 | z0 z1 | q0 q1), so that a lane's pair is two 16-byte loads feeding packed
@@ -92,7 +97,7 @@ template <> struct PairStage<double> {
   static constexpr int kCap = 256;
   __align__(16) float f[kCap * 4];            // fp32 copy for the scan (q slots unused)
   double4 d[kCap];                            // full precision for the drain
-  unsigned char list[kCap * 8];               // hit r of lane l at [r * 32 + l]; a lane scans kCap / 4 candidates
+  unsigned char list[kCap / kPairPhases * 32];   // hit r of lane l at [r * 32 + l]; a lane scans kCap / kPairPhases candidates
   __device__ __forceinline__ void put(int k, double4 r) {
     d[k] = r;
     float* q = f + pair_slot(k);
@@ -176,7 +181,8 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
   constexpr bool kSplit = !MI;
   __shared__ PairStage<T> stage[kPairWarps];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  const int il = lane & 7, jq = lane >> 3;
+  const int il = lane & (kPairCluster - 1), jq = lane / kPairCluster;   // i-particle and candidate phase of this lane
+  const int l8 = lane & 7;                          // staging: eight lanes per neighbour row
   PairStage<T>& sj = stage[wid];
   const int row = blockIdx.x;                       // (cy, cz); blockIdx.y strides over the row's clusters
   const int cy = row % prm.nc[1], cz = row / prm.nc[1];
@@ -241,7 +247,7 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
    for (int first = 0; first <= last;) {
     const int fp0 = first;
     const int binf = __shfl_sync(0xffffffffu, bxi, first);
-    const unsigned fits = __ballot_sync(0xffffffffu, inrow && il >= first && bxi - binf <= span_max) & 0xffu;
+    const unsigned fits = __ballot_sync(0xffffffffu, inrow && il >= first && bxi - binf <= span_max) & ((1u << kPairCluster) - 1u);
     const int sub_last = 31 - __clz((int)fits);            // sub-bins ascend with il
     const bool iv = il >= first && il <= sub_last;
     const int binl = __shfl_sync(0xffffffffu, bxi, sub_last);
@@ -315,7 +321,7 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
       {
         const int gs = grp == 0 ? e0 : grp == 1 ? e1 : grp == 2 ? e2 : e3;
         const int ge = grp == 0 ? b0 : grp == 1 ? b1 : grp == 2 ? b2 : total;
-        const int pos = gs + il;
+        const int pos = gs + l8;
         if (pos < ge && pos >= base && pos < hi) sj.put(pos - base, make_vec4<T>(far, 0, 0, 0));
       }
       // ---- stage: four rows at a time, eight lanes per row, into the cluster's frame
@@ -329,7 +335,7 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
           // four elements per lane and batch: all eight loads of a batch are issued before the
           // first store, so a batch costs one global-memory latency instead of four
 #pragma unroll 1
-          for (int tb = max(0, base - o0) + il; tb < t1; tb += 32) {
+          for (int tb = max(0, base - o0) + l8; tb < t1; tb += 32) {
             V4 rj[4];
             int cj[4];
 #pragma unroll
@@ -357,13 +363,13 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
       }
       __syncwarp();
 
-      // ---- candidates [lo, hi2) of the flat list (multiples of 8) against the 8 particles.
+      // ---- candidates [lo, hi2) of the flat list (multiples of 8) against the cluster's particles.
       // MODE: kPairPlain / kPairImage / kPairImageF; SELF: the range may hold the cluster's own
       // particles (index test)
       auto run = [&](int lo, int hi2, auto modec, auto selfc) {
         constexpr int MODE = decltype(modec)::value;
         constexpr bool SELF = decltype(selfc)::value;
-        const int nsteps = (hi2 - lo) >> 3;
+        const int nsteps = (hi2 - lo) / kPairStep;
         if (nsteps <= 0) return;
         if constexpr (kPacked) {
           const float ia2 = (float)inv_a2, nia = -(float)inv_a, t3 = (float)two_inv_a3;
@@ -382,7 +388,7 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
             float2 qj;
             if (SELF) {
               qj = make_float2((r2.x < a2_scan && jdx != 0) ? zq.z : 0.f, (r2.y < a2_scan && jdx != -1) ? zq.w : 0.f);
-              jdx += 8;
+              jdx += kPairStep;
             } else {
               qj = make_float2(r2.x < a2_scan ? zq.z : 0.f, r2.y < a2_scan ? zq.w : 0.f);
             }
@@ -405,7 +411,7 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
             } else {
               A2.ax = __ffma2_rn(fs, dx, A2.ax); A2.ay = __ffma2_rn(fs, dy, A2.ay); A2.az = __ffma2_rn(fs, dz, A2.az);
             }
-            fp += 32;
+            fp += 4 * kPairStep;
           }
         } else if constexpr (kLists) {
           // scan: packed fp32 distance test of this lane's candidate pairs, hits appended to its list
@@ -425,8 +431,8 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
               const float2 r2 = __ffma2_rn(dx, dx, __ffma2_rn(dy, dy, __fmul2_rn(dz, dz)));
               if (r2.x < a2_scan && idx != selfl) { *le = (unsigned char)idx; le += 32; }
               if (r2.y < a2_scan && idx + 1 != selfl) { *le = (unsigned char)(idx + 1); le += 32; }
-              fp += 32;
-              idx += 8;
+              fp += 4 * kPairStep;
+              idx += kPairStep;
             }
           }
           const int n = (int)(le - lp) >> 5;                    // hits of this lane
@@ -454,7 +460,7 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
           for (int s = 0; s < nsteps; ++s) {
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-              const int pos = lo + s * 8 + 2 * jq + h;
+              const int pos = lo + s * kPairStep + 2 * jq + h;
               const V4 pj = sj.full(pos - base);
               T dx = xi - pj.x, dy = yi - pj.y, dz = zi - pj.z;
               if (mix) dx -= prm.box[0] * rint(dx * prm.inv_box[0]);
@@ -532,12 +538,13 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
         W[3] += 0.5 * (fx * ry + fy * rx); W[4] += 0.5 * (fx * rz + fz * rx); W[5] += 0.5 * (fy * rz + fz * ry);
       }
     }
-    // total force factor sums; the four phases of a particle, in a fixed order
+    // total force factor sums; the phases of a particle, in a fixed order
     A.ax += A.bx; A.ay += A.by; A.az += A.bz;
-    A.ax += __shfl_xor_sync(0xffffffffu, A.ax, 8); A.ay += __shfl_xor_sync(0xffffffffu, A.ay, 8);
-    A.az += __shfl_xor_sync(0xffffffffu, A.az, 8); A.av += __shfl_xor_sync(0xffffffffu, A.av, 8);
-    A.ax += __shfl_xor_sync(0xffffffffu, A.ax, 16); A.ay += __shfl_xor_sync(0xffffffffu, A.ay, 16);
-    A.az += __shfl_xor_sync(0xffffffffu, A.az, 16); A.av += __shfl_xor_sync(0xffffffffu, A.av, 16);
+#pragma unroll
+    for (int o = kPairCluster; o < 32; o <<= 1) {
+      A.ax += __shfl_xor_sync(0xffffffffu, A.ax, o); A.ay += __shfl_xor_sync(0xffffffffu, A.ay, o);
+      A.az += __shfl_xor_sync(0xffffffffu, A.az, o); A.av += __shfl_xor_sync(0xffffffffu, A.av, o);
+    }
     if (iv && jq == 0) {
       const int orig = porder[ki];
       T* Fp = Fsr + (size_t)blockIdx.z * 3 * prm.part_stride;   // partial of this split
