@@ -56,6 +56,9 @@ struct ConvLevel {
   const void* vtaps;          // per chunk: 4 x 2g, 4 x 2g dx, 4 x 2g dx^2
   const int4* vrows2;         // fp32 packed virial: half-space rows d and d - 1 merged, d = 0 .. R[2]+1
   const void* vtaps2;         // per chunk 24 floats: for 2g, 2g dx, 2g dx^2: 4 taps x (row d, row d - 1)
+  const int4* vlist;          // list-driven virial: byte offsets (window, chunk of pair 0, of pair 1 in vtaps2), dy as float bits
+  const int* vhead;           // [R[2] + 4][kConvListTypes + 1]: list bounds per input plane offset zr
+  int n_vtaps2q, vsunit0;     // float4 quads of vtaps2; first unit of this level in the list-driven virial launch
   const void* pad;            // omega'-filtered haloed grid charge
   const void* Q;              // grid charge (virial)
   void* out;                  // E^l if nslices == 1, else scratch [slice][z][y][x]
@@ -63,11 +66,12 @@ struct ConvLevel {
 };
 
 constexpr int kConvListTypes = 7;   // both full | pair 0 full | pair 1 full | pair 0 lower, upper half | pair 1 lower, upper half
+constexpr int kConvVW = 16;   // warps (units) per block of the list-driven virial kernel (one block per SM)
 constexpr int kConvSW = 8;    // warps (units) per block of the shared-table convolution kernel
 
 struct ConvTable {
   int nlev;
-  int total_units, total_vunits, total_sunits;
+  int total_units, total_vunits, total_sunits, total_vsunits;
   ConvLevel lev[kMaxConvLevels];
 };
 
@@ -492,6 +496,13 @@ __device__ __forceinline__ float4 lds128(unsigned addr) {
   return v;
 }
 
+template <int OFF>
+__device__ __forceinline__ unsigned long long lds64(unsigned addr) {
+  unsigned long long v;
+  asm("ld.shared.b64 %0, [%1+%2];" : "=l"(v) : "r"(addr), "n"(OFF));
+  return v;
+}
+
 template <int XT, int M0, int M1>
 __device__ __forceinline__ void conv_list_run(int b, int e, const int4* __restrict__ el, unsigned srow0, unsigned taps2,
                                               unsigned long long (&acc)[2][XT]) {
@@ -871,6 +882,158 @@ k_conv_virial_f2(const ConvTable* __restrict__ tabp, ConvSmemLayout sl) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
     if (lane == 0) g.wpart[(size_t)cu.local * 6 + k] = v;
+  }
+}
+
+// ---------------------------------------------------- virial, fp32, list-driven (see k_conv_f2l)
+// One block of kConvVW warps per SM with the level's interleaved moment taps in shared memory. A
+// list entry is one 4-tap chunk of one stencil row; after its taps the entry's three x-moment sums
+// go straight into six packed fp32 sums with the row's dy and the plane pair's dz as factors (seven
+// packed instructions per entry and plane pair), which are added to the fp64 sums once per input
+// plane: ~200 fp32 additions per sum and plane.
+template <int XT, int M>
+__device__ __forceinline__ void virial_entry(const int4 cur, int k, unsigned srow0, unsigned vtaps, float fy,
+                                             const unsigned long long (&qr)[2][XT], unsigned long long fz, unsigned long long fz2,
+                                             unsigned long long (&S)[6]) {
+  static_assert(XT == 16, "window of 20 floats");
+  const unsigned w = srow0 + (unsigned)cur.x;
+  float win[XT + 4];
+  {
+    const float4 t0 = lds128<0>(w), t1 = lds128<16>(w), t2 = lds128<32>(w), t3 = lds128<48>(w), t4 = lds128<64>(w);
+    win[0] = t0.x; win[1] = t0.y; win[2] = t0.z; win[3] = t0.w;
+    win[4] = t1.x; win[5] = t1.y; win[6] = t1.z; win[7] = t1.w;
+    win[8] = t2.x; win[9] = t2.y; win[10] = t2.z; win[11] = t2.w;
+    win[12] = t3.x; win[13] = t3.y; win[14] = t3.z; win[15] = t3.w;
+    win[16] = t4.x; win[17] = t4.y; win[18] = t4.z; win[19] = t4.w;
+  }
+  const unsigned tp = vtaps + (unsigned)(k == 0 ? cur.y : cur.z);
+  // moment m of tap t, as (row d, row d - 1): 8 bytes at 32 m + 8 t, loaded tap by tap (few live registers)
+  unsigned long long e0 = 0ull, e1 = 0ull, e2 = 0ull;
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    if ((M == 2 && t >= 2) || (M == 3 && t < 2)) continue;
+    unsigned long long c0 = 0ull, c1 = 0ull;
+#pragma unroll
+    for (int i = 0; i < XT; i += 2) {
+      ffma2_bcast(c0, win[i + t], qr[k][i]);
+      ffma2_bcast(c1, win[i + 1 + t], qr[k][i + 1]);
+    }
+    const unsigned long long ct = fadd2_pp(c0, c1);
+    if (t == 0) { ffma2_pp(e0, lds64<0>(tp), ct); ffma2_pp(e1, lds64<32>(tp), ct); ffma2_pp(e2, lds64<64>(tp), ct); }
+    if (t == 1) { ffma2_pp(e0, lds64<8>(tp), ct); ffma2_pp(e1, lds64<40>(tp), ct); ffma2_pp(e2, lds64<72>(tp), ct); }
+    if (t == 2) { ffma2_pp(e0, lds64<16>(tp), ct); ffma2_pp(e1, lds64<48>(tp), ct); ffma2_pp(e2, lds64<80>(tp), ct); }
+    if (t == 3) { ffma2_pp(e0, lds64<24>(tp), ct); ffma2_pp(e1, lds64<56>(tp), ct); ffma2_pp(e2, lds64<88>(tp), ct); }
+  }
+  // xx: x^2 moment; yy: dy^2 e0; zz: dz^2 e0; xy: dy e1; xz: dz e1; yz: dy dz e0
+  S[0] = fadd2_pp(S[0], e2);
+  ffma2_bcast(S[1], fy * fy, e0);
+  ffma2_pp(S[2], fz2, e0);
+  ffma2_bcast(S[3], fy, e1);
+  ffma2_pp(S[4], fz, e1);
+  unsigned long long ze = 0ull;
+  ffma2_pp(ze, fz, e0);
+  ffma2_bcast(S[5], fy, ze);
+}
+
+template <int XT, int M0, int M1>
+__device__ __forceinline__ void virial_list_run(int b, int e, const int4* __restrict__ el, unsigned srow0, unsigned vtaps,
+                                                const unsigned long long (&qr)[2][XT], const unsigned long long (&fz)[2],
+                                                const unsigned long long (&fz2)[2], unsigned long long (&S)[6]) {
+  if (b >= e) return;
+  int4 nxt = __ldg(el + b);
+#pragma unroll 1
+  for (int i = b; i < e; ++i) {
+    const int4 cur = nxt;
+    nxt = __ldg(el + i + 1);                          // (guard entry behind the end)
+    const float fy = __int_as_float(cur.w);
+    if (M0 != 0) virial_entry<XT, M0>(cur, 0, srow0, vtaps, fy, qr, fz[0], fz2[0], S);
+    if (M1 != 0) virial_entry<XT, M1>(cur, 1, srow0, vtaps, fy, qr, fz[1], fz2[1], S);
+  }
+}
+
+template <int XT>
+__global__ void __launch_bounds__(32 * kConvVW, 1)
+k_conv_virial_f2l(const ConvTable* __restrict__ tabp, int plane_bytes) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const ConvTable& tab = *tabp;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int l = 0;
+#pragma unroll 1
+  for (int k = 1; k < tab.nlev; ++k)
+    if ((int)blockIdx.x * kConvVW >= tab.lev[k].vsunit0) l = k;
+  const ConvLevel& g = tab.lev[l];
+  float4* staps = reinterpret_cast<float4*>(smem_raw);
+  float* planes = reinterpret_cast<float*>(staps + g.n_vtaps2q);
+  const float4* gt = reinterpret_cast<const float4*>(g.vtaps2);
+  for (int i = threadIdx.x; i < g.n_vtaps2q; i += 32 * kConvVW) staps[i] = __ldg(gt + i);
+  __syncthreads();
+  int r = (int)blockIdx.x * kConvVW + warp - g.vsunit0;
+  if (r >= g.tiles[0] * g.tiles[1] * g.tiles[2] * g.vslices) return;         // padding unit
+  const int local = r;
+  const int slice = r % g.vslices; r /= g.vslices;
+  const int X = (r % g.tiles[0]) * XT; r /= g.tiles[0];
+  const int Y = (r % g.tiles[1]) * 32;
+  const int Z = (r / g.tiles[1]) * 4;
+  float* plane = planes + (size_t)warp * (plane_bytes / 4);
+  const int Ry = g.R[1], Rz = g.R[2];
+  const int nrow = 32 + 2 * Ry;
+  const int WX = XT + 2 * g.X0 + 4;
+  const float* __restrict__ qpad = reinterpret_cast<const float*>(g.pad);
+  const float* __restrict__ Q = reinterpret_cast<const float*>(g.Q);
+  const int4* __restrict__ el = g.vlist;
+  unsigned srow0, vtaps;
+  asm volatile("mov.u32 %0, %1;" : "=r"(srow0) : "r"((unsigned)__cvta_generic_to_shared(plane + lane * g.pitch)));
+  asm volatile("mov.u32 %0, %1;" : "=r"(vtaps) : "r"((unsigned)__cvta_generic_to_shared(staps)));
+
+  unsigned long long qr[2][XT];                       // (Q of plane 2k, Q of plane 2k + 1)
+#pragma unroll
+  for (int k = 0; k < 2; ++k)
+#pragma unroll
+    for (int i = 0; i < XT; ++i) {
+      const int x = X + i, y = Y + lane, z = Z + 2 * k;
+      const bool in = x < g.M[0] && y < g.M[1];
+      const float lo = in && z < g.M[2] ? Q[((size_t)z * g.M[1] + y) * g.M[0] + x] : 0.f;
+      const float hi = in && z + 1 < g.M[2] ? Q[((size_t)(z + 1) * g.M[1] + y) * g.M[0] + x] : 0.f;
+      qr[k][i] = pack2(lo, hi);
+    }
+  double S[6] = {0, 0, 0, 0, 0, 0};
+
+  const int p0 = g.vb[slice], p1 = g.vb[slice + 1];
+#pragma unroll 1
+  for (int zr = p0; zr < p1; ++zr) {                  // input plane z = Z + zr, only dz >= 0
+    const int4 h0 = __ldg(reinterpret_cast<const int4*>(g.vhead + zr * (kConvListTypes + 1)));
+    const int4 h1 = __ldg(reinterpret_cast<const int4*>(g.vhead + zr * (kConvListTypes + 1)) + 1);
+    stage_plane<float>(g, qpad, plane, Z + zr + Rz, X, Y, nrow, WX, lane);   // commits and waits
+    // plane pair k takes the merged layer d = zr - 2k: dz = d for its lower plane, d - 1 for the upper
+    unsigned long long fz[2], fz2[2], Sp[6];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const float a = (float)(zr - 2 * k), b = (float)(zr - 2 * k - 1);
+      fz[k] = pack2(a, b);
+      fz2[k] = pack2(a * a, b * b);
+    }
+#pragma unroll
+    for (int k = 0; k < 6; ++k) Sp[k] = 0ull;
+    virial_list_run<XT, 1, 1>(h0.x, h0.y, el, srow0, vtaps, qr, fz, fz2, Sp);
+    virial_list_run<XT, 1, 0>(h0.y, h0.z, el, srow0, vtaps, qr, fz, fz2, Sp);
+    virial_list_run<XT, 0, 1>(h0.z, h0.w, el, srow0, vtaps, qr, fz, fz2, Sp);
+    virial_list_run<XT, 2, 0>(h0.w, h1.x, el, srow0, vtaps, qr, fz, fz2, Sp);
+    virial_list_run<XT, 3, 0>(h1.x, h1.y, el, srow0, vtaps, qr, fz, fz2, Sp);
+    virial_list_run<XT, 0, 2>(h1.y, h1.z, el, srow0, vtaps, qr, fz, fz2, Sp);
+    virial_list_run<XT, 0, 3>(h1.z, h1.w, el, srow0, vtaps, qr, fz, fz2, Sp);
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+      float lo, hi;
+      unpack2(Sp[k], lo, hi);
+      S[k] += (double)lo + (double)hi;
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 6; ++k) {
+    double v = S[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (lane == 0) g.wpart[(size_t)local * 6 + k] = v;
   }
 }
 

@@ -157,6 +157,9 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   g.rows2 = nullptr;
   g.elist = nullptr;
   g.ehead = nullptr;
+  g.vlist = nullptr;
+  g.vhead = nullptr;
+  g.n_vtaps2q = 0;
   g.taps2 = nullptr;
   g.vrows2 = nullptr;
   g.vtaps2 = nullptr;
@@ -253,6 +256,55 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
       }
     g.vrows2 = up_rows(vr2);
     g.vtaps2 = upload(p, tv2);
+    g.n_vtaps2q = (int)(tv2.size() / 4);
+    // entry lists of the list-driven virial kernel (as for the potential, see below): input plane zr
+    // (dz >= 0 only) feeds the plane pairs k = 0, 1 through the merged half-space layers zr and zr - 2
+    {
+      auto vstate = [&](int d, int j, int c, int& chunk) {     // 0 off, 1 full, 2 lower half, 3 upper half
+        if (d < 0 || d > Rz + 1) return 0;
+        const int4& r = vr2[(size_t)d * ny + j];
+        if (c < r.y || c > r.z) return 0;
+        chunk = r.x + (c - r.y);
+        const bool lo = 2 * c >= (r.w & 0xffff), hi = 2 * c + 1 <= (r.w >> 16);
+        return lo && hi ? 1 : lo ? 2 : hi ? 3 : 0;
+      };
+      std::vector<int4> el;
+      std::vector<int> eh;
+      const int cmax = (2 * g.X0) / 4 + 1;
+      for (int zr = 0; zr <= Rz + 3; ++zr) {
+        std::vector<int4> lists[kConvListTypes];
+        for (int j = 0; j < ny; ++j) {
+          const float fy = (float)(j - st.R[1]);
+          int fyb;
+          std::memcpy(&fyb, &fy, 4);
+          for (int c = 0; c <= cmax; ++c) {
+            int c0 = 0, c1 = 0;
+            const int s0 = vstate(zr, j, c, c0), s1 = vstate(zr - 2, j, c, c1);
+            const int4 e = make_int4((j * g.pitch + 4 * c) * 4, c0 * 96, c1 * 96, fyb);   // bytes
+            if (s0 == 1 && s1 == 1) { lists[0].push_back(e); continue; }
+            if (s0 == 1) lists[1].push_back(e);
+            if (s1 == 1) lists[2].push_back(e);
+            if (s0 == 2) lists[3].push_back(e);
+            if (s0 == 3) lists[4].push_back(e);
+            if (s1 == 2) lists[5].push_back(e);
+            if (s1 == 3) lists[6].push_back(e);
+          }
+        }
+        for (int t = 0; t < kConvListTypes; ++t) {
+          eh.push_back((int)el.size());
+          el.insert(el.end(), lists[t].begin(), lists[t].end());
+        }
+        eh.push_back((int)el.size());
+      }
+      el.push_back(make_int4(0, 0, 0, 0));
+      int4* eld = (int4*)dev_alloc(p, el.size() * sizeof(int4));
+      int* ehd = (int*)dev_alloc(p, eh.size() * sizeof(int));
+      if (cudaMemcpy(eld, el.data(), el.size() * sizeof(int4), cudaMemcpyHostToDevice) != cudaSuccess ||
+          cudaMemcpy(ehd, eh.data(), eh.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess)
+        throw CudaFail();
+      g.vlist = eld;
+      g.vhead = ehd;
+    }
     d.tab[3] = TapTable{const_cast<void*>(g.vtaps2), upload_desc(p, tv2d), (int)tv2.size()};
     g.rows2 = up_rows(r2);
     void* t2dev = upload(p, t2);
@@ -337,8 +389,12 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   g.vunit0 = p->conv.total_vunits;
   g.sunit0 = p->conv.total_sunits;                       // blocks of kConvSW units never straddle two levels
   p->conv.total_sunits += (tiles * g.nslices + kConvSW - 1) / kConvSW * kConvSW;
-  if (p->fp32)
+  g.vsunit0 = p->conv.total_vsunits;
+  p->conv.total_vsunits += (tiles * g.vslices + kConvVW - 1) / kConvVW * kConvVW;
+  if (p->fp32) {
     p->conv_tables_smem = std::max(p->conv_tables_smem, (size_t)g.n_taps2q * 16 + (size_t)g.n_rows2 * 16);
+    p->conv_vtables_smem = std::max(p->conv_vtables_smem, (size_t)g.n_vtaps2q * 16);
+  }
   p->conv.total_units += tiles * g.nslices;
   p->conv.total_vunits += tiles * g.vslices;
   if (g.nslices > 1) {

@@ -385,6 +385,17 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     };
     auto launch_virial = [&](cudaStream_t vs) {
       if constexpr (sizeof(T) == 4) {
+        // list-driven kernel, one block of kConvVW warps per SM with the tap tables in shared memory
+        // (not for small jobs: the table copy does not pay)
+        const size_t plane_b = (p->conv_smem + 15) / 16 * 16;
+        const size_t sm_l = p->conv_vtables_smem + kConvVW * plane_b;
+        static const bool no_l = std::getenv("MSM_CONV_NO_LISTS") != nullptr;
+        if (!no_l && sm_l <= 226 * 1024 && p->conv.total_vunits >= 2048) {
+          auto kern = k_conv_virial_f2l<XT>;
+          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_l);
+          MSM_LAUNCH(p, (kern<<<p->conv.total_vsunits / kConvVW, 32 * kConvVW, sm_l, vs>>>(p->d_conv, (int)plane_b)));
+          return;
+        }
         auto kern = k_conv_virial_f2<XT>;             // packed FMAs (FFMA2)
         size_t sm;
         const ConvSmemLayout sl = conv_layout(24, 2, sm);

@@ -78,6 +78,7 @@ struct msm_plan {
   size_t conv_smem = 0;
   int conv_ny_max = 0, conv_maxc = 0;   // largest row count 2 R_y + 1 and chunks per stencil row over the levels
   bool conv_lists = true;                            // fp32: every level has the entry lists of k_conv_f2l
+  size_t conv_vtables_smem = 0;                      // fp32: largest interleaved virial tap table of a level (bytes)
   size_t conv_tables_smem = 0;                       // fp32: largest row + tap table of a level (bytes)
   int conv_slices = 1, conv_vslices = 1;             // input-plane slices per output tile (potential, virial kernel)
   double* conv_wpart = nullptr;                      // total_vunits x 6
