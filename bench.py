@@ -182,10 +182,10 @@ def whole_job_value(world: int, particles: int, steps: int, ms_total: float) -> 
 
 def stored_traffic(kernel: str, workload: str, dtype: str):
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full`
-    capture) of the stage's kernel on this workload, from profiles/r2_dram_traffic.csv; None if
+    capture) of the stage's kernel on this workload, from profiles/r2b_dram_traffic.csv; None if
     that kernel / workload pair was not captured."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")) as f:
+        with open(os.path.join(ROOT, "profiles", "r2b_dram_traffic.csv")) as f:
             for line in f:
                 c = [x.strip() for x in line.split(",")]
                 if len(c) >= 4 and c[0] == kernel and c[1] == workload and c[2] == dtype:
@@ -317,7 +317,7 @@ def measure(w, prec, local, dev, steps, warmup, world, flush, sampler=None, full
         "roofline": {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"],
                      "peak": round(alu_peak, 2) if d["bound"] == "alu" else peaks["hbm_gbs"], "unit": d["unit"],
                      "frac": d["frac"], "traffic": stored_traffic(dom, w.name, dtype),
-                     "traffic_unit": "DRAM bytes per launch, ncu --set full (profiles/r2_dram_traffic.csv)",
+                     "traffic_unit": "DRAM bytes per launch, ncu --set full (profiles/r2b_dram_traffic.csv)",
                      "algorithmic": stage_work(dom, w, plan, esz, pairs)[1],
                      "algorithmic_unit": "flop per launch" if d["bound"] == "alu" else "bytes per launch",
                      "peak_source": ("derived: 148 SM x %d lanes x 2 x 1.965 GHz" % (128 if dtype == "f32" else 64))
