@@ -130,6 +130,34 @@ __device__ __forceinline__ void stage_plane(const ConvLevel& g, const T* __restr
   __syncwarp();
 }
 
+// The same plane through the bulk-copy engine (TMA, SASS UBLKCP): one cp.async.bulk per row of
+// WX * 4 bytes (a multiple of 16, like every row's source and destination address), completion
+// counted in bytes on the warp's own mbarrier. Two instructions per lane and plane instead of
+// ~18 LDGSTS with their index arithmetic. `phase` is the barrier's parity, flipped per plane.
+__device__ __forceinline__ void mbar_init(unsigned mbar) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(mbar) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void stage_plane_bulk(const ConvLevel& g, const float* __restrict__ qpad, unsigned plane_s,
+                                                 unsigned mbar, unsigned& phase, int pz, int X, int Y, int nrow, int WX,
+                                                 int lane) {
+  const float* src = qpad + ((size_t)pz * g.P[1] + Y) * g.P[0] + X;
+  __syncwarp();                                         // every lane is done reading the previous plane
+  if (lane == 0)
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(mbar), "r"((unsigned)(nrow * WX * 4)) : "memory");
+  __syncwarp();
+  for (int r = lane; r < nrow; r += 32)
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(plane_s + (unsigned)(r * g.pitch * 4)), "l"(src + (size_t)r * g.P[0]), "r"((unsigned)(WX * 4)), "r"(mbar)
+                 : "memory");
+  unsigned done;
+  do {
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(done) : "r"(mbar), "r"(phase) : "memory");
+  } while (!done);
+  phase ^= 1u;
+}
+
 struct ConvUnit {
   int lev, X, Y, Z, slice, local;
 };
@@ -573,6 +601,12 @@ k_conv_f2l(const ConvTable* __restrict__ tabp, int plane_bytes) {
   const int WX = XT + 2 * g.X0 + 4;
   const float* __restrict__ qpad = reinterpret_cast<const float*>(g.pad);
   const int4* __restrict__ el = g.elist;
+  // the warp's mbarrier (behind the planes) for the bulk copies of its input planes
+  const unsigned plane_s = (unsigned)__cvta_generic_to_shared(plane);
+  const unsigned mbar = (unsigned)__cvta_generic_to_shared(planes + (size_t)kConvSW * (plane_bytes / 4)) + 8u * warp;
+  unsigned phase = 0;
+  if (lane == 0) mbar_init(mbar);
+  __syncwarp();
   // (opaque moves: the compiler would otherwise recompute the lane's row address in every iteration)
   unsigned srow0, taps2;
   asm volatile("mov.u32 %0, %1;" : "=r"(srow0) : "r"((unsigned)__cvta_generic_to_shared(plane + lane * g.pitch)));
@@ -589,7 +623,7 @@ k_conv_f2l(const ConvTable* __restrict__ tabp, int plane_bytes) {
   for (int pz = p0; pz < p1; ++pz) {                  // input plane z = Z + pz - Rz: list set d0 = pz - Rz
     const int4 h0 = __ldg(reinterpret_cast<const int4*>(g.ehead + pz * (kConvListTypes + 1)));
     const int4 h1 = __ldg(reinterpret_cast<const int4*>(g.ehead + pz * (kConvListTypes + 1)) + 1);
-    stage_plane<float>(g, qpad, plane, Z + pz, X, Y, nrow, WX, lane);     // commits and waits
+    stage_plane_bulk(g, qpad, plane_s, mbar, phase, Z + pz, X, Y, nrow, WX, lane);
     conv_list_run<XT, 1, 1>(h0.x, h0.y, el, srow0, taps2, acc);
     conv_list_run<XT, 1, 0>(h0.y, h0.z, el, srow0, taps2, acc);
     conv_list_run<XT, 0, 1>(h0.z, h0.w, el, srow0, taps2, acc);
@@ -981,6 +1015,11 @@ k_conv_virial_f2l(const ConvTable* __restrict__ tabp, int plane_bytes) {
   const float* __restrict__ qpad = reinterpret_cast<const float*>(g.pad);
   const float* __restrict__ Q = reinterpret_cast<const float*>(g.Q);
   const int4* __restrict__ el = g.vlist;
+  const unsigned plane_s = (unsigned)__cvta_generic_to_shared(plane);
+  const unsigned mbar = (unsigned)__cvta_generic_to_shared(planes + (size_t)kConvVW * (plane_bytes / 4)) + 8u * warp;
+  unsigned phase = 0;
+  if (lane == 0) mbar_init(mbar);
+  __syncwarp();
   unsigned srow0, vtaps;
   asm volatile("mov.u32 %0, %1;" : "=r"(srow0) : "r"((unsigned)__cvta_generic_to_shared(plane + lane * g.pitch)));
   asm volatile("mov.u32 %0, %1;" : "=r"(vtaps) : "r"((unsigned)__cvta_generic_to_shared(staps)));
@@ -1003,7 +1042,7 @@ k_conv_virial_f2l(const ConvTable* __restrict__ tabp, int plane_bytes) {
   for (int zr = p0; zr < p1; ++zr) {                  // input plane z = Z + zr, only dz >= 0
     const int4 h0 = __ldg(reinterpret_cast<const int4*>(g.vhead + zr * (kConvListTypes + 1)));
     const int4 h1 = __ldg(reinterpret_cast<const int4*>(g.vhead + zr * (kConvListTypes + 1)) + 1);
-    stage_plane<float>(g, qpad, plane, Z + zr + Rz, X, Y, nrow, WX, lane);   // commits and waits
+    stage_plane_bulk(g, qpad, plane_s, mbar, phase, Z + zr + Rz, X, Y, nrow, WX, lane);
     // plane pair k takes the merged layer d = zr - 2k: dz = d for its lower plane, d - 1 for the upper
     unsigned long long fz[2], fz2[2], Sp[6];
 #pragma unroll
