@@ -573,6 +573,42 @@ def test_batched_small_systems_against_their_own_oracle_runs():
     assert U1 == U[5] and np.array_equal(W1, W[5]) and torch.equal(F1, F0[5, :n[5]])
 
 
+def test_dynamic_cell_on_the_large_grid_kernels():
+    """msm_plan_set_box on a plan large enough for the list-driven fp32 convolution kernels (128^3
+    finest grid: their entry lists are built from the reserved table STRUCTURE, the tap VALUES are
+    rebuilt on the device): every output and grid at an anisotropically deformed box against a
+    fresh oracle with the same grid counts."""
+    import torch
+    from oracle import Oracle
+    from paper_2510_05961_b200 import msm
+    from paper_2510_05961_b200.workloads import Workload
+    rng = np.random.default_rng(4242)
+    n, box, periodic = 60001, (128.0, 128.0, 128.0), (1, 1, 1)
+    h, a, p, levels = 1.0, 4.0, 4, 4
+    frac = rng.random((n, 3))
+    q = rng.uniform(-1, 1, n); q -= q.mean()
+    dev = torch.device("cuda", 0)
+    plan = msm.Plan(box, periodic, h, a, p, levels, "fp32", max_particles=n, reserve=0.05)
+    assert tuple(plan.grid_dims(1)) == (128, 128, 128)
+    for name, scale in (("box0", (1.0, 1.0, 1.0)), ("box1", (0.97, 1.02, 1.04))):
+        b = tuple(bb * s for bb, s in zip(box, scale))
+        plan.set_box(b)
+        w = Workload("dyn128", frac * np.array(b), q, b, periodic, h=h, a=a, p=p, levels=levels).as_precision("fp32")
+        pos = torch.tensor(w.positions, dtype=torch.float32, device=dev)
+        qq = torch.tensor(w.charges, dtype=torch.float32, device=dev)
+        F = torch.zeros((n, 3), dtype=torch.float32, device=dev); V = torch.zeros(n, dtype=torch.float32, device=dev)
+        U, W = plan.evaluate(pos, qq, F, V)
+        gpu = {"energy": U, "virial": W, "forces": F.cpu().numpy().astype(np.float64),
+               "potentials": V.cpu().numpy().astype(np.float64), "plan": plan}
+        # a target spacing that reproduces 128 points on every axis of the deformed box
+        hh = float(np.exp(np.mean(np.log([b[ax] / 128 for ax in range(3)]))))
+        orc = Oracle(b, periodic, hh, a, p, levels)
+        assert [orc.level_info(1)["M"][ax] for ax in range(3)] == [128, 128, 128]
+        ref = orc.evaluate(w.positions, w.charges); ref["oracle"] = orc
+        _log(f"dyn128_fp32_{name}", compare(w, gpu, ref, "fp32"))
+    plan.close()
+
+
 @pytest.mark.parametrize("periodic,box,precision", [((1, 1, 1), (24.0, 26.0, 22.0), "fp64"),
                                                     ((1, 1, 0), (26.0, 24.0, 9.0), "fp64"),
                                                     ((1, 1, 1), (24.0, 26.0, 22.0), "fp32")])
