@@ -529,6 +529,7 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
     long long ntiles = 1;
     for (int ax = 0; ax < 3; ++ax) {
       p->at.T[ax] = prm->p - 1 <= tdim[ax] ? tdim[ax] : 8;   // power of two >= p - 1: divides periodic M, <= 2 tiles per node and axis
+      p->at.tshift[ax] = p->at.T[ax] == 8 ? 3 : 2;
       p->at.D[ax] = p->at.T[ax] + prm->p - 1;
       p->at.nt[ax] = (bg.ng[ax] + p->at.T[ax] - 1) / p->at.T[ax];
       ntiles *= p->at.nt[ax];

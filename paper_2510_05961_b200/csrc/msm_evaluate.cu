@@ -220,12 +220,11 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     const int ntiles = p->at.nt[0] * p->at.nt[1] * p->at.nt[2] * p->at.split;
     MSM_LAUNCH(p, (k_anterp_tiles<T, P><<<ntiles, 32, sm, st>>>(gg, p->at, tab, p->gstart, (const V4*)p->grec,
                                                                  p->gcell_sorted, (T*)p->anterp_scratch)));
+    const dim3 cgrid((H.lev[1].M[0] + 31) / 32, (H.lev[1].M[1] + 3) / 4, H.lev[1].M[2]), cblock(32, 4);
     if (p->at.split > 1)
-      MSM_LAUNCH(p, (k_anterp_combine<T, P, true><<<blocks_for(H.lev[1].points(), 128), 128, 0, st>>>(
-                        gg, p->at, (const T*)p->anterp_scratch, (T*)p->lev[1].Q)));
+      MSM_LAUNCH(p, (k_anterp_combine<T, P, true><<<cgrid, cblock, 0, st>>>(gg, p->at, (const T*)p->anterp_scratch, (T*)p->lev[1].Q)));
     else
-      MSM_LAUNCH(p, (k_anterp_combine<T, P, false><<<blocks_for(H.lev[1].points(), 128), 128, 0, st>>>(
-                        gg, p->at, (const T*)p->anterp_scratch, (T*)p->lev[1].Q)));
+      MSM_LAUNCH(p, (k_anterp_combine<T, P, false><<<cgrid, cblock, 0, st>>>(gg, p->at, (const T*)p->anterp_scratch, (T*)p->lev[1].Q)));
   } else {
     MSM_LAUNCH(p, (k_anterpolate<T, P><<<blocks_for(H.lev[1].points(), 128), 128, 0, st>>>(
                       gg, tab, p->gstart, (const V4*)p->grec, (T*)p->lev[1].Q)));
