@@ -94,7 +94,7 @@ template <> struct PairStage<float> {
   }
 };
 template <> struct PairStage<double> {
-  static constexpr int kCap = 256;
+  static constexpr int kCap = 192;            // 12 KB per warp: 8 blocks of 2 warps per SM
   __align__(16) float f[kCap * 4];            // fp32 copy for the scan (q slots unused)
   double4 d[kCap];                            // full precision for the drain
   unsigned char list[kCap / kPairPhases * 32];   // hit r of lane l at [r * 32 + l]; a lane scans kCap / kPairPhases candidates
