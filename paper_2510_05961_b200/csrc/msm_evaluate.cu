@@ -226,7 +226,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     else
       MSM_LAUNCH(p, (k_anterp_combine<T, P, false><<<cgrid, cblock, 0, st>>>(gg, p->at, (const T*)p->anterp_scratch, (T*)p->lev[1].Q)));
   } else {
-    MSM_LAUNCH(p, (k_anterpolate<T, P><<<blocks_for(H.lev[1].points(), 128), 128, 0, st>>>(
+    MSM_LAUNCH(p, (k_anterpolate<T, P><<<blocks_for(H.lev[1].points() * 16, 128), 128, 0, st>>>(
                       gg, tab, p->gstart, (const V4*)p->grec, (T*)p->lev[1].Q)));
   }
   mark();

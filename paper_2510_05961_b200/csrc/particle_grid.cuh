@@ -12,49 +12,54 @@ struct GridGeom {
   int periodic[3];
 };
 
-// One thread per level-1 grid point m: q~_m = sum_i q_i phi_m(r_i), gathered from the particles of
-// the p^3 grid cells whose support contains m, in a fixed order (cell by cell, particles inside a
-// cell in ascending original index) -> no atomics, bit-reproducible.
+// Sixteen lanes per level-1 grid point m: q~_m = sum_i q_i phi_m(r_i), gathered from the particles
+// of the p^3 grid cells whose support contains m. Lane s of a node's group takes the cell rows
+// (jz, jy) with index s (mod 16) and walks their p cells along x (ascending cell index, particles
+// inside a cell in ascending original index); the 16 partial sums are added in a fixed shuffle
+// tree -> no atomics, bit-reproducible. (One thread per node walked p^3 cells one after the other,
+// two dependent global loads each: 43 us for 3000 particles on a 16^3 grid.)
 template <typename T, int P>
 __global__ void __launch_bounds__(128)
 k_anterpolate(GridGeom g, SplineTab<T, P> tab, const int* __restrict__ gstart,
               const typename Vec4<T>::type* __restrict__ grec, T* __restrict__ Q) {
   constexpr int HP = P / 2;
   const int total = g.M[0] * g.M[1] * g.M[2];
-  const int m = blockIdx.x * blockDim.x + threadIdx.x;
-  if (m >= total) return;
-  const int mx = m % g.M[0], my = (m / g.M[0]) % g.M[1], mz = m / (g.M[0] * g.M[1]);
+  const int sub = threadIdx.x & 15;
+  const int m = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 4);
+  const bool live = m < total;                       // (whole groups: every lane reaches the shuffles)
+  const int mc = live ? m : 0;
+  const int mx = mc % g.M[0], my = (mc / g.M[0]) % g.M[1], mz = mc / (g.M[0] * g.M[1]);
   const int nx = mx + g.lo[0], ny = my + g.lo[1], nz = mz + g.lo[2];   // node indices
   T acc = 0;
   // node n = i0 + j, j = -HP+1..HP  ->  cell i0 = n - j, spline row j + HP - 1
 #pragma unroll 1
-  for (int jz = -HP + 1; jz <= HP; ++jz) {
-    int cz = nz - jz;
+  for (int row = sub; row < P * P; row += 16) {
+    const int jz = row / P - HP + 1, jy = row % P - HP + 1;
+    int cz = nz - jz, cy = ny - jy;
     if (g.periodic[2]) cz = imod(cz, g.ng[2]);
     else if (cz < 0 || cz >= g.ng[2]) continue;
-#pragma unroll 1
-    for (int jy = -HP + 1; jy <= HP; ++jy) {
-      int cy = ny - jy;
-      if (g.periodic[1]) cy = imod(cy, g.ng[1]);
-      else if (cy < 0 || cy >= g.ng[1]) continue;
-      const int rowbase = (cz * g.ng[1] + cy) * g.ng[0];
+    if (g.periodic[1]) cy = imod(cy, g.ng[1]);
+    else if (cy < 0 || cy >= g.ng[1]) continue;
+    if (!live) continue;
+    const int rowbase = (cz * g.ng[1] + cy) * g.ng[0];
 #pragma unroll
-      for (int jx = HP; jx >= -HP + 1; --jx) {       // ascending cell index
-        int cx = nx - jx;
-        if (g.periodic[0]) cx = imod(cx, g.ng[0]);
-        else if (cx < 0 || cx >= g.ng[0]) continue;
-        const int s = gstart[rowbase + cx], e = gstart[rowbase + cx + 1];
-        for (int k = s; k < e; ++k) {
-          const auto r = ldg4(grec + k);
-          const T wx = spline_weight_row<T, P>(tab, jx + HP - 1, r.x);
-          const T wy = spline_weight_row<T, P>(tab, jy + HP - 1, r.y);
-          const T wz = spline_weight_row<T, P>(tab, jz + HP - 1, r.z);
-          acc = fma(r.w, wx * wy * wz, acc);
-        }
+    for (int jx = HP; jx >= -HP + 1; --jx) {         // ascending cell index
+      int cx = nx - jx;
+      if (g.periodic[0]) cx = imod(cx, g.ng[0]);
+      else if (cx < 0 || cx >= g.ng[0]) continue;
+      const int s = gstart[rowbase + cx], e = gstart[rowbase + cx + 1];
+      for (int k = s; k < e; ++k) {
+        const auto r = ldg4(grec + k);
+        const T wx = spline_weight_row<T, P>(tab, jx + HP - 1, r.x);
+        const T wy = spline_weight_row<T, P>(tab, jy + HP - 1, r.y);
+        const T wz = spline_weight_row<T, P>(tab, jz + HP - 1, r.z);
+        acc = fma(r.w, wx * wy * wz, acc);
       }
     }
   }
-  Q[m] = acc;
+#pragma unroll
+  for (int o = 8; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if (live && sub == 0) Q[m] = acc;
 }
 
 // One thread per particle (grid-cell order): V_i^lr = sum_m e_m phi_m(r_i), grad = sum_m e_m grad
