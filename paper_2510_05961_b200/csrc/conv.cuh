@@ -30,6 +30,7 @@ namespace msm {
 
 constexpr int kMaxConvLevels = 16;
 constexpr int kMaxConvSlices = 71;
+constexpr int kMaxRowSlices = 6;     // small jobs: units per plane slice (by stencil rows)
 
 struct ConvLevel {
   int M[3];        // output grid dims
@@ -41,6 +42,7 @@ struct ConvLevel {
   int ny;          // 2 R[1] + 1
   int nslices;     // potential kernel: slices of the 2 R[2] + ZT input planes
   int vslices;     // virial kernel: slices of the R[2] + ZT input planes with dz >= 0
+  int ysl, vysl;   // small jobs: each plane slice is dealt to this many units by stencil rows (dy); nslices / vslices count them all
   unsigned char pb[kMaxConvSlices + 1];   // slice s covers input planes [pb[s], pb[s+1]) (balanced by taps)
   unsigned char vb[kMaxConvSlices + 1];
   int unit0, vunit0;          // first unit of this level in the potential / virial launch
@@ -162,6 +164,21 @@ struct ConvUnit {
   int lev, X, Y, Z, slice, local;
 };
 
+// input planes [p0, p1) and stencil rows [j0, j1) of slice `slice` (plane slices fastest)
+struct SliceRange { int p0, p1, j0, j1; };
+template <bool VIRIAL>
+__device__ __forceinline__ SliceRange slice_range(const ConvLevel& g, int slice) {
+  const int ysl = VIRIAL ? g.vysl : g.ysl;
+  const int ps = (VIRIAL ? g.vslices : g.nslices) / ysl;
+  const int s = slice % ps, y = slice / ps;
+  SliceRange r;
+  r.p0 = VIRIAL ? g.vb[s] : g.pb[s];
+  r.p1 = VIRIAL ? g.vb[s + 1] : g.pb[s + 1];
+  r.j0 = y * g.ny / ysl;
+  r.j1 = (y + 1) * g.ny / ysl;
+  return r;
+}
+
 template <bool VIRIAL, int XT, int ZT>
 __device__ __forceinline__ ConvUnit decode_unit(const ConvTable& tab, int u) {
   ConvUnit cu;
@@ -247,7 +264,8 @@ k_conv(const ConvTable* __restrict__ tabp, ConvSmemLayout sl) {
 #pragma unroll
     for (int i = 0; i < XT; ++i) acc[k][i] = 0;
 
-  const int p0 = g.pb[cu.slice], p1 = g.pb[cu.slice + 1];
+  const SliceRange sr = slice_range<false>(g, cu.slice);
+  const int p0 = sr.p0, p1 = sr.p1;
   for (int pz = p0; pz < p1; ++pz) {
     const int zr = pz - Rz;              // input plane z = Z + zr
     stage_rows<ZT>(srows, rows, ny, lane, [&](int k) {
@@ -255,12 +273,12 @@ k_conv(const ConvTable* __restrict__ tabp, ConvSmemLayout sl) {
       return dz >= -Rz && dz <= Rz ? (dz + Rz) * ny : -1;
     });
     stage_plane<T>(g, qpad, plane, Z + pz, X, Y, nrow, WX, lane);     // commits and waits (the row entries too)
-    issue_row_taps<T, ZT, 4>(srows, ny, 0, staps, stap, sl.tapk, lane);
-    for (int dy = -Ry; dy <= Ry; ++dy) {
+    issue_row_taps<T, ZT, 4>(srows, ny, sr.j0, staps, stap + (sr.j0 & 1) * sl.tapbuf, sl.tapk, lane);
+    for (int dy = sr.j0 - Ry; dy < sr.j1 - Ry; ++dy) {
       const int j = dy + Ry;
       cp_async_wait<0>();                                  // this row's taps have landed
       __syncwarp();
-      if (dy < Ry) issue_row_taps<T, ZT, 4>(srows, ny, j + 1, staps, stap + ((j + 1) & 1) * sl.tapbuf, sl.tapk, lane);
+      if (j + 1 < sr.j1) issue_row_taps<T, ZT, 4>(srows, ny, j + 1, staps, stap + ((j + 1) & 1) * sl.tapbuf, sl.tapk, lane);
       const T* tapb = stap + (j & 1) * sl.tapbuf;
       int4 re[ZT];
       int cl = 1 << 30, ch = -1;
@@ -362,7 +380,8 @@ __device__ __forceinline__ void conv_f2_unit(const ConvLevel& g, const ConvUnit&
 #pragma unroll
     for (int i = 0; i < XT; ++i) acc[k][i] = 0ull;
 
-  const int p0 = g.pb[cu.slice], p1 = g.pb[cu.slice + 1];
+  const SliceRange sr = slice_range<false>(g, cu.slice);
+  const int p0 = sr.p0, p1 = sr.p1;
   for (int pz = p0; pz < p1; ++pz) {
     const int zr = pz - Rz;                           // input plane z = Z + zr
     if (!SM)
@@ -371,14 +390,16 @@ __device__ __forceinline__ void conv_f2_unit(const ConvLevel& g, const ConvUnit&
         return d >= -Rz && d <= Rz + 1 ? (d + Rz) * ny : -1;
       });
     stage_plane<float>(g, qpad, plane, Z + pz, X, Y, nrow, WX, lane);     // commits and waits
-    if (!SM) issue_row_taps<float, ZP, 8>(wrows, ny, 0, reinterpret_cast<const float*>(taps2), stap, sl.tapk, lane);
-    for (int dy = -Ry; dy <= Ry; ++dy) {
+    if (!SM)
+      issue_row_taps<float, ZP, 8>(wrows, ny, sr.j0, reinterpret_cast<const float*>(taps2), stap + (sr.j0 & 1) * sl.tapbuf, sl.tapk,
+                                   lane);
+    for (int dy = sr.j0 - Ry; dy < sr.j1 - Ry; ++dy) {
       const int jr = dy + Ry;
       const float* tapb = nullptr;
       if (!SM) {
         cp_async_wait<0>();                           // this row's taps have landed
         __syncwarp();
-        if (dy < Ry)
+        if (jr + 1 < sr.j1)
           issue_row_taps<float, ZP, 8>(wrows, ny, jr + 1, reinterpret_cast<const float*>(taps2),
                                        stap + ((jr + 1) & 1) * sl.tapbuf, sl.tapk, lane);
         tapb = stap + (jr & 1) * sl.tapbuf;
@@ -697,7 +718,8 @@ k_conv_virial(const ConvTable* __restrict__ tabp, ConvSmemLayout sl) {
   double S[6] = {0, 0, 0, 0, 0, 0};
 
   // only dz = zr - k >= 0: input planes zr in [0, ZT - 1 + Rz], padded index pz = zr + Rz
-  const int p0 = g.vb[cu.slice], p1 = g.vb[cu.slice + 1];
+  const SliceRange sr = slice_range<true>(g, cu.slice);
+  const int p0 = sr.p0, p1 = sr.p1;
   for (int pp = p0; pp < p1; ++pp) {
     const int zr = pp;
     stage_rows<ZT>(srows, rows, ny, lane, [&](int k) {
@@ -705,12 +727,12 @@ k_conv_virial(const ConvTable* __restrict__ tabp, ConvSmemLayout sl) {
       return dz >= 0 && dz <= Rz ? dz * ny : -1;
     });
     stage_plane<T>(g, qpad, plane, Z + zr + Rz, X, Y, nrow, WX, lane);   // commits and waits (the row entries too)
-    issue_row_taps<T, ZT, 12>(srows, ny, 0, vtaps, stap, sl.tapk, lane);
-    for (int dy = -Ry; dy <= Ry; ++dy) {
+    issue_row_taps<T, ZT, 12>(srows, ny, sr.j0, vtaps, stap + (sr.j0 & 1) * sl.tapbuf, sl.tapk, lane);
+    for (int dy = sr.j0 - Ry; dy < sr.j1 - Ry; ++dy) {
       const int j = dy + Ry;
       cp_async_wait<0>();                                  // this row's taps have landed
       __syncwarp();
-      if (dy < Ry) issue_row_taps<T, ZT, 12>(srows, ny, j + 1, vtaps, stap + ((j + 1) & 1) * sl.tapbuf, sl.tapk, lane);
+      if (j + 1 < sr.j1) issue_row_taps<T, ZT, 12>(srows, ny, j + 1, vtaps, stap + ((j + 1) & 1) * sl.tapbuf, sl.tapk, lane);
       const T* tapb = stap + (j & 1) * sl.tapbuf;
       int4 re[ZT];
       int cl = 1 << 30, ch = -1;
@@ -828,7 +850,8 @@ k_conv_virial_f2(const ConvTable* __restrict__ tabp, ConvSmemLayout sl) {
     }
   double S[6] = {0, 0, 0, 0, 0, 0};
 
-  const int p0 = g.vb[cu.slice], p1 = g.vb[cu.slice + 1];
+  const SliceRange sr = slice_range<true>(g, cu.slice);
+  const int p0 = sr.p0, p1 = sr.p1;
   for (int zr = p0; zr < p1; ++zr) {                  // input plane z = Z + zr, only dz >= 0
     // row entries of the merged layers to shared memory with the plane; the taps of stencil row
     // dy + 1 are copied (cp.async) while row dy is computed: no FMA waits for a table load
@@ -837,12 +860,12 @@ k_conv_virial_f2(const ConvTable* __restrict__ tabp, ConvSmemLayout sl) {
       return d >= 0 && d <= Rz + 1 ? d * ny : -1;
     });
     stage_plane<float>(g, qpad, plane, Z + zr + Rz, X, Y, nrow, WX, lane);   // commits and waits
-    issue_row_taps<float, ZP, 24>(srows, ny, 0, vtaps, stap, sl.tapk, lane);
-    for (int dy = -Ry; dy <= Ry; ++dy) {
+    issue_row_taps<float, ZP, 24>(srows, ny, sr.j0, vtaps, stap + (sr.j0 & 1) * sl.tapbuf, sl.tapk, lane);
+    for (int dy = sr.j0 - Ry; dy < sr.j1 - Ry; ++dy) {
       const int jr = dy + Ry;
       cp_async_wait<0>();                             // this row's taps have landed
       __syncwarp();
-      if (dy < Ry) issue_row_taps<float, ZP, 24>(srows, ny, jr + 1, vtaps, stap + ((jr + 1) & 1) * sl.tapbuf, sl.tapk, lane);
+      if (jr + 1 < sr.j1) issue_row_taps<float, ZP, 24>(srows, ny, jr + 1, vtaps, stap + ((jr + 1) & 1) * sl.tapbuf, sl.tapk, lane);
       const float* tapb = stap + (jr & 1) * sl.tapbuf;
       int4 re[ZP];
       int cl = 1 << 30, ch = -1;

@@ -389,7 +389,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
         const size_t plane_b = (p->conv_smem + 15) / 16 * 16;
         const size_t sm_l = p->conv_vtables_smem + kConvVW * plane_b + kConvVW * 8;   // + one mbarrier per warp
         static const bool no_l = std::getenv("MSM_CONV_NO_LISTS") != nullptr;
-        if (!no_l && sm_l <= 226 * 1024 && p->conv.total_vunits >= 2048) {
+        if (!no_l && !p->conv_rowsliced && sm_l <= 226 * 1024 && p->conv.total_vunits >= 2048) {
           auto kern = k_conv_virial_f2l<XT>;
           cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_l);
           MSM_LAUNCH(p, (kern<<<p->conv.total_vsunits / kConvVW, 32 * kConvVW, sm_l, vs>>>(p->d_conv, (int)plane_b)));
@@ -425,7 +425,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
         const size_t sm_s = p->conv_tables_smem + kConvSW * plane_b;
         static const bool no_s = std::getenv("MSM_CONV_GLOBAL_TAPS") != nullptr;
         static const bool no_l = std::getenv("MSM_CONV_NO_LISTS") != nullptr;
-        if (!no_s && sm_s <= 110 * 1024 && p->conv.total_units >= 4096) {   // small jobs: the table copy does not pay
+        if (!no_s && !p->conv_rowsliced && sm_s <= 110 * 1024 && p->conv.total_units >= 4096) {   // small jobs: the table copy does not pay
           // list-driven inner loops when every level has its entry lists (msm_create.cu)
           auto kern = p->conv_lists && !no_l ? k_conv_f2l<XT> : k_conv_f2s<XT>;
           const size_t sm_k = sm_s + kConvSW * 8;       // + one mbarrier per warp (k_conv_f2l)

@@ -77,6 +77,7 @@ struct msm_plan {
   msm::ConvTable* d_conv = nullptr;
   size_t conv_smem = 0;
   int conv_ny_max = 0, conv_maxc = 0;   // largest row count 2 R_y + 1 and chunks per stencil row over the levels
+  bool conv_rowsliced = false;                       // some level splits its plane slices by stencil rows (small jobs: no list kernels)
   bool conv_lists = true;                            // fp32: every level has the entry lists of k_conv_f2l
   size_t conv_vtables_smem = 0;                      // fp32: largest interleaved virial tap table of a level (bytes)
   size_t conv_tables_smem = 0;                       // fp32: largest row + tap table of a level (bytes)
