@@ -190,7 +190,8 @@ void msm_plan_destroy(msm_plan_t *plan);
  *   d_forces / d_potentials  device, same layout, may be NULL
  *   h_energy      host, batch doubles; h_virial host, batch x 6 doubles; either may be NULL. With
  *                 both NULL the call is stream-ordered and does not synchronise.
- * The graph is rebuilt when any argument changes. Results equal msm_evaluate's for each system. */
+ * The graph is rebuilt when any argument changes. Results equal msm_evaluate's for each system up
+ * to rounding (a plan inside a batch sums the anterpolation of a small grid in another order). */
 msm_status_t msm_batch_create(const msm_params_t *params, int batch, msm_batch_t **batch_out);
 msm_status_t msm_evaluate_batch(msm_batch_t *batch, const int *h_n, const void *d_positions,
                                 const void *d_charges, void *d_forces, void *d_potentials,

@@ -381,18 +381,18 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
       wv[pz] += 0.3;
     }
   const int tiles = g.tiles[0] * g.tiles[1] * g.tiles[2];
-  // units per tile: slices of the input planes; a level with fewer plane-slice units than SMs (16^3
-  // grids: 96) deals each plane slice to several units by stencil rows, at least three rows each.
+  // units per tile: slices of the input planes; a PLAN with fewer plane-slice units than SMs over all
+  // its levels (16^3 grids: 96) deals each plane slice to several units by stencil rows, at least three rows each.
   // Measured: N = 3000 (16^3) 0.147 -> 0.135 ms per evaluation; applied to 32^3 grids (432 units)
   // it made config 2 slower (0.26 -> 0.32 ms: the units crowd out the pair kernel beside them)
   const int pslices = std::max(1, std::min({p->conv_slices, nplanes, kMaxConvSlices}));
   const int pvslices = std::max(1, std::min({p->conv_vslices, vplanes, kMaxConvSlices}));
   const int ymax = std::max(1, std::min(kMaxRowSlices, ny / 3));
   auto row_slices = [&](int units) {
-    return units < p->sm_count ? std::max(1, std::min(ymax, (2 * p->sm_count + units - 1) / units)) : 1;
+    return units < p->sm_count && !p->in_batch ? std::max(1, std::min(ymax, (2 * p->sm_count + units - 1) / units)) : 1;
   };
-  g.ysl = row_slices(tiles * pslices);
-  g.vysl = row_slices(tiles * pvslices);
+  g.ysl = row_slices((int)std::min<long long>(p->conv_tiles_total * pslices, 1 << 30));
+  g.vysl = row_slices((int)std::min<long long>(p->conv_tiles_total * pvslices, 1 << 30));
   if (g.ysl > 1 || g.vysl > 1) p->conv_rowsliced = true;
   g.nslices = pslices * g.ysl;
   g.vslices = pvslices * g.vysl;
@@ -457,6 +457,7 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
     long long tiles = 0;
     for (int l = 1; l < p->n_t; ++l)
       tiles += (long long)((H.lev[l].M[0] + XTc - 1) / XTc) * ((H.lev[l].M[1] + 31) / 32) * ((H.lev[l].M[2] + 3) / 4);
+    p->conv_tiles_total = tiles;
     const long long slots = (long long)p->sm_count * 16;
     if (p->fp32) {
       auto per_tile = [&](long long units) {
@@ -622,7 +623,8 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
       cudaEventCreateWithFlags(&p->join_ev, cudaEventDisableTiming) != cudaSuccess ||
       cudaStreamCreateWithPriority(&p->vstream, cudaStreamNonBlocking, prio_hi) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->fork2_ev, cudaEventDisableTiming) != cudaSuccess ||
-      cudaEventCreateWithFlags(&p->join2_ev, cudaEventDisableTiming) != cudaSuccess)
+      cudaEventCreateWithFlags(&p->join2_ev, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->top_ev, cudaEventDisableTiming) != cudaSuccess)
     return MSM_ERR_CUDA;
   if (const char* e = std::getenv("MSM_NO_OVERLAP")) p->overlap = std::atoi(e) == 0;
   if (const char* e = std::getenv("MSM_GRID_STREAM_MIN")) p->stream_min_points = p->prolong_stream_min_points = p->filter_stream_min_points = std::atoll(e);
@@ -772,6 +774,7 @@ void msm_plan_destroy(msm_plan_t* p) {
   if (p->vstream) cudaStreamDestroy(p->vstream);
   if (p->fork2_ev) cudaEventDestroy(p->fork2_ev);
   if (p->join2_ev) cudaEventDestroy(p->join2_ev);
+  if (p->top_ev) cudaEventDestroy(p->top_ev);
   if (p->fork_ev) cudaEventDestroy(p->fork_ev);
   if (p->join_ev) cudaEventDestroy(p->join_ev);
   if (p->gexec) cudaGraphExecDestroy(p->gexec);
@@ -790,12 +793,23 @@ msm_status_t msm_plan_create(const msm_params_t* params, msm_plan_t** plan_out) 
 }
 
 msm_status_t msm_plan_create_dynamic(const msm_params_t* params, double reserve, msm_plan_t** plan_out) {
+  return msm::plan_create_opts(params, reserve, false, plan_out);
+}
+
+}  // extern "C"
+
+// (internal) in_batch: the plan is one of many that run side by side in one graph (msm_batch_create):
+// no extra units or streams for latency's sake, the batch fills the GPU
+msm_status_t msm::plan_create_opts(const msm_params_t* params, double reserve, bool in_batch, msm_plan_t** plan_out) {
   if (!plan_out) return MSM_ERR_INVALID_ARG;
   *plan_out = nullptr;
   if (!params || !(reserve >= 0.0) || reserve > 0.5) return MSM_ERR_INVALID_ARG;
   msm_plan* p = new (std::nothrow) msm_plan();
   if (!p) return MSM_ERR_NOMEM;
   p->reserve = reserve;
+  p->in_batch = in_batch;
+  p->top_beside = !in_batch;
+  if (const char* e = std::getenv("MSM_TOP_BESIDE")) p->top_beside = p->top_beside && std::atoi(e) != 0;
   msm_status_t st;
   int prev_dev = -1;
   if (cudaGetDevice(&prev_dev) != cudaSuccess) { prev_dev = -1; cudaGetLastError(); }
@@ -818,6 +832,8 @@ msm_status_t msm_plan_create_dynamic(const msm_params_t* params, double reserve,
   *plan_out = p;
   return MSM_OK;
 }
+
+extern "C" {
 
 msm_status_t msm_plan_info(const msm_plan_t* p, msm_plan_info_t* info) {
   if (!p || !info) return MSM_ERR_INVALID_ARG;

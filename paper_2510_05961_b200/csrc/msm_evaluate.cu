@@ -226,8 +226,10 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     else
       MSM_LAUNCH(p, (k_anterp_combine<T, P, false><<<cgrid, cblock, 0, st>>>(gg, p->at, (const T*)p->anterp_scratch, (T*)p->lev[1].Q)));
   } else {
-    MSM_LAUNCH(p, (k_anterpolate<T, P><<<blocks_for(H.lev[1].points() * 16, 128), 128, 0, st>>>(
-                      gg, tab, p->gstart, (const V4*)p->grec, (T*)p->lev[1].Q)));
+    // lanes per node: 16; 1 in a batch (64 x 512 particles: 0.91 against 1.00 ms per batch with 16)
+    const int lg = p->in_batch ? 0 : 4;
+    MSM_LAUNCH(p, (k_anterpolate<T, P><<<blocks_for(H.lev[1].points() << lg, 128), 128, 0, st>>>(
+                      gg, tab, p->gstart, (const V4*)p->grec, (T*)p->lev[1].Q, lg)));
   }
   mark();
 
@@ -370,6 +372,17 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     }
   }
   mark();
+  bool top_early = false;
+  auto launch_top = [&](cudaStream_t ts) {
+    LevelDev& d = p->lev[p->n_t];
+    const unsigned nb = blocks_for((size_t)p->G * 32, 128);
+    if (want_virial)
+      MSM_LAUNCH(p, (k_top_dense<T, true><<<nb, 128, 0, ts>>>(p->G, (const T*)p->topT, (const T*)p->topTD, (const T*)d.Q,
+                                                             (T*)d.E, p->top_wrow)));
+    else
+      MSM_LAUNCH(p, (k_top_dense<T, false><<<nb, 128, 0, ts>>>(p->G, (const T*)p->topT, (const T*)p->topTD, (const T*)d.Q,
+                                                              (T*)d.E, p->top_wrow)));
+  };
   if (p->conv.nlev > 0) {
     constexpr int XT = sizeof(T) == 4 ? 16 : 8, ZT = 4;
     // shared memory of a generic (fp64) unit: plane | row entries of ZT layers | two row-tap buffers
@@ -410,10 +423,24 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
     };
     // the virial correlation only needs the filtered grid charge: it runs on a third stream beside
     // the potential convolution (not with per-stage profiling on) and joins before the reductions
-    if (want_virial && p->overlap && !p->profiling && p->vstream) {
+    // So does the dense top-level operator (it needs only the restricted charge): it goes first on
+    // that stream and the prolongation waits for it (a small system's critical path is its chain of
+    // dependent kernels: 0.025 ms of 0.13 at N = 3000).
+    // Only where that stream is forked anyway (virial requested: a fork for the top operator alone
+    // costs more than it gives) and only for small jobs outside a batch: at N = 10^6 it costs 0.06 ms (the virial kernel then starts
+    // behind the potential kernel instead of in front of it), and the extra graph nodes of 64 batched
+    // systems cost more than the overlap gives (0.94 -> 1.09 ms per batch).
+    const bool beside = p->overlap && !p->profiling && p->vstream;
+    const bool top_beside = beside && want_virial && p->top_beside && p->conv.total_units < 4096;
+    if (beside && want_virial) {
       cudaEventRecord(p->fork2_ev, st);
       cudaStreamWaitEvent(p->vstream, p->fork2_ev, 0);
-      launch_virial(p->vstream);
+      if (top_beside) {
+        launch_top(p->vstream);
+        cudaEventRecord(p->top_ev, p->vstream);
+        top_early = true;
+      }
+      if (want_virial) launch_virial(p->vstream);
       cudaEventRecord(p->join2_ev, p->vstream);
       forked_v = true;
     }
@@ -474,19 +501,12 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   }
 
   // ---------------- S6 top level
-  {
-    LevelDev& d = p->lev[p->n_t];
-    const unsigned nb = blocks_for((size_t)p->G * 32, 128);
-    if (want_virial) {
-      MSM_LAUNCH(p, (k_top_dense<T, true><<<nb, 128, 0, st>>>(p->G, (const T*)p->topT, (const T*)p->topTD,
-                                                             (const T*)d.Q, (T*)d.E, p->top_wrow)));
-      Seg& s = fa.seg[nseg++];
-      s.ptr = p->top_wrow; s.count = p->G; s.width = 6;
-      for (int k = 0; k < 6; ++k) s.scale[k] = 1.0;
-    } else {
-      MSM_LAUNCH(p, (k_top_dense<T, false><<<nb, 128, 0, st>>>(p->G, (const T*)p->topT, (const T*)p->topTD,
-                                                              (const T*)d.Q, (T*)d.E, p->top_wrow)));
-    }
+  if (top_early) cudaStreamWaitEvent(st, p->top_ev, 0);
+  else launch_top(st);
+  if (want_virial) {
+    Seg& s = fa.seg[nseg++];
+    s.ptr = p->top_wrow; s.count = p->G; s.width = 6;
+    for (int k = 0; k < 6; ++k) s.scale[k] = 1.0;
   }
   mark();
 
@@ -793,7 +813,7 @@ msm_status_t msm_batch_create(const msm_params_t* params, int batch, msm_batch_t
     b->plans.reserve(batch);
     for (int i = 0; i < batch; ++i) {
       msm_plan_t* p = nullptr;
-      const msm_status_t s = msm_plan_create(params, &p);
+      const msm_status_t s = msm::plan_create_opts(params, 0.0, true, &p);
       if (s != MSM_OK) { msm_batch_destroy(b); return s; }
       p->graph_enabled = false;                     // the batch owns the graph
       b->plans.push_back(p);

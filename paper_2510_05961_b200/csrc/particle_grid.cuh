@@ -12,20 +12,22 @@ struct GridGeom {
   int periodic[3];
 };
 
-// Sixteen lanes per level-1 grid point m: q~_m = sum_i q_i phi_m(r_i), gathered from the particles
-// of the p^3 grid cells whose support contains m. Lane s of a node's group takes the cell rows
-// (jz, jy) with index s (mod 16) and walks their p cells along x (ascending cell index, particles
-// inside a cell in ascending original index); the 16 partial sums are added in a fixed shuffle
-// tree -> no atomics, bit-reproducible. (One thread per node walked p^3 cells one after the other,
-// two dependent global loads each: 43 us for 3000 particles on a 16^3 grid.)
+// 2^lg lanes per level-1 grid point m (16 for a plan on its own, 1 inside a batch, where the other
+// systems fill the GPU): q~_m = sum_i q_i phi_m(r_i), gathered from the particles of the p^3 grid
+// cells whose support contains m. Lane s of a node's group takes the cell rows (jz, jy) with index
+// s (mod 2^lg) and walks their p cells along x (ascending cell index, particles inside a cell in
+// ascending original index); the partial sums are added in a fixed shuffle tree -> no atomics,
+// bit-reproducible. (One thread per node walks p^3 cells one after the other, two dependent global
+// loads each: 43 us for 3000 particles on a 16^3 grid, 11 us with 16 lanes.)
 template <typename T, int P>
 __global__ void __launch_bounds__(128)
 k_anterpolate(GridGeom g, SplineTab<T, P> tab, const int* __restrict__ gstart,
-              const typename Vec4<T>::type* __restrict__ grec, T* __restrict__ Q) {
+              const typename Vec4<T>::type* __restrict__ grec, T* __restrict__ Q, int lg) {
   constexpr int HP = P / 2;
   const int total = g.M[0] * g.M[1] * g.M[2];
-  const int sub = threadIdx.x & 15;
-  const int m = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 4);
+  const int G = 1 << lg;
+  const int sub = threadIdx.x & (G - 1);
+  const int m = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> lg);
   const bool live = m < total;                       // (whole groups: every lane reaches the shuffles)
   const int mc = live ? m : 0;
   const int mx = mc % g.M[0], my = (mc / g.M[0]) % g.M[1], mz = mc / (g.M[0] * g.M[1]);
@@ -33,7 +35,7 @@ k_anterpolate(GridGeom g, SplineTab<T, P> tab, const int* __restrict__ gstart,
   T acc = 0;
   // node n = i0 + j, j = -HP+1..HP  ->  cell i0 = n - j, spline row j + HP - 1
 #pragma unroll 1
-  for (int row = sub; row < P * P; row += 16) {
+  for (int row = sub; row < P * P; row += G) {
     const int jz = row / P - HP + 1, jy = row % P - HP + 1;
     int cz = nz - jz, cy = ny - jy;
     if (g.periodic[2]) cz = imod(cz, g.ng[2]);
@@ -57,8 +59,7 @@ k_anterpolate(GridGeom g, SplineTab<T, P> tab, const int* __restrict__ gstart,
       }
     }
   }
-#pragma unroll
-  for (int o = 8; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
   if (live && sub == 0) Q[m] = acc;
 }
 

@@ -77,6 +77,9 @@ struct msm_plan {
   msm::ConvTable* d_conv = nullptr;
   size_t conv_smem = 0;
   int conv_ny_max = 0, conv_maxc = 0;   // largest row count 2 R_y + 1 and chunks per stencil row over the levels
+  bool in_batch = false;                             // one of the plans of an msm_batch
+  bool top_beside = true;                            // small jobs: the top-level operator runs beside the convolution (not in a batch)
+  long long conv_tiles_total = 0;                    // output tiles of all tiled levels
   bool conv_rowsliced = false;                       // some level splits its plane slices by stencil rows (small jobs: no list kernels)
   bool conv_lists = true;                            // fp32: every level has the entry lists of k_conv_f2l
   size_t conv_vtables_smem = 0;                      // fp32: largest interleaved virial tap table of a level (bytes)
@@ -132,7 +135,7 @@ struct msm_plan {
   // second stream for the pair kernel (runs beside the grid pipeline)
   bool overlap = true;
   cudaStream_t pstream = nullptr, vstream = nullptr;
-  cudaEvent_t fork_ev = nullptr, join_ev = nullptr, fork2_ev = nullptr, join2_ev = nullptr;
+  cudaEvent_t fork_ev = nullptr, join_ev = nullptr, fork2_ev = nullptr, join2_ev = nullptr, top_ev = nullptr;
 
   // profiling
   bool profiling = false;
@@ -143,3 +146,7 @@ struct msm_plan {
   std::vector<const char*> stage_names;
   int launches = 0;
 };
+
+namespace msm {
+msm_status_t plan_create_opts(const msm_params_t* params, double reserve, bool in_batch, msm_plan_t** plan_out);
+}

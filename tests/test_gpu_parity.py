@@ -566,11 +566,13 @@ def test_batched_small_systems_against_their_own_oracle_runs():
     nfull = [cap] * B
     U3, _ = batch.evaluate(nfull, tp, tq, F, V)
     assert np.abs(U3 - U).max() <= 1e-11 * np.abs(U).max()
-    # one system through a plain plan: identical bits
+    # one system through a plain plan: the same to rounding (a plan on its own sums the anterpolation
+    # of this small grid with 16 lanes per node, a plan inside a batch with one)
     plan = msm.Plan((20.0,) * 3, (0, 0, 0), 2.0, 6.0, 4, 3, "fp64", max_particles=cap)
     F1 = torch.zeros((n[5], 3), dtype=torch.float64, device=dev)
     U1, W1 = plan.evaluate(tp[5, :n[5]].contiguous(), tq[5, :n[5]].contiguous(), F1)
-    assert U1 == U[5] and np.array_equal(W1, W[5]) and torch.equal(F1, F0[5, :n[5]])
+    assert abs(U1 - U[5]) <= 1e-13 * abs(U[5]) and np.abs(W1 - W[5]).max() <= 1e-13 * np.abs(W[5]).max()
+    assert float((F1 - F0[5, :n[5]]).abs().max()) <= 1e-13 * float(F1.abs().max())
 
 
 def test_dynamic_cell_on_the_large_grid_kernels():
