@@ -575,6 +575,25 @@ def test_batched_small_systems_against_their_own_oracle_runs():
     assert float((F1 - F0[5, :n[5]]).abs().max()) <= 1e-13 * float(F1.abs().max())
 
 
+@pytest.mark.parametrize("periodic,box,h,a,p,n", [
+    ((1, 1, 0), (128.0, 128.0, 36.0), 1.0, 4.0, 4, 44001),    # slab: zero halo planes above and below the grid
+    ((1, 1, 1), (120.0, 136.0, 128.0), 1.0, 4.5, 6, 60001),   # unequal spacings (ellipsoidal stencil), p = 6
+])
+def test_list_driven_convolution_other_geometries(periodic, box, h, a, p, n):
+    """The list-driven fp32 convolution / virial kernels (jobs of at least 4096 units: their entry
+    lists depend on the stencil's shape) on a slab and on a box with three different spacings:
+    every output and every level's grids against the oracle."""
+    from paper_2510_05961_b200 import msm
+    rng = np.random.default_rng(1234)
+    pos = rng.random((n, 3)) * np.array(box)
+    q = rng.uniform(-1, 1, n); q -= q.mean()
+    w = _custom(f"lists_{''.join(map(str, periodic))}_p{p}", pos, q, box, periodic, h, a, p, 4, "fp32")
+    gpu = run_gpu(w, precision="fp32")
+    assert tuple(gpu["plan"].grid_dims(1))[:2] == (128, 128)
+    ref = run_oracle(w)
+    _log(w.name, compare(w, gpu, ref, "fp32"))
+
+
 def test_dynamic_cell_on_the_large_grid_kernels():
     """msm_plan_set_box on a plan large enough for the list-driven fp32 convolution kernels (128^3
     finest grid: their entry lists are built from the reserved table STRUCTURE, the tap VALUES are
