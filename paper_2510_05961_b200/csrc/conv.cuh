@@ -58,6 +58,9 @@ struct ConvLevel {
   const void* vtaps;          // per chunk: 4 x 2g, 4 x 2g dx, 4 x 2g dx^2
   const int4* vrows2;         // fp32 packed virial: half-space rows d and d - 1 merged, d = 0 .. R[2]+1
   const void* vtaps2;         // per chunk 24 floats: for 2g, 2g dx, 2g dx^2: 4 taps x (row d, row d - 1)
+  const int4* dlist;          // fp64 list-driven potential kernel: entry = 2 x int4 byte offsets (window, taps of planes 0 .. 3, -, -, -)
+  const int* dhead;           // [2 R[2] + 4][kConvListTypes + 1]
+  int n_stapsq, dsunit0;      // 16-byte quads of staps; first unit of this level in the fp64 list launch
   const int4* vlist;          // list-driven virial: byte offsets (window, chunk of pair 0, of pair 1 in vtaps2), dy as float bits
   const int* vhead;           // [R[2] + 4][kConvListTypes + 1]: list bounds per input plane offset zr
   int n_vtaps2q, vsunit0;     // float4 quads of vtaps2; first unit of this level in the list-driven virial launch
@@ -68,12 +71,13 @@ struct ConvLevel {
 };
 
 constexpr int kConvListTypes = 7;   // both full | pair 0 full | pair 1 full | pair 0 lower, upper half | pair 1 lower, upper half
+constexpr int kConvDW = 12;   // warps (units) per block of the fp64 list-driven potential kernel (one block per SM)
 constexpr int kConvVW = 16;   // warps (units) per block of the list-driven virial kernel (one block per SM)
 constexpr int kConvSW = 8;    // warps (units) per block of the shared-table convolution kernel
 
 struct ConvTable {
   int nlev;
-  int total_units, total_vunits, total_sunits, total_vsunits;
+  int total_units, total_vunits, total_sunits, total_vsunits, total_dsunits;
   ConvLevel lev[kMaxConvLevels];
 };
 
@@ -1096,6 +1100,147 @@ k_conv_virial_f2l(const ConvTable* __restrict__ tabp, int plane_bytes) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
     if (lane == 0) g.wpart[(size_t)local * 6 + k] = v;
+  }
+}
+
+// --------------------------------------------------------- potential, fp64, list-driven (see k_conv_f2l)
+// One block of kConvDW warps per SM with the level's tap table (mirrored rows stored once) in shared
+// memory; a unit is an 8 x 32 x 4 output tile and a slice of input planes. The chunks of each input
+// plane offset are sorted into seven lists: all four output planes take the chunk / planes (0, 1) /
+// planes (2, 3) / one of the four planes alone.
+template <int OFF>
+__device__ __forceinline__ double2 lds128d(unsigned addr) {
+  double2 v;
+  asm("ld.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(v.x), "=d"(v.y) : "r"(addr), "n"(OFF));
+  return v;
+}
+
+// MASK: bit k set = output plane k takes this chunk
+template <int MASK>
+__device__ __forceinline__ void convd_list_run(int b, int e, const int4* __restrict__ el, unsigned srow0, unsigned staps,
+                                               double (&acc)[4][8]) {
+  if (b >= e) return;
+  int4 n0 = __ldg(el + 2 * b), n1 = __ldg(el + 2 * b + 1);
+#pragma unroll 1
+  for (int i = b; i < e; ++i) {
+    const int4 c0 = n0, c1 = n1;                      // (window, taps 0, taps 1, taps 2), (taps 3, -, -, -)
+    n0 = __ldg(el + 2 * i + 2);                       // (guard entry behind the end)
+    n1 = __ldg(el + 2 * i + 3);
+    const unsigned w = srow0 + (unsigned)c0.x;
+    double win[12];
+    {
+      const double2 t0 = lds128d<0>(w), t1 = lds128d<16>(w), t2 = lds128d<32>(w), t3 = lds128d<48>(w), t4 = lds128d<64>(w),
+                    t5 = lds128d<80>(w);
+      win[0] = t0.x; win[1] = t0.y; win[2] = t1.x; win[3] = t1.y; win[4] = t2.x; win[5] = t2.y;
+      win[6] = t3.x; win[7] = t3.y; win[8] = t4.x; win[9] = t4.y; win[10] = t5.x; win[11] = t5.y;
+    }
+    double tp[4][4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      if (!(MASK & (1 << k))) continue;
+      const unsigned ta = staps + (unsigned)(k == 0 ? c0.y : k == 1 ? c0.z : k == 2 ? c0.w : c1.x);
+      const double2 a = lds128d<0>(ta), bq = lds128d<16>(ta);
+      tp[k][0] = a.x; tp[k][1] = a.y; tp[k][2] = bq.x; tp[k][3] = bq.y;
+    }
+#pragma unroll
+    for (int t = 0; t < 4; ++t)
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        if (!(MASK & (1 << k))) continue;
+#pragma unroll
+        for (int x = 0; x < 8; ++x) acc[k][x] = fma(tp[k][t], win[x + t], acc[k][x]);
+      }
+  }
+}
+
+template <int XT>
+__global__ void __launch_bounds__(32 * kConvDW, 1)
+k_conv_dl(const ConvTable* __restrict__ tabp, int plane_bytes) {
+  static_assert(XT == 8, "window of 12 doubles");
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const ConvTable& tab = *tabp;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int l = 0;
+#pragma unroll 1
+  for (int k = 1; k < tab.nlev; ++k)
+    if ((int)blockIdx.x * kConvDW >= tab.lev[k].dsunit0) l = k;
+  const ConvLevel& g = tab.lev[l];
+  double2* stq = reinterpret_cast<double2*>(smem_raw);
+  unsigned char* planes = reinterpret_cast<unsigned char*>(stq + g.n_stapsq);
+  const double2* gt = reinterpret_cast<const double2*>(g.staps);
+  for (int i = threadIdx.x; i < g.n_stapsq; i += 32 * kConvDW) stq[i] = __ldg(gt + i);
+  __syncthreads();
+  int r = (int)blockIdx.x * kConvDW + warp - g.dsunit0;
+  if (r >= g.tiles[0] * g.tiles[1] * g.tiles[2] * g.nslices) return;         // padding unit
+  const int slice = r % g.nslices; r /= g.nslices;
+  const int X = (r % g.tiles[0]) * XT; r /= g.tiles[0];
+  const int Y = (r % g.tiles[1]) * 32;
+  const int Z = (r / g.tiles[1]) * 4;
+  double* plane = reinterpret_cast<double*>(planes + (size_t)warp * plane_bytes);
+  const int Ry = g.R[1], Rz = g.R[2];
+  const int nrow = 32 + 2 * Ry;
+  const int WX = XT + 2 * g.X0 + 4;
+  const double* __restrict__ qpad = reinterpret_cast<const double*>(g.pad);
+  const int4* __restrict__ el = g.dlist;
+  unsigned srow0, staps;
+  asm volatile("mov.u32 %0, %1;" : "=r"(srow0) : "r"((unsigned)__cvta_generic_to_shared(plane + lane * g.pitch)));
+  asm volatile("mov.u32 %0, %1;" : "=r"(staps) : "r"((unsigned)__cvta_generic_to_shared(stq)));
+  const unsigned plane_s = (unsigned)__cvta_generic_to_shared(plane);
+  const unsigned mbar = (unsigned)__cvta_generic_to_shared(planes + (size_t)kConvDW * plane_bytes) + 8u * warp;
+  unsigned phase = 0;
+  if (lane == 0) mbar_init(mbar);
+  __syncwarp();
+
+  double acc[4][XT];
+#pragma unroll
+  for (int k = 0; k < 4; ++k)
+#pragma unroll
+    for (int i = 0; i < XT; ++i) acc[k][i] = 0.0;
+
+  const int p0 = g.pb[slice], p1 = g.pb[slice + 1];
+#pragma unroll 1
+  for (int pz = p0; pz < p1; ++pz) {                  // input plane z = Z + pz - Rz feeds output plane k with dz = pz - Rz - k
+    const int4 h0 = __ldg(reinterpret_cast<const int4*>(g.dhead + pz * (kConvListTypes + 1)));
+    const int4 h1 = __ldg(reinterpret_cast<const int4*>(g.dhead + pz * (kConvListTypes + 1)) + 1);
+    // rows of WX doubles: one bulk copy each
+    {
+      const double* src = qpad + ((size_t)(Z + pz) * g.P[1] + Y) * g.P[0] + X;
+      __syncwarp();
+      if (lane == 0)
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(mbar), "r"((unsigned)(nrow * WX * 8)) : "memory");
+      __syncwarp();
+      for (int rr = lane; rr < nrow; rr += 32)
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     :: "r"(plane_s + (unsigned)(rr * g.pitch * 8)), "l"(src + (size_t)rr * g.P[0]), "r"((unsigned)(WX * 8)), "r"(mbar)
+                     : "memory");
+      unsigned done;
+      do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(done) : "r"(mbar), "r"(phase) : "memory");
+      } while (!done);
+      phase ^= 1u;
+    }
+    convd_list_run<15>(h0.x, h0.y, el, srow0, staps, acc);
+    convd_list_run<3>(h0.y, h0.z, el, srow0, staps, acc);
+    convd_list_run<12>(h0.z, h0.w, el, srow0, staps, acc);
+    convd_list_run<1>(h0.w, h1.x, el, srow0, staps, acc);
+    convd_list_run<2>(h1.x, h1.y, el, srow0, staps, acc);
+    convd_list_run<4>(h1.y, h1.z, el, srow0, staps, acc);
+    convd_list_run<8>(h1.z, h1.w, el, srow0, staps, acc);
+  }
+  const int y = Y + lane;
+  if (y < g.M[1]) {
+    double* out = reinterpret_cast<double*>(g.out) + (size_t)slice * g.M[0] * g.M[1] * g.M[2];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int z = Z + k;
+      if (z < g.M[2]) {
+        double* dst = out + ((size_t)z * g.M[1] + y) * g.M[0] + X;
+#pragma unroll
+        for (int i = 0; i < XT; ++i)
+          if (X + i < g.M[0]) dst[i] = acc[k][i];
+      }
+    }
   }
 }
 

@@ -100,6 +100,7 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   std::vector<int4> rows((size_t)ny * nz), vrows((size_t)ny * (Rz + 1));
   std::vector<double> ts, tv;
   std::vector<double> wz(nz, 0.0), wzv(Rz + 1, 0.0);     // chunks per tap plane (work weights)
+  std::map<std::pair<int, int>, int> seen_rows;
   for (int dz = -Rz; dz <= Rz; ++dz)
     for (int dy = -st.R[1]; dy <= st.R[1]; ++dy) {
       int4& r = rows[(size_t)(dz + Rz) * ny + (dy + st.R[1])];
@@ -113,16 +114,22 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
       if (Rx < 0) { r = make_int4(0, 1, 0, 0); }
       else {
         const int clo = (-Rx + g.X0) / 4, chi = (Rx + g.X0) / 4;
-        r = make_int4((int)(ts.size() / 4), clo, chi, 0);
         p->conv_maxc = std::max(p->conv_maxc, chi - clo + 1);
         wz[dz + Rz] += chi - clo + 1 + 0.5;
-        for (int c = clo; c <= chi; ++c)
-          for (int t = 0; t < 4; ++t) {
-            const int dx = 4 * c - g.X0 + t;
-            const bool in = dx >= -Rx && dx <= Rx;
-            ts.push_back(in ? st.at(st.s, dx, dy, dz) : 0.0);
-            tsd.push_back(make_int4(dx, dy, dz, in ? 1 : 0));
-          }
+        // s is even in every coordinate (for any spacings): the rows (+-dz, +-dy) share one copy
+        const std::pair<int, int> key(std::abs(dz), std::abs(dy));
+        auto it = seen_rows.find(key);
+        if (it == seen_rows.end()) {
+          it = seen_rows.emplace(key, (int)(ts.size() / 4)).first;
+          for (int c = clo; c <= chi; ++c)
+            for (int t = 0; t < 4; ++t) {
+              const int dx = 4 * c - g.X0 + t;
+              const bool in = dx >= -Rx && dx <= Rx;
+              ts.push_back(in ? st.at(st.s, dx, dy, dz) : 0.0);
+              tsd.push_back(make_int4(dx, dy, dz, in ? 1 : 0));
+            }
+        }
+        r = make_int4(it->second, clo, chi, 0);
       }
       // virial: half space n > 0 (z, then y, then x), weight 2 (C(n) is even, reading V)
       if (dz < 0) continue;
@@ -153,6 +160,53 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   g.staps = upload(p, ts);
   g.vtaps = upload(p, tv);
   d.tab[0] = TapTable{const_cast<void*>(g.staps), upload_desc(p, tsd), (int)ts.size()};
+  g.dlist = nullptr;
+  g.dhead = nullptr;
+  g.n_stapsq = (int)((ts.size() * p->esz + 15) / 16);
+  if (!p->fp32) {
+    // entry lists of the fp64 list-driven potential kernel (k_conv_dl): input plane offset zr feeds
+    // output plane k through stencil layer dz = zr - k; lists: all four planes / planes (0, 1) /
+    // planes (2, 3) / one plane alone
+    auto on = [&](int dz, int j, int c, int& chunk) {
+      if (dz < -Rz || dz > Rz) return false;
+      const int4& r = rows[(size_t)(dz + Rz) * ny + j];
+      if (c < r.y || c > r.z) return false;
+      chunk = r.x + (c - r.y);
+      return true;
+    };
+    std::vector<int4> el;
+    std::vector<int> eh;
+    const int cmax = (2 * g.X0) / 4 + 1;
+    for (int zr = -Rz; zr <= Rz + 3; ++zr) {
+      std::vector<int4> lists[kConvListTypes];
+      for (int j = 0; j < ny; ++j)
+        for (int c = 0; c <= cmax; ++c) {
+          int ch[4] = {0, 0, 0, 0};
+          bool a[4];
+          for (int k = 0; k < 4; ++k) a[k] = on(zr - k, j, c, ch[k]);
+          if (!(a[0] || a[1] || a[2] || a[3])) continue;
+          const int4 e0 = make_int4((j * g.pitch + 4 * c) * 8, ch[0] * 32, ch[1] * 32, ch[2] * 32), e1 = make_int4(ch[3] * 32, 0, 0, 0);
+          auto put = [&](int t) { lists[t].push_back(e0); lists[t].push_back(e1); };
+          if (a[0] && a[1] && a[2] && a[3]) { put(0); continue; }
+          if (a[0] && a[1]) put(1); else { if (a[0]) put(3); if (a[1]) put(4); }
+          if (a[2] && a[3]) put(2); else { if (a[2]) put(5); if (a[3]) put(6); }
+        }
+      for (int t = 0; t < kConvListTypes; ++t) {
+        eh.push_back((int)(el.size() / 2));
+        el.insert(el.end(), lists[t].begin(), lists[t].end());
+      }
+      eh.push_back((int)(el.size() / 2));
+    }
+    el.push_back(make_int4(0, 0, 0, 0));
+    el.push_back(make_int4(0, 0, 0, 0));
+    int4* eld = (int4*)dev_alloc(p, el.size() * sizeof(int4));
+    int* ehd = (int*)dev_alloc(p, eh.size() * sizeof(int));
+    if (cudaMemcpy(eld, el.data(), el.size() * sizeof(int4), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(ehd, eh.data(), eh.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess)
+      throw CudaFail();
+    g.dlist = eld;
+    g.dhead = ehd;
+  }
   d.tab[2] = TapTable{const_cast<void*>(g.vtaps), upload_desc(p, tvd), (int)tv.size()};
   g.rows2 = nullptr;
   g.elist = nullptr;
@@ -402,6 +456,9 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   g.vunit0 = p->conv.total_vunits;
   g.sunit0 = p->conv.total_sunits;                       // blocks of kConvSW units never straddle two levels
   p->conv.total_sunits += (tiles * g.nslices + kConvSW - 1) / kConvSW * kConvSW;
+  g.dsunit0 = p->conv.total_dsunits;
+  p->conv.total_dsunits += (tiles * g.nslices + kConvDW - 1) / kConvDW * kConvDW;
+  if (!p->fp32) p->conv_dtables_smem = std::max(p->conv_dtables_smem, (size_t)g.n_stapsq * 16);
   g.vsunit0 = p->conv.total_vsunits;
   p->conv.total_vsunits += (tiles * g.vslices + kConvVW - 1) / kConvVW * kConvVW;
   if (p->fp32) {

@@ -466,11 +466,22 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
           MSM_LAUNCH(p, (kern<<<p->conv.total_units, 32, sm, st>>>(p->d_conv, sl)));
         }
       } else {
+        // fp64: list-driven kernel, one block of kConvDW warps per SM with the tap table in shared
+        // memory (large jobs)
+        const size_t plane_b = (p->conv_smem + 15) / 16 * 16;
+        const size_t sm_d = p->conv_dtables_smem + kConvDW * plane_b + kConvDW * 8;
+        static const bool no_l = std::getenv("MSM_CONV_NO_LISTS") != nullptr;
+        if (!no_l && !p->conv_rowsliced && sm_d <= 226 * 1024 && p->conv.total_units >= 4096) {
+          auto kern = k_conv_dl<8>;
+          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_d);
+          MSM_LAUNCH(p, (kern<<<p->conv.total_dsunits / kConvDW, 32 * kConvDW, sm_d, st>>>(p->d_conv, (int)plane_b)));
+        } else {
         auto kern = k_conv<T, XT, ZT>;
         size_t sm;
         const ConvSmemLayout sl = conv_layout(4, ZT, sm);
         if (sm > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
         MSM_LAUNCH(p, (kern<<<p->conv.total_units, 32, sm, st>>>(p->d_conv, sl)));
+        }
       }
       for (int l = 1; l < p->n_t; ++l) {
         const ConvLevel& g = p->conv.lev[l - 1];

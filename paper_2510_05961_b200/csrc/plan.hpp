@@ -82,6 +82,7 @@ struct msm_plan {
   long long conv_tiles_total = 0;                    // output tiles of all tiled levels
   bool conv_rowsliced = false;                       // some level splits its plane slices by stencil rows (small jobs: no list kernels)
   bool conv_lists = true;                            // fp32: every level has the entry lists of k_conv_f2l
+  size_t conv_dtables_smem = 0;                      // fp64: largest 4-tap chunk table of a level (bytes)
   size_t conv_vtables_smem = 0;                      // fp32: largest interleaved virial tap table of a level (bytes)
   size_t conv_tables_smem = 0;                       // fp32: largest row + tap table of a level (bytes)
   int conv_slices = 1, conv_vslices = 1;             // input-plane slices per output tile (potential, virial kernel)
