@@ -100,7 +100,7 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
   std::vector<int4> rows((size_t)ny * nz), vrows((size_t)ny * (Rz + 1));
   std::vector<double> ts, tv;
   std::vector<double> wz(nz, 0.0), wzv(Rz + 1, 0.0);     // chunks per tap plane (work weights)
-  std::map<std::pair<int, int>, int> seen_rows;
+  std::map<std::pair<int, int>, int> seen_rows, seen_vrows;
   for (int dz = -Rz; dz <= Rz; ++dz)
     for (int dy = -st.R[1]; dy <= st.R[1]; ++dy) {
       int4& r = rows[(size_t)(dz + Rz) * ny + (dy + st.R[1])];
@@ -138,17 +138,23 @@ void build_conv_tables(msm_plan* p, int l, int XT, int ZT) {
       if (Rx < 0 || !(whole || centre) || (centre && Rx < 1)) { v = make_int4(0, 1, 0, 0); continue; }
       const int xlo = centre ? 1 : -Rx;
       const int clo = (xlo + g.X0) / 4, chi = (Rx + g.X0) / 4;
-      v = make_int4((int)(tv.size() / 12), clo, chi, 0);
       wzv[dz] += chi - clo + 1 + 0.5;
-      for (int c = clo; c <= chi; ++c)
-        for (int m = 0; m < 3; ++m)
-          for (int t = 0; t < 4; ++t) {
-            const int dx = 4 * c - g.X0 + t;
-            const bool in = dx >= xlo && dx <= Rx;
-            const double gv = in ? 2.0 * st.at(st.g, dx, dy, dz) : 0.0;
-            tv.push_back(m == 0 ? gv : m == 1 ? gv * dx : gv * dx * dx);
-            tvd.push_back(make_int4(dx, dy, dz, in ? 2 + m : 0));
-          }
+      // g is even in every coordinate: the whole rows (dz > 0, +-dy) share one copy
+      const std::pair<int, int> vkey(dz, dz > 0 ? std::abs(dy) : dy);
+      auto vit = seen_vrows.find(vkey);
+      if (vit == seen_vrows.end()) {
+        vit = seen_vrows.emplace(vkey, (int)(tv.size() / 12)).first;
+        for (int c = clo; c <= chi; ++c)
+          for (int m = 0; m < 3; ++m)
+            for (int t = 0; t < 4; ++t) {
+              const int dx = 4 * c - g.X0 + t;
+              const bool in = dx >= xlo && dx <= Rx;
+              const double gv = in ? 2.0 * st.at(st.g, dx, dy, dz) : 0.0;
+              tv.push_back(m == 0 ? gv : m == 1 ? gv * dx : gv * dx * dx);
+              tvd.push_back(make_int4(dx, dy, dz, in ? 2 + m : 0));
+            }
+      }
+      v = make_int4(vit->second, clo, chi, 0);
     }
   auto up_rows = [&](const std::vector<int4>& r) {
     int4* dptr = (int4*)dev_alloc(p, r.size() * sizeof(int4));
