@@ -136,7 +136,8 @@ msm_status_t msm_plan_set_box(msm_plan_t *plan, const double *box /* 3 doubles *
  * one-sweep restriction / prolongation / filter kernels run; default 4 Mi points for restriction
  * and filter, 0 for prolongation), MSM_FILTER_STREAM_MIN=<points> (the same for the filter alone),
  * MSM_CONV_SLICES=<n> / MSM_CONV_VSLICES=<n> (input-plane slices per convolution / virial tile),
- * MSM_CONV_NO_LISTS=1 (fp32 convolution with the row/chunk loops instead of the entry lists), MSM_CONV_GLOBAL_TAPS=1 (fp32
+ * MSM_CONV_NO_LISTS=1 (convolution kernels with the row/chunk loops instead of the entry lists),
+ * MSM_TOP_BESIDE=0 (small jobs: the top-level operator after the convolution instead of beside it), MSM_CONV_GLOBAL_TAPS=1 (fp32
  * convolution reads its stencil tables from global memory), MSM_ANTERP_TILED=0 /
  * MSM_ANTERP_MIN_TILES=<n> (choice between the tiled and the gather anterpolation),
  * MSM_PAIR_SUBBINS_LOG2=<0..3> (x sub-bins per pair cell). */
