@@ -132,7 +132,7 @@ msm_status_t enqueue_t(msm_plan* p, int n, const void* d_pos, const void* d_q, v
   MSM_LAUNCH(p, (k_scatter<<<blocks_for(n, 256), 256, 0, st>>>(n, p->pcell, p->gcell, p->pstart, p->gstart,
                                                                  p->pslot, p->gslot, p->porder, p->gorder)));
   MSM_LAUNCH(p, (k_sort_cells<<<dim3(blocks_for(std::max(p->n_pcells, p->n_gcells), 128), 2), 128, 0, st>>>(
-                    p->n_pcells, p->pstart, p->porder, p->n_gcells, p->gstart, p->gorder)));
+                    p->n_pcells, p->pstart, p->porder, p->pslot, p->n_gcells, p->gstart, p->gorder, p->gslot)));
   MSM_LAUNCH(p, (k_build_records<T><<<blocks_for(n, 256), 256, 0, st>>>(
                     n, pos, q, p->bg, p->porder, p->pcell, p->gorder, p->gcell, (V4*)p->prec, (V4*)p->grec,
                     p->gcell_sorted, p->pcellx)));

@@ -201,21 +201,45 @@ __global__ void k_scatter(int n, const int* __restrict__ pcell, const int* __res
   gorder[gstart[gcell[i]] + gslot[i]] = i;
 }
 
-// pass 3: canonical order inside each cell (ascending original index): insertion sort per cell
+// pass 3: canonical order inside each cell (ascending original index). One thread per cell with an
+// insertion sort for the usual few particles per cell; a cell with more than kSortWarpMin particles
+// (clustered input: the single thread would do O(k^2) dependent global loads and stores) is then
+// rank-sorted by its whole warp through `tmp` (the arrival slots of pass 2, dead by now): every
+// element counts the smaller ones (the indices are distinct) and goes to that position.
 // (blockIdx.y = 0: the pair bins, 1: the grid cells)
-__global__ void k_sort_cells(int ncell0, const int* __restrict__ start0, int* __restrict__ order0, int ncell1,
-                             const int* __restrict__ start1, int* __restrict__ order1) {
+constexpr int kSortWarpMin = 24;
+__global__ void k_sort_cells(int ncell0, const int* __restrict__ start0, int* __restrict__ order0, int* __restrict__ tmp0,
+                             int ncell1, const int* __restrict__ start1, int* __restrict__ order1, int* __restrict__ tmp1) {
   const int ncell = blockIdx.y == 0 ? ncell0 : ncell1;
   const int* __restrict__ start = blockIdx.y == 0 ? start0 : start1;
   int* __restrict__ order = blockIdx.y == 0 ? order0 : order1;
+  int* __restrict__ tmp = blockIdx.y == 0 ? tmp0 : tmp1;
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= ncell) return;
-  const int s = start[c], e = start[c + 1];
-  for (int i = s + 1; i < e; ++i) {
-    const int v = order[i];
-    int j = i - 1;
-    while (j >= s && order[j] > v) { order[j + 1] = order[j]; --j; }
-    order[j + 1] = v;
+  const int lane = threadIdx.x & 31;
+  int s = 0, e = 0;
+  if (c < ncell) { s = start[c]; e = start[c + 1]; }
+  if (e - s <= kSortWarpMin) {
+    for (int i = s + 1; i < e; ++i) {
+      const int v = order[i];
+      int j = i - 1;
+      while (j >= s && order[j] > v) { order[j + 1] = order[j]; --j; }
+      order[j + 1] = v;
+    }
+  }
+  unsigned big = __ballot_sync(0xffffffffu, e - s > kSortWarpMin);
+  while (big) {
+    const int L = __ffs(big) - 1;
+    big &= big - 1;
+    const int bs = __shfl_sync(0xffffffffu, s, L), be = __shfl_sync(0xffffffffu, e, L);
+    for (int i = bs + lane; i < be; i += 32) {
+      const int v = order[i];
+      int rank = 0;
+      for (int j = bs; j < be; ++j) rank += order[j] < v;
+      tmp[bs + rank] = v;
+    }
+    __syncwarp();
+    for (int i = bs + lane; i < be; i += 32) order[i] = tmp[i];
+    __syncwarp();
   }
 }
 

@@ -316,17 +316,18 @@ def test_tiled_anterpolation_shapes(periodic, box, p, precision):
     _log(w.name, compare(w, gpu, ref, precision))
 
 
-@pytest.mark.parametrize("precision", ["fp64", "fp32"])
-def test_clustered_particles(precision):
+@pytest.mark.parametrize("precision,sigma", [("fp64", 3.0), ("fp32", 3.0), ("fp64", 1.4)])
+def test_clustered_particles(precision, sigma):
     """A dense blob in a large periodic box: cells with > 100 particles (several candidate batches
-    per neighbour row, many tiles per cell row) next to empty cells."""
+    per neighbour row, many tiles per cell row; sigma = 1.4: ~200 particles per sort cell, the
+    warp-cooperative in-cell sort) next to empty cells."""
     rng = np.random.default_rng(5)
     n = 3000
     box = (48.0, 48.0, 48.0)
-    pos = 24.0 + rng.normal(0.0, 3.0, (n, 3))
+    pos = 24.0 + rng.normal(0.0, sigma, (n, 3))
     pos = np.mod(pos, 48.0)
     q = rng.uniform(-1, 1, n); q -= q.mean()
-    w = _custom(f"blob_{precision}", pos, q, box, (1, 1, 1), 1.5, 6.0, 4, 2, precision)
+    w = _custom(f"blob_{precision}_{sigma}", pos, q, box, (1, 1, 1), 1.5, 6.0, 4, 2, precision)
     gpu = run_gpu(w, precision=precision)
     ref = run_oracle(w)
     errs = compare(w, gpu, ref, precision)
