@@ -169,15 +169,19 @@ struct ConvUnit {
 };
 
 // input planes [p0, p1) and stencil rows [j0, j1) of slice `slice` (plane slices fastest)
-struct SliceRange { int p0, p1, j0, j1; };
+struct SliceRange { int p0, p1, pstep, j0, j1; };   // planes p0, p0 + pstep, .. < p1
 template <bool VIRIAL>
 __device__ __forceinline__ SliceRange slice_range(const ConvLevel& g, int slice) {
   const int ysl = VIRIAL ? g.vysl : g.ysl;
   const int ps = (VIRIAL ? g.vslices : g.nslices) / ysl;
   const int s = slice % ps, y = slice / ps;
   SliceRange r;
-  r.p0 = VIRIAL ? g.vb[s] : g.pb[s];
-  r.p1 = VIRIAL ? g.vb[s + 1] : g.pb[s + 1];
+  if (VIRIAL) {
+    // the virial kernels deal the planes round-robin (equal taps and plane counts per slice)
+    r.p0 = s; r.p1 = g.R[2] + 4; r.pstep = ps;
+  } else {
+    r.p0 = g.pb[s]; r.p1 = g.pb[s + 1]; r.pstep = 1;
+  }
   r.j0 = y * g.ny / ysl;
   r.j1 = (y + 1) * g.ny / ysl;
   return r;
@@ -724,7 +728,7 @@ k_conv_virial(const ConvTable* __restrict__ tabp, ConvSmemLayout sl) {
   // only dz = zr - k >= 0: input planes zr in [0, ZT - 1 + Rz], padded index pz = zr + Rz
   const SliceRange sr = slice_range<true>(g, cu.slice);
   const int p0 = sr.p0, p1 = sr.p1;
-  for (int pp = p0; pp < p1; ++pp) {
+  for (int pp = p0; pp < p1; pp += sr.pstep) {
     const int zr = pp;
     stage_rows<ZT>(srows, rows, ny, lane, [&](int k) {
       const int dz = zr - k;
@@ -856,7 +860,7 @@ k_conv_virial_f2(const ConvTable* __restrict__ tabp, ConvSmemLayout sl) {
 
   const SliceRange sr = slice_range<true>(g, cu.slice);
   const int p0 = sr.p0, p1 = sr.p1;
-  for (int zr = p0; zr < p1; ++zr) {                  // input plane z = Z + zr, only dz >= 0
+  for (int zr = p0; zr < p1; zr += sr.pstep) {        // input plane z = Z + zr, only dz >= 0
     // row entries of the merged layers to shared memory with the plane; the taps of stencil row
     // dy + 1 are copied (cp.async) while row dy is computed: no FMA waits for a table load
     stage_rows<ZP>(srows, rows, ny, lane, [&](int k) {
