@@ -533,6 +533,17 @@ msm_status_t create_impl(const msm_params_t* prm, msm_plan* p) {
       // (N = 10^6: 4 / 2 slices 1.736 / 1.545 ms, 2 / 1 slices 1.812 / 1.567 ms)
       p->conv_slices = tiles > 0 ? (int)std::max<long long>(1, std::min<long long>(kMaxConvSlices, (3 * slots + tiles - 1) / tiles)) : 1;
       p->conv_vslices = p->conv_slices;             // (virial 1.55 -> 1.48 ms at N = 10^6 against half as many)
+      // large jobs run the list-driven potential kernel, ONE block of kConvDW warps per SM: few slices
+      // whose blocks fill whole waves of SMs (N = 10^6, 2336 tiles: 3 slices = 3.95 waves 1.22 ms,
+      // 4 slices = 5.26 waves 1.40 ms, 6 slices = 7.9 waves 1.38 ms)
+      if (tiles * p->conv_slices >= 4096) {
+        double best = -1.0;
+        for (int sl = 2; sl <= 8; ++sl) {
+          const double waves = (double)((tiles * sl + kConvDW - 1) / kConvDW) / (double)p->sm_count;
+          const double score = waves / std::ceil(waves) - 0.01 * sl;
+          if (tiles * sl >= 4096 && score > best) { best = score; p->conv_slices = sl; }
+        }
+      }
     }
     if (const char* e = std::getenv("MSM_CONV_SLICES")) p->conv_slices = std::max(1, std::atoi(e));
     if (const char* e = std::getenv("MSM_CONV_VSLICES")) p->conv_vslices = std::max(1, std::atoi(e));
