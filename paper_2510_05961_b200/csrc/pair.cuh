@@ -111,14 +111,19 @@ __device__ __forceinline__ float rsqrt_fast(float x) {
   asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-// fp64: fp32 hardware seed (relative error 2^-22.9) + two Newton steps y <- y (3/2 - x/2 y^2), each of
-// which squares the error: ~1e-13, then below the fp64 rounding unit. x is a squared distance inside
-// the cutoff (far from the fp32 range limits).
+// fp64: fp32 hardware seed (relative error 2^-22.9 incl. the rounding of x to fp32) + ONE Newton step
+// y <- y (3/2 - x/2 y^2), which squares the error (times 3/2): <= 2.5e-14 relative per pair term,
+// 4000 times inside the 1e-10 parity tolerance (measured force error 1.2e-14 at cfg5). A second step
+// (-DMSM_RSQRT_TWO_STEPS) reaches the fp64 rounding unit and costs 3.8 % of the fp64 pair kernel: it
+// sits on the drain's dependent chain. x is a squared distance inside the cutoff (far from the fp32
+// range limits).
 __device__ __forceinline__ double rsqrt_fast(double x) {
   double y = (double)rsqrt_fast((float)x);
   const double hx = 0.5 * x;
   y = y * fma(-hx, y * y, 1.5);
+#ifdef MSM_RSQRT_TWO_STEPS
   y = y * fma(-hx, y * y, 1.5);
+#endif
   return y;
 }
 
