@@ -207,7 +207,7 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
   T cf[P], cd[P];                                   // g(s) = sum cf[k] s^k, g'(s) = sum cd[k] s^(k-1)
 #pragma unroll
   for (int k = 0; k < P; ++k) { cf[k] = prm.c[k]; cd[k] = (T)k * prm.c[k]; }
-  T cds[P];                                         // 2/a^3 g'(s) for the scalar path: one fp64 multiply less per pair
+  T cds[P];                                         // 2/a^3 g'(s): one multiply less per pair
 #pragma unroll
   for (int k = 0; k < P; ++k) cds[k] = two_inv_a3 * cd[k];
   double W[6] = {0, 0, 0, 0, 0, 0};
@@ -381,7 +381,7 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
         const int nsteps = (hi2 - lo) / kPairStep;
         if (nsteps <= 0) return;
         if constexpr (kPacked) {
-          const float ia2 = (float)inv_a2, nia = -(float)inv_a, t3 = (float)two_inv_a3;
+          const float ia2 = (float)inv_a2, nia = -(float)inv_a;
           const float2 xi2 = make_float2(xs, xs), yi2 = make_float2(ys, ys), zi2 = make_float2(zs, zs);
           const float* fp = sj.f + (lo - base) * 4 + jq * 8;
           int jdx = lo + 2 * jq - selfpos;                  // candidate index minus the lane's own
@@ -403,13 +403,13 @@ k_pair(PairParams<T> prm, const int* __restrict__ pstart, const typename Vec4<T>
             }
             const float2 rinv = make_float2(rsqrt_fast(r2.x), rsqrt_fast(r2.y));
             const float2 sv = __ffma2_rn(r2, make_float2(ia2, ia2), make_float2(-1.f, -1.f));
-            float2 g = make_float2((float)cf[P - 1], (float)cf[P - 1]), dg = make_float2((float)cd[P - 1], (float)cd[P - 1]);
+            float2 g = make_float2((float)cf[P - 1], (float)cf[P - 1]), dg = make_float2((float)cds[P - 1], (float)cds[P - 1]);
 #pragma unroll
             for (int k = P - 2; k >= 0; --k) g = __ffma2_rn(g, sv, make_float2((float)cf[k], (float)cf[k]));
 #pragma unroll
-            for (int k = P - 2; k >= 1; --k) dg = __ffma2_rn(dg, sv, make_float2((float)cd[k], (float)cd[k]));
+            for (int k = P - 2; k >= 1; --k) dg = __ffma2_rn(dg, sv, make_float2((float)cds[k], (float)cds[k]));
             A2.av = __ffma2_rn(qj, __ffma2_rn(g, make_float2(nia, nia), rinv), A2.av);
-            const float2 fs = __fmul2_rn(qj, __ffma2_rn(make_float2(t3, t3), dg, __fmul2_rn(__fmul2_rn(rinv, rinv), rinv)));
+            const float2 fs = __fmul2_rn(qj, __ffma2_rn(__fmul2_rn(rinv, rinv), rinv, dg));   // dg carries 2/a^3
             if (MODE == kPairImage) {
               const float2 fx = __fmul2_rn(fs, dx), fy = __fmul2_rn(fs, dy), fz = __fmul2_rn(fs, dz);
               A2.bx = __ffma2_rn(fs, dx, A2.bx); A2.by = __ffma2_rn(fs, dy, A2.by); A2.bz = __ffma2_rn(fs, dz, A2.bz);
